@@ -1,0 +1,317 @@
+/*
+ * sc_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, obviously-correct CPU implementation of the Sutton-Chen hot path
+ * of arXiv 1210.3559, written from the paper's equations.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call it.  It shares no code, header, table or constant with the CUDA library
+ * (paper_1210_3559_b200/csrc); the unit-conversion literals below are retyped here.
+ *
+ * What it computes (free, non-periodic cluster, all pairs):
+ *   Eq. (2)  rho_i = sum_{j != i} (a / r_ij)^m
+ *            (the extracted text has the garbled index "i != i"; reading Q2: j != i)
+ *   Eq. (1)  U = eps * sum_i [ 1/2 sum_{j != i} (a / r_ij)^n - c sqrt(rho_i) ]
+ *   F_i = -dU/dr_i = eps * sum_{j != i} [ n (a/r)^n - (c m / 2)(rho_i^-1/2 + rho_j^-1/2)(a/r)^m ]
+ *                          * (r_i - r_j) / r^2
+ *            (the paper prints no force formula; this is minus the gradient of Eq. (1),
+ *             pinned by central differences in tests/test_oracle_pins.py; two sweeps
+ *             as in PAPER.md:127 "first sweep calculating all rho_i ... then ... forces")
+ *   velocity-Verlet, dt in fs ("Verlet integrator ... 1 fs"; reading Q3):
+ *            v += (dt/2) ACC F/m ; r += dt v ; recompute F ; v += (dt/2) ACC F/m
+ *   KE = 1/2 m sum |v|^2 / ACC ;  T = 2 KE / (kB (3N - 3))        (reading Q5)
+ *   rescale thermostat after the second half kick: v *= sqrt(T_target / T)   (reading Q6)
+ *   cutoff variant (not in the paper; reading Q7): a pair contributes to
+ *            rho, pair energy and force iff r2 < r_cut*r_cut, strict, where the decision
+ *            value is r2 = fma(dz, dz, fma(dy, dy, dx*dx)) in binary64 with
+ *            dx = x_i - x_j etc. in binary64 -- the one place where the precision of an
+ *            intermediate is fixed, because floating point decides a set membership.
+ *   rho_i == 0 (atom with no neighbour in range, or N = 1): rho^-1/2 := 0, sqrt(rho) := 0
+ *            (reading Q9).  Self term excluded by index (Q11).
+ *
+ * Powers are repeated multiplication, never pow().  No blocking, no fusion, no Newton's-
+ * third-law halving: every ordered pair (i, j) is visited in both sweeps, exactly as the
+ * definition reads.  Rows i are independent, so the OpenMP split over i does not change
+ * any result.
+ *
+ * Two builds of this one file:
+ *   -DSC_ORACLE_LONG_DOUBLE : pair arithmetic and accumulators in x87 80-bit long double.
+ *                             This is the PARITY reference (accurate to ~1e-18 per term).
+ *   (default)               : everything in binary64.  This is the build that is TIMED as
+ *                             the cpu_baseline.  The two must agree to ~1e-13 (tested).
+ *
+ * Parity pins: tests/test_oracle_pins.py (closed-form dimer / triangle / tetrahedron /
+ * icosahedron / cuboctahedron, mpmath brute force, F = -grad E by central differences,
+ * Newton's third law, zero torque, rigid-motion invariance, homogeneity, NVE drift,
+ * time reversal, bulk-limit lattice sums, SURVEY.md's independently computed values).
+ * Nothing here is "parity unpinned" except absolute energies against a published
+ * number -- the paper prints none.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef SC_ORACLE_LONG_DOUBLE
+typedef long double real;
+#define R_SQRT sqrtl
+#else
+typedef double real;
+#define R_SQRT sqrt
+#endif
+
+/* unit system: Angstrom, fs, eV, u, K.  CODATA-2018 (reading Q4). */
+static const double ORACLE_ACC = 9.648533215665e-3;  /* A fs^-2 per (eV A^-1 u^-1) */
+static const double ORACLE_KB = 8.617333262e-5;      /* eV / K */
+
+typedef struct {
+    int32_t n, m;            /* exponents, n > m > 0 */
+    double eps, c, a, mass;  /* eV, -, Angstrom, u */
+    double r_cut;            /* Angstrom; <= 0 means all pairs (the paper's case) */
+} oracle_params;
+
+static real ipow(real u, int k) {
+    real p = u;
+    for (int t = 1; t < k; ++t) p = p * u;
+    return p;
+}
+
+/* cutoff membership, decided in binary64 exactly as the header states */
+static int pair_in_range(const double *pi, const double *pj, double r_cut) {
+    if (r_cut <= 0.0) return 1;
+    double dx = pi[0] - pj[0], dy = pi[1] - pj[1], dz = pi[2] - pj[2];
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    return r2 < r_cut * r_cut;
+}
+
+static real pair_distance(const double *pi, const double *pj, real *d) {
+    d[0] = (real)pi[0] - (real)pj[0];
+    d[1] = (real)pi[1] - (real)pj[1];
+    d[2] = (real)pi[2] - (real)pj[2];
+    return R_SQRT(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+}
+
+/* Eq. (2): rho_i for every i (first sweep). */
+static void density_real(int64_t N, const double *pos, const oracle_params *p, real *rho) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < N; ++i) {
+        real acc = 0;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
+            real d[3];
+            real r = pair_distance(pos + 3 * i, pos + 3 * j, d);
+            real u = (real)p->a / r;
+            acc += ipow(u, p->m);
+        }
+        rho[i] = acc;
+    }
+}
+
+static real inv_sqrt_or_zero(real rho) { return rho > 0 ? (real)1 / R_SQRT(rho) : (real)0; }
+
+/* second sweep for one row i: force on i and sum_j (a/r)^n */
+static void force_row(int64_t N, const double *pos, const oracle_params *p, const real *s,
+                      int64_t i, real f[3], real *pair_sum) {
+    real fx = 0, fy = 0, fz = 0, ps = 0;
+    const real half_cm = (real)p->c * (real)p->m / 2;
+    for (int64_t j = 0; j < N; ++j) {
+        if (j == i) continue;
+        if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
+        real d[3];
+        real r = pair_distance(pos + 3 * i, pos + 3 * j, d);
+        real u = (real)p->a / r;
+        real un = ipow(u, p->n);
+        real um = ipow(u, p->m);
+        real bracket = (real)p->n * un - half_cm * (s[i] + s[j]) * um;
+        real g = (real)p->eps * bracket / (r * r);
+        fx += g * d[0];
+        fy += g * d[1];
+        fz += g * d[2];
+        ps += un;
+    }
+    f[0] = fx; f[1] = fy; f[2] = fz;
+    *pair_sum = ps;
+}
+
+/* Both sweeps.  Any output pointer may be NULL.  Returns 0, or 1 on allocation failure. */
+static int energy_forces_real(int64_t N, const double *pos, const oracle_params *p,
+                              real *rho, real *force /*N*3*/, real *e_pair, real *e_emb) {
+    real *s = (real *)malloc(sizeof(real) * (size_t)(N > 0 ? N : 1));
+    real *ps = (real *)malloc(sizeof(real) * (size_t)(N > 0 ? N : 1));
+    if (!s || !ps) { free(s); free(ps); return 1; }
+    density_real(N, pos, p, rho);
+    for (int64_t i = 0; i < N; ++i) s[i] = inv_sqrt_or_zero(rho[i]);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < N; ++i) {
+        real f[3];
+        force_row(N, pos, p, s, i, f, &ps[i]);
+        if (force) { force[3 * i] = f[0]; force[3 * i + 1] = f[1]; force[3 * i + 2] = f[2]; }
+    }
+    real ep = 0, ee = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        ep += ps[i] / 2;
+        ee += (rho[i] > 0 ? R_SQRT(rho[i]) : (real)0);
+    }
+    if (e_pair) *e_pair = (real)p->eps * ep;
+    if (e_emb) *e_emb = -(real)p->eps * (real)p->c * ee;
+    free(s); free(ps);
+    return 0;
+}
+
+static void kinetic_real(int64_t N, const real *vel, double mass, real *ke, real *temp) {
+    real acc = 0;
+    for (int64_t i = 0; i < 3 * N; ++i) acc += vel[i] * vel[i];
+    real k = (real)mass * acc / 2 / (real)ORACLE_ACC;
+    *ke = k;
+    int64_t ndof = 3 * N - 3;
+    *temp = ndof > 0 ? 2 * k / ((real)ORACLE_KB * (real)ndof) : (real)0;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* exported C entry points (ctypes)                                                       */
+/* ------------------------------------------------------------------------------------ */
+
+int oracle_real_bits(void) { return (int)(sizeof(real) * 8); }
+
+int oracle_density(int64_t N, const double *pos, const oracle_params *p, double *rho_out) {
+    real *rho = (real *)malloc(sizeof(real) * (size_t)(N > 0 ? N : 1));
+    if (!rho) return 1;
+    density_real(N, pos, p, rho);
+    for (int64_t i = 0; i < N; ++i) rho_out[i] = (double)rho[i];
+    free(rho);
+    return 0;
+}
+
+/* rho_out[N], force_out[N*3], energies[3] = {U, U_pair, U_emb}; any may be NULL */
+int oracle_energy_forces(int64_t N, const double *pos, const oracle_params *p,
+                         double *rho_out, double *force_out, double *energies) {
+    size_t n = (size_t)(N > 0 ? N : 1);
+    real *rho = (real *)malloc(sizeof(real) * n);
+    real *f = (real *)malloc(sizeof(real) * 3 * n);
+    if (!rho || !f) { free(rho); free(f); return 1; }
+    real ep, ee;
+    int rc = energy_forces_real(N, pos, p, rho, f, &ep, &ee);
+    if (!rc) {
+        if (rho_out) for (int64_t i = 0; i < N; ++i) rho_out[i] = (double)rho[i];
+        if (force_out) for (int64_t i = 0; i < 3 * N; ++i) force_out[i] = (double)f[i];
+        if (energies) { energies[0] = (double)(ep + ee); energies[1] = (double)ep; energies[2] = (double)ee; }
+    }
+    free(rho); free(f);
+    return rc;
+}
+
+/* Second sweep for a chosen subset of rows, given rho for ALL atoms (from oracle_density).
+ * Lets the full-size parity tests check sampled outputs one by one.
+ * force_out[nrows*3], pair_sum_out[nrows] (= sum_j (a/r)^n for that row). */
+int oracle_forces_rows(int64_t N, const double *pos, const oracle_params *p, const double *rho_all,
+                       const int64_t *rows, int64_t nrows, double *force_out, double *pair_sum_out) {
+    real *s = (real *)malloc(sizeof(real) * (size_t)(N > 0 ? N : 1));
+    if (!s) return 1;
+    for (int64_t i = 0; i < N; ++i) s[i] = inv_sqrt_or_zero((real)rho_all[i]);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < nrows; ++k) {
+        real f[3], ps;
+        force_row(N, pos, p, s, rows[k], f, &ps);
+        force_out[3 * k] = (double)f[0];
+        force_out[3 * k + 1] = (double)f[1];
+        force_out[3 * k + 2] = (double)f[2];
+        if (pair_sum_out) pair_sum_out[k] = (double)ps;
+    }
+    free(s);
+    return 0;
+}
+
+/* First sweep for a chosen subset of rows. */
+int oracle_density_rows(int64_t N, const double *pos, const oracle_params *p,
+                        const int64_t *rows, int64_t nrows, double *rho_out) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < nrows; ++k) {
+        int64_t i = rows[k];
+        real acc = 0;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
+            real d[3];
+            real r = pair_distance(pos + 3 * i, pos + 3 * j, d);
+            acc += ipow((real)p->a / r, p->m);
+        }
+        rho_out[k] = (double)acc;
+    }
+    return 0;
+}
+
+int oracle_kinetic(int64_t N, const double *vel, double mass, double *ke_out, double *temp_out) {
+    real *v = (real *)malloc(sizeof(real) * 3 * (size_t)(N > 0 ? N : 1));
+    if (!v) return 1;
+    for (int64_t i = 0; i < 3 * N; ++i) v[i] = (real)vel[i];
+    real ke, t;
+    kinetic_real(N, v, mass, &ke, &t);
+    *ke_out = (double)ke; *temp_out = (double)t;
+    free(v);
+    return 0;
+}
+
+/* In-range ordered pairs (the cutoff path's "pair interactions"), counted per the header's rule. */
+int64_t oracle_count_pairs(int64_t N, const double *pos, double r_cut) {
+    int64_t total = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : total)
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t j = 0; j < N; ++j)
+            if (j != i && pair_in_range(pos + 3 * i, pos + 3 * j, r_cut)) ++total;
+    return total;
+}
+
+/*
+ * nsteps of velocity-Verlet from (pos, vel), in place.
+ *   thermo_kind 0: NVE.   1: rescale after the second half kick of step k (k = 1..nsteps)
+ *   to T_target(k) = T_start + (T_end - T_start) * k / nsteps   (reading Q6).
+ * Traces (may be NULL), length nsteps + 1, index 0 = initial state:
+ *   epot_trace[k], ekin_trace[k] after step k (after the rescale, if any).
+ * pos_trace (may be NULL): (nsteps+1) * N * 3 positions.
+ * The state is carried in `real` across the whole run.
+ */
+int oracle_run(int64_t N, double *pos, double *vel, const oracle_params *p, double dt, int64_t nsteps,
+               int32_t thermo_kind, double T_start, double T_end,
+               double *epot_trace, double *ekin_trace, double *pos_trace) {
+    size_t n3 = 3 * (size_t)(N > 0 ? N : 1);
+    real *x = (real *)malloc(sizeof(real) * n3);
+    real *v = (real *)malloc(sizeof(real) * n3);
+    real *f = (real *)malloc(sizeof(real) * n3);
+    real *rho = (real *)malloc(sizeof(real) * n3);
+    double *xd = (double *)malloc(sizeof(double) * n3);
+    if (!x || !v || !f || !rho || !xd) { free(x); free(v); free(f); free(rho); free(xd); return 1; }
+    for (int64_t i = 0; i < 3 * N; ++i) { x[i] = (real)pos[i]; v[i] = (real)vel[i]; xd[i] = pos[i]; }
+    real ep, ee, ke, temp;
+    int rc = energy_forces_real(N, xd, p, rho, f, &ep, &ee);
+    if (rc) goto done;
+    kinetic_real(N, v, p->mass, &ke, &temp);
+    if (epot_trace) epot_trace[0] = (double)(ep + ee);
+    if (ekin_trace) ekin_trace[0] = (double)ke;
+    if (pos_trace) memcpy(pos_trace, xd, sizeof(double) * 3 * (size_t)N);
+    const real half_kick = (real)dt / 2 * (real)ORACLE_ACC / (real)p->mass;
+    for (int64_t k = 1; k <= nsteps; ++k) {
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] += half_kick * f[i];
+        for (int64_t i = 0; i < 3 * N; ++i) x[i] += (real)dt * v[i];
+        /* positions are binary64 state at the boundary: round once per step (no-op in the
+         * binary64 build) so that the force routine and the next drift see the same x */
+        for (int64_t i = 0; i < 3 * N; ++i) { xd[i] = (double)x[i]; x[i] = (real)xd[i]; }
+        rc = energy_forces_real(N, xd, p, rho, f, &ep, &ee);
+        if (rc) goto done;
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] += half_kick * f[i];
+        kinetic_real(N, v, p->mass, &ke, &temp);
+        if (thermo_kind == 1) {
+            real target = (real)T_start + ((real)T_end - (real)T_start) * (real)k / (real)nsteps;
+            real lambda = temp > 0 ? R_SQRT(target / temp) : (real)1;
+            for (int64_t i = 0; i < 3 * N; ++i) v[i] *= lambda;
+            kinetic_real(N, v, p->mass, &ke, &temp);
+        }
+        if (epot_trace) epot_trace[k] = (double)(ep + ee);
+        if (ekin_trace) ekin_trace[k] = (double)ke;
+        if (pos_trace) memcpy(pos_trace + (size_t)k * 3 * (size_t)N, xd, sizeof(double) * 3 * (size_t)N);
+    }
+    for (int64_t i = 0; i < 3 * N; ++i) { pos[i] = (double)x[i]; vel[i] = (double)v[i]; }
+done:
+    free(x); free(v); free(f); free(rho); free(xd);
+    return rc;
+}
