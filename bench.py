@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- Sutton-Chen MD hot path on B200: pair interactions/s and MD steps/s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = one pass of the whole hot path over the synthetic cluster: a velocity-Verlet MD step
+(half kick + drift, density sweep, force + energy sweep, half kick + kinetic-energy reduction)
+through libscmd's sc_step.  Default workload: BASELINE.json configs[3], the Ni65536 fcc cluster,
+all pairs, FP64 -- the configuration the metric's roofline target (N >= 65,536) is quoted on.
+Prints ONE JSON line.  N > 1 GPUs = N independent replicas
+(the paper's own use: up to 15 independent trajectories per temperature); the
+only collective is the timing reduction.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_1210_3559_b200 import workloads as W  # noqa: E402
+
+METRIC = "pair_interactions_per_s"
+UNIT = "ordered pairs/s (both sweeps)"
+
+# FP64-pipe instructions per ordered pair in the shipped (9,6) kernels (SASS-counted)
+I_DENSITY = 11
+I_FORCE_ENERGY = 22
+# nominal B200 FP64 peak: 148 SMs x 64 lanes x 2 FLOP x 1.965 GHz
+SM_COUNT, FP64_LANES, SM_MAX_GHZ = 148, 64, 1.965
+FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES * 2 * SM_MAX_GHZ / 1e3
+
+
+def make_workload(name: str, rank: int = 0) -> W.Workload:
+    if name == "Ni65536-fcc-allpairs-fp64":
+        return W.config_c4(seed=4001 + rank)
+    if name == "Ni1415-fcc-allpairs-fp64":
+        return W.config_c2(seed=2001 + rank)
+    if name == "Ni8000-liquid-allpairs-fp64":
+        return W.config_c3(seed=3001 + rank)
+    if name == "Ni147-mackay-allpairs-fp64":
+        return W.config_c1(seed=1001 + rank)
+    if name.startswith("Ni") and name.endswith("-fcc-sweep-fp64"):
+        n = int(name[2:].split("-")[0])
+        return W.fcc_cluster(n, 1500.0, 5000 + int(round(np.log2(n) / 2)) + rank)
+    raise SystemExit(f"unknown workload {name}")
+
+
+# ------------------------------------------------------------------------------------------- #
+# clocks
+# ------------------------------------------------------------------------------------------- #
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------- #
+# distributed plumbing (replicas only; the timing reduction is the one collective)
+# ------------------------------------------------------------------------------------------- #
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate(local_ms: float, local_units: float, world: int, backend_device="cuda"):
+    """-> (max over ranks of the timed milliseconds, sum over ranks of the units processed)."""
+    if world == 1:
+        return local_ms, local_units
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([local_ms], dtype=torch.float64, device=backend_device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------------------------- #
+# reference arm / cpu baseline: the oracle as it stands, on host cores, bounded sample
+# ------------------------------------------------------------------------------------------- #
+def oracle_sample_rows(n_atoms: int, target_pair_passes: float = 2.5e9) -> np.ndarray:
+    """Rows of the workload the CPU baseline evaluates: evenly spaced, sized for ~10-30 s."""
+    nrows = int(max(1, min(n_atoms, target_pair_passes / (2.0 * n_atoms))))
+    return np.unique(np.linspace(0, n_atoms - 1, nrows).astype(np.int64))
+
+
+def oracle_time_sample(w: W.Workload, rows: np.ndarray):
+    """Both sweeps of the binary64 oracle build for `rows` (all j): seconds, ordered pairs."""
+    from oracle.sc_oracle import Oracle
+    o = Oracle("plain")
+    P = o.params()
+    rho_all = np.full(w.n_atoms, 100.0)          # timing only: any positive density works as s_j input
+    t0 = time.perf_counter()
+    rho_rows = o.density_rows(w.pos, P, rows)
+    rho_all[rows] = rho_rows
+    o.forces_rows(w.pos, P, rho_all, rows)
+    dt = time.perf_counter() - t0
+    return dt, float(rows.size) * (w.n_atoms - 1)
+
+
+def cpu_baseline(w: W.Workload) -> dict:
+    rows = oracle_sample_rows(w.n_atoms)
+    dt, pairs = oracle_time_sample(w, rows)
+    return {"value": pairs / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+            "seconds": dt,
+            "sample": f"{rows.size} evenly spaced rows i of {w.name} (all j, both sweeps), binary64 oracle build, OpenMP"}
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w = make_workload(args.workload)
+    rows = oracle_sample_rows(w.n_atoms, target_pair_passes=6e8)
+    for _ in range(args.warmup):
+        oracle_time_sample(w, rows)
+    total_s, total_pairs = 0.0, 0.0
+    for _ in range(args.steps):
+        dt, pairs = oracle_time_sample(w, rows)
+        total_s += dt; total_pairs += pairs
+    value = total_pairs / total_s
+    sample = (f"each step = {rows.size} evenly spaced rows i of {w.name} (all j, both sweeps), "
+              f"binary64 oracle build, OpenMP on {os.cpu_count()} host cores")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "n_atoms": w.n_atoms},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------- #
+# our arm
+# ------------------------------------------------------------------------------------------- #
+def run_ours(args):
+    import torch
+    import paper_1210_3559_b200 as scmd
+
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank if world > 1 else 0)
+    torch.cuda.set_device(dev)
+    scmd.load_library()
+
+    w = make_workload(args.workload, rank)
+    N = w.n_atoms
+    pairs_per_step = float(N) * (N - 1)
+    sc = scmd.SuttonChen(N)
+    d_pos = torch.as_tensor(w.pos, device=dev)
+    d_vel = torch.as_tensor(w.vel, device=dev)
+    sc.sc_set_state(d_pos, d_vel)
+    sc.sc_profile(True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def one_step():
+        sc.sc_step(1.0, 1)
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()
+    launches0 = sc.sc_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ms_force, ms_density = [], []
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        flush.zero_()                                                  # L2 flush, outside the timed events
+        ev[k][0].record(stream)
+        one_step()
+        ev[k][1].record(stream)
+        prof = sc.sc_profile_read()                                    # synchronises
+        ms_force.append(prof["ms_force"]); ms_density.append(prof["ms_density"])
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = sc.sc_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    local_ms = sum(a.elapsed_time(b) for a, b in ev)
+    total_ms, total_pairs = aggregate(local_ms, pairs_per_step * args.steps, world)
+    value = total_pairs / (total_ms * 1e-3)
+
+    # end to end through the host-buffer entry point: upload positions, both sweeps, download
+    # forces + energy (pinned host memory), every step
+    h_pos = torch.as_tensor(w.pos).pin_memory()
+    h_force = torch.empty(N, 3, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        sc.sc_eval_host(h_pos, h_force)
+    torch.cuda.synchronize()
+    e2e_steps = max(3, min(args.steps, 10))
+    t_e2e = 0.0
+    for _ in range(e2e_steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sc.sc_eval_host(h_pos, h_force)                                # returns after the D2H copy
+        t_e2e += time.perf_counter() - t0
+    e2e_ms, e2e_pairs = aggregate(t_e2e * 1e3, pairs_per_step * e2e_steps, world)
+
+    if rank != 0:
+        return
+    t_force = statistics.mean(ms_force) * 1e-3
+    t_density = statistics.mean(ms_density) * 1e-3
+    achieved = I_FORCE_ENERGY * 2.0 * pairs_per_step / t_force / 1e12
+    try:
+        dfma_rate, probe_mhz = scmd.probe_throughput(0)
+        peak_measured = dfma_rate * 2.0 / 1e12
+    except Exception:
+        peak_measured, probe_mhz = None, None
+    traffic = None
+    tfile = ROOT / "profiles" / "roofline_traffic.json"
+    if tfile.exists():
+        traffic = json.loads(tfile.read_text()).get(args.workload, {}).get("force_sweep_dram_bytes_per_launch")
+    roofline = {"bound": "alu", "kernel": "allpairs64_kernel<force+energy>", "achieved": achieved,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
+                "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no FP64 figure",
+                "peak_measured_dfma_probe": peak_measured, "probe_sm_mhz": probe_mhz,
+                "fp64_inst_per_pair": I_FORCE_ENERGY, "ms_force_sweep": t_force * 1e3,
+                "ms_density_sweep": t_density * 1e3,
+                "density_sweep_frac": I_DENSITY * 2.0 * pairs_per_step / t_density / 1e12 / FP64_PEAK_TFLOPS,
+                "both_sweeps_frac": (I_DENSITY + I_FORCE_ENERGY) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / FP64_PEAK_TFLOPS}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "md_steps_per_s": world * args.steps / (total_ms * 1e-3),
+            "config": {"workload": args.workload, "n_atoms": N, "pairs_per_step": pairs_per_step,
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "flushed between timed steps (256 MiB memset outside the per-step events)",
+                       "step": "sc_step(dt=1 fs, nsteps=1): kick+drift, density sweep, force+energy sweep, kick+KE"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * N,
+                    "d2h_bytes_per_step": 24 * N + 16, "call": "sc_eval_host (pinned host buffers)",
+                    "ms_per_call": e2e_ms / e2e_steps},
+            "roofline": roofline, "cpu_baseline": cpu_baseline(w)}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="Ni65536-fcc-allpairs-fp64")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

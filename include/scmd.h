@@ -1,0 +1,182 @@
+/*
+ * scmd.h -- C ABI of libscmd: the Sutton-Chen molecular-dynamics hot path of
+ * arXiv 1210.3559 (Yakubovich et al., "Kinetics of liquid-solid phase transition in
+ * large nickel clusters") for one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes, for a free (non-periodic) cluster of N atoms at r_i:
+ *
+ *   rho_i = sum_{j != i} (a / r_ij)^m                               Eq. (2)
+ *   U     = eps * sum_i [ 1/2 sum_{j != i} (a / r_ij)^n - c sqrt(rho_i) ]   Eq. (1)
+ *   F_i   = -dU/dr_i = eps * sum_{j != i} [ n (a/r_ij)^n
+ *             - (c m / 2) (rho_i^-1/2 + rho_j^-1/2) (a/r_ij)^m ] (r_i - r_j) / r_ij^2
+ *           evaluated as two sweeps over pairs -- first all rho_i, then the forces --
+ *           exactly as PAPER.md:127 reduces the many-body term;
+ *   velocity-Verlet time stepping, dt in fs ("Verlet integrator with a
+ *           time-step of 1 fs"), optionally followed by a velocity-rescale thermostat
+ *           (BASELINE.json config 3; the paper's Langevin thermostat, is
+ *           listed as SC_THERMO_LANGEVIN and not implemented yet).
+ *   Parameters for nickel: eps = 1.5707e-2 eV, a = 3.52 A, c = 39.432,
+ *           n = 9, m = 6.  The paper runs all pairs with no cutoff; r_cut > 0
+ *           selects the cell-list / Verlet-list variant BASELINE.json adds: a pair counts in
+ *           rho, energy and force iff r_ij^2 < r_cut^2 (strict, plain truncation).
+ *
+ * Units: Angstrom, fs, eV, atomic mass unit u, Kelvin.
+ *   acceleration = F * SC_ACC / mass,  SC_ACC = 9.648533215665e-3 A fs^-2 per (eV A^-1 u^-1)
+ *   KE = 1/2 mass sum |v|^2 / SC_ACC,  T = 2 KE / (kB (3N - 3)),  kB = 8.617333262e-5 eV/K
+ *   (T := 0 for N = 1).
+ *
+ * Pointers: a name starting with d_ is DEVICE memory, h_ is HOST memory.  All arrays are
+ * binary64, contiguous, atom-major (N x 3: x0 y0 z0 x1 ...).  The caller owns every buffer
+ * it passes, including the workspace, and must keep the workspace alive and untouched
+ * until sc_destroy.  The library allocates no device memory of its own.
+ *
+ * Stream: every call enqueues on the cudaStream_t given to sc_create and returns without
+ * waiting, except the calls that return a host scalar or copy to host memory
+ * (sc_energy, sc_kinetic, sc_stats, sc_eval_host, sc_step_host), which synchronise that stream.
+ *
+ * Errors: every call returns an sc_status; nothing is thrown across the ABI and nothing is
+ * printed.  sc_last_error gives a human-readable message for the last failing call on a ctx.
+ * There is no CPU fallback: without a CUDA device sc_create returns SC_ERR_CUDA.
+ */
+#ifndef SCMD_H_
+#define SCMD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sc_ctx sc_ctx; /* opaque; created by sc_create, freed by sc_destroy */
+
+typedef struct {
+    int32_t n, m;           /* exponents of Eq. (1)/(2); n > m > 0              */
+    double eps, c, a;       /* eV, dimensionless, Angstrom                      */
+    double mass;            /* u; BASELINE.json fixes 58.69 for Ni (the paper states none)    */
+    double r_cut;           /* Angstrom; <= 0 selects all pairs (the paper's case)            */
+} sc_params;
+
+typedef enum {
+    SC_OK = 0,
+    SC_ERR_INVALID = 1,     /* bad argument: n <= m, m <= 0, N < 1, eps/a/mass <= 0, dt <= 0,
+                               skin < 0, NULL pointer, unknown precision / thermostat kind    */
+    SC_ERR_CUDA = 2,        /* a CUDA runtime call failed, or no device                        */
+    SC_ERR_NOMEM = 3,       /* workspace smaller than sc_workspace_bytes                       */
+    SC_ERR_STATE = 4,       /* call needs state that was never set (positions / velocities)   */
+    SC_ERR_NONFINITE = 5,   /* a returned scalar is NaN or +-inf (e.g. coincident atoms)       */
+    SC_ERR_CAPACITY = 6     /* a neighbour row overflowed its capacity (never truncated)      */
+} sc_status;
+
+typedef enum {
+    SC_PREC_FP64 = 0,       /* pair arithmetic and accumulation in binary64                    */
+    SC_PREC_MIXED = 1       /* pair arithmetic in binary32 on split (hi + lo) coordinates,
+                               accumulation in binary64                                        */
+} sc_precision;
+
+typedef enum { SC_THERMO_NONE = 0, SC_THERMO_RESCALE = 1, SC_THERMO_LANGEVIN = 2 } sc_thermo_kind;
+
+typedef struct {
+    int32_t kind;           /* sc_thermo_kind; SC_THERMO_LANGEVIN returns SC_ERR_INVALID (next) */
+    double T_start, T_end;  /* K; step k = 1..nsteps of ONE sc_step call is rescaled, after its
+                               second half kick, to T_start + (T_end - T_start) * k / nsteps    */
+    double gamma;           /* 1/fs; Langevin only                                              */
+    uint64_t seed;          /* Langevin only                                                    */
+} sc_thermostat;
+
+/* Runtime options (sc_set_option).  Values are integers; 0 always means "library default". */
+typedef enum {
+    SC_OPT_ROWS_PER_THREAD = 1,   /* i-atoms held in registers per thread: 1, 2 or 4           */
+    SC_OPT_LANES_PER_ROW = 2,     /* lanes of a warp that share one row group: 1,2,4,8,16,32    */
+    SC_OPT_WARPS_PER_CTA = 3,     /* consumer warps per CTA (they split the j range): 1..8      */
+    SC_OPT_PERSISTENT = 4,        /* 1: whole sc_step loop in one cooperative kernel (small N);
+                                     2: never; 0: choose by N                                    */
+    SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
+    SC_OPT_NEIGHBOUR_CAPACITY = 6 /* K_max rows of the Verlet list (cutoff path)                */
+} sc_option;
+
+/* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */
+size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t precision, double skin);
+
+/*
+ * Create a context for n_atoms atoms.
+ *   precision        sc_precision
+ *   skin             Angstrom, >= 0; Verlet-list skin for r_cut > 0 (list radius r_cut + skin,
+ *                    rebuilt when any atom has moved more than skin / 2 since the last build);
+ *                    ignored for r_cut <= 0
+ *   d_workspace      device memory, 256-byte aligned, workspace_bytes long, caller-owned
+ *   cuda_stream      a cudaStream_t (NULL = legacy default stream)
+ *   out              receives the context
+ */
+sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
+                    void *d_workspace, size_t workspace_bytes, void *cuda_stream, sc_ctx **out);
+sc_status sc_destroy(sc_ctx *ctx);
+sc_status sc_set_option(sc_ctx *ctx, int32_t option, int64_t value);
+
+/* Copy positions (required) and velocities (d_vel may be NULL: velocities unset) in. */
+sc_status sc_set_state(sc_ctx *ctx, const double *d_pos, const double *d_vel);
+/* Copy positions / velocities out, in the caller's atom order; either pointer may be NULL. */
+sc_status sc_get_state(sc_ctx *ctx, double *d_pos, double *d_vel);
+
+/* First sweep, Eq. (2): d_rho[N]. */
+sc_status sc_density(sc_ctx *ctx, double *d_rho);
+/* Both sweeps: d_force[N*3] in eV/A.  Also refreshes the cached energy. */
+sc_status sc_forces(sc_ctx *ctx, double *d_force);
+/* Eq. (1): potential energy in eV of the current positions -> *h_epot.
+ * Runs the sweeps if the cached value is stale.  SC_ERR_NONFINITE if not finite. */
+sc_status sc_energy(sc_ctx *ctx, double *h_epot);
+/* Kinetic energy (eV) and temperature (K) of the current velocities. */
+sc_status sc_kinetic(sc_ctx *ctx, double *h_ke, double *h_temperature);
+/* nsteps velocity-Verlet steps of dt_fs femtoseconds; thermostat NULL = NVE.
+ * SC_ERR_STATE if velocities were never set. */
+sc_status sc_step(sc_ctx *ctx, double dt_fs, const sc_thermostat *thermostat, int64_t nsteps);
+/* Cutoff-path bookkeeping since sc_create: number of list builds; in-range ordered pairs
+ * (r_ij^2 < r_cut^2) at the last force evaluation (N(N-1) for all pairs); longest neighbour
+ * row at the last build.  Any pointer may be NULL. */
+sc_status sc_stats(sc_ctx *ctx, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int64_t *max_neighbours);
+
+/*
+ * Host-buffer entry points (the end-to-end path): copies are part of the call.
+ * sc_eval_host: upload h_pos[N*3], run both sweeps, download h_force[N*3], h_rho[N] (either
+ *   may be NULL) and the potential energy *h_epot (may be NULL).
+ * sc_step_host: upload h_pos, h_vel, run nsteps, download both in place, and write
+ *   h_scalars[3] = { U, KE, T } of the final state (may be NULL).
+ */
+sc_status sc_eval_host(sc_ctx *ctx, const double *h_pos, double *h_force, double *h_rho, double *h_epot);
+sc_status sc_step_host(sc_ctx *ctx, double *h_pos, double *h_vel, double dt_fs,
+                       const sc_thermostat *thermostat, int64_t nsteps, double *h_scalars);
+
+/* Launch accounting: kernels this context has launched since creation. */
+sc_status sc_launch_count(sc_ctx *ctx, int64_t *n_launches);
+/* Sweep timing for bench.py's roofline line.  After sc_profile(ctx, 1) every force evaluation
+ * that runs both sweeps records CUDA events on the ctx stream around each sweep;
+ * sc_profile_read synchronises and returns the milliseconds of the most recent one
+ * (SC_ERR_STATE if none was recorded). */
+sc_status sc_profile(sc_ctx *ctx, int32_t enable);
+sc_status sc_profile_read(sc_ctx *ctx, double *h_ms_density, double *h_ms_force);
+
+/*
+ * Diagnostics that need no context.  d_scratch: caller-owned device memory, >= 64 KiB.
+ *
+ * sc_probe_throughput: register-only dependent-FMA-chain kernel on every SM; reports
+ *   thread-level instructions per second and the SM clock (MHz) held during the run.
+ *   kind 0: FP64 DFMA   1: FP32 FFMA   2: packed FP32x2 FMA (counted as 2 per lane)
+ *        3: MUFU.RSQ (binary32)        4: FP64 reciprocal seed (MUFU.RCP64H)
+ *   bench.py prints the measured figure beside the nominal ALU peak.
+ * sc_probe_reciprocal: maximum relative error, over n_samples log-uniform x in [lo, hi], of
+ *   h_err4 = { rcp seed, refined 1/x, rsqrt seed, refined x^-1/2 } as used by the FP64 sweeps,
+ *   against IEEE division / sqrt on the device.
+ * Both synchronise the stream.
+ */
+sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, size_t scratch_bytes,
+                              double *h_inst_per_s, double *h_sm_clock_mhz);
+sc_status sc_probe_reciprocal(double lo, double hi, int32_t n_samples, void *cuda_stream, void *d_scratch,
+                              size_t scratch_bytes, double *h_err4);
+
+const char *sc_last_error(const sc_ctx *ctx);
+const char *sc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCMD_H_ */

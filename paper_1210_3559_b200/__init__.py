@@ -1,0 +1,14 @@
+"""paper_1210_3559_b200 -- thin Python binding over libscmd (include/scmd.h).
+
+Argument marshalling only: every step of the Sutton-Chen hot path (density sweep, force +
+energy sweep, velocity-Verlet, thermostat) runs in the CUDA
+kernels under csrc/.  PyTorch is used for device memory and streams.  There is no CPU
+fallback: if libscmd.so is missing or no CUDA device is present, calls raise.
+"""
+from .binding import (  # noqa: F401
+    SC_OK, SC_PREC_FP64, SC_PREC_MIXED, SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN,
+    SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
+    SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY,
+    ScError, ScParams, ScThermostat, SuttonChen, load_library, library_path, exported_symbols,
+    probe_throughput, probe_reciprocal, NI_PARAMS,
+)

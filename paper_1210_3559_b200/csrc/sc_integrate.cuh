@@ -1,0 +1,146 @@
+// sc_integrate.cuh -- O(N) kernels around the sweeps: state packing, velocity-Verlet kicks and
+// drift (reading Q3), kinetic-energy / temperature reduction, rescale thermostat
+// (reading Q6), fixed-order scalar reductions.  All streaming, 24..72 B per atom.
+#pragma once
+#include "sc_device.cuh"
+
+namespace scmd {
+
+constexpr double kAcc = 9.648533215665e-3;   // A fs^-2 per (eV A^-1 u^-1), CODATA-2018 e / u
+constexpr double kBoltzmann = 8.617333262e-5;   // eV / K
+
+// device scalar slots (double scal[kNumScalars])
+enum ScalarSlot {
+    kSlotEPair = 0,     // U_pair (eV)
+    kSlotEEmb = 1,      // U_emb (eV)
+    kSlotKE = 2,        // kinetic energy (eV)
+    kSlotTemp = 3,      // temperature (K)
+    kSlotLambda = 4,    // pending velocity scale of the rescale thermostat (1 = none)
+    kSlotMaxDisp2 = 5,  // max squared displacement since the last list build (cutoff path)
+    kNumScalars = 16
+};
+
+// pos[N*3] -> xs[N] = (x, y, z, 0)
+__global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, int N) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) xs[i] = make_double4(pos[3 * size_t(i)], pos[3 * size_t(i) + 1], pos[3 * size_t(i) + 2], 0.0);
+}
+__global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *__restrict__ pos, int N) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) {
+        const double4 p = xs[i];
+        pos[3 * size_t(i)] = p.x; pos[3 * size_t(i) + 1] = p.y; pos[3 * size_t(i) + 2] = p.z;
+    }
+}
+
+// first half kick + drift:  v <- lambda v (pending thermostat scale);  v += hk F;  x += dt v
+// (hk = dt/2 * ACC / m).  ref (may be NULL): positions at the last list build; the largest squared
+// displacement from it goes to scal[kSlotMaxDisp2] through an integer atomicMax (order-free).
+__global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__ vel, const double *__restrict__ force,
+                                  double *__restrict__ scal, const double4 *__restrict__ ref, int N, double hk,
+                                  double dt) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double d2 = 0.0;
+    if (i < N) {
+        const double lambda = scal[kSlotLambda];
+        double4 p = xs[i];
+        double vx = vel[3 * size_t(i)] * lambda, vy = vel[3 * size_t(i) + 1] * lambda, vz = vel[3 * size_t(i) + 2] * lambda;
+        vx = fma(hk, force[3 * size_t(i)], vx);
+        vy = fma(hk, force[3 * size_t(i) + 1], vy);
+        vz = fma(hk, force[3 * size_t(i) + 2], vz);
+        p.x = fma(dt, vx, p.x); p.y = fma(dt, vy, p.y); p.z = fma(dt, vz, p.z);
+        vel[3 * size_t(i)] = vx; vel[3 * size_t(i) + 1] = vy; vel[3 * size_t(i) + 2] = vz;
+        xs[i] = p;
+        if (ref) {
+            const double4 r = ref[i];
+            const double ex = p.x - r.x, ey = p.y - r.y, ez = p.z - r.z;
+            d2 = fma(ez, ez, fma(ey, ey, ex * ex));
+        }
+    }
+    if (ref) {
+        // non-negative doubles order like their bit patterns
+        unsigned long long bits = __double_as_longlong(d2);
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            unsigned long long o = __shfl_xor_sync(0xffffffffu, bits, off);
+            bits = o > bits ? o : bits;
+        }
+        if ((threadIdx.x & 31) == 0 && bits != 0ull)
+            atomicMax(reinterpret_cast<unsigned long long *>(scal + kSlotMaxDisp2), bits);
+    }
+}
+
+// second half kick + per-block sum of |v|^2 -> part[blockIdx.x]
+__global__ void kick_ke_kernel(double *__restrict__ vel, const double *__restrict__ force, double *__restrict__ part,
+                               int N, double hk) {
+    __shared__ double scratch[32];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double v2 = 0.0;
+    if (i < N) {
+        double vx = fma(hk, force[3 * size_t(i)], vel[3 * size_t(i)]);
+        double vy = fma(hk, force[3 * size_t(i) + 1], vel[3 * size_t(i) + 1]);
+        double vz = fma(hk, force[3 * size_t(i) + 2], vel[3 * size_t(i) + 2]);
+        vel[3 * size_t(i)] = vx; vel[3 * size_t(i) + 1] = vy; vel[3 * size_t(i) + 2] = vz;
+        v2 = fma(vz, vz, fma(vy, vy, vx * vx));
+    }
+    const double t = block_sum(v2, scratch);
+    if (threadIdx.x == 0) part[blockIdx.x] = t;
+}
+
+// per-block sum of |v|^2 without a kick (sc_kinetic)
+__global__ void sum_v2_kernel(const double *__restrict__ vel, double *__restrict__ part, int N, double lambda_apply,
+                              const double *__restrict__ scal) {
+    __shared__ double scratch[32];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double v2 = 0.0;
+    if (i < N) {
+        const double l = lambda_apply != 0.0 ? scal[kSlotLambda] : 1.0;
+        const double vx = vel[3 * size_t(i)] * l, vy = vel[3 * size_t(i) + 1] * l, vz = vel[3 * size_t(i) + 2] * l;
+        v2 = fma(vz, vz, fma(vy, vy, vx * vx));
+    }
+    const double t = block_sum(v2, scratch);
+    if (threadIdx.x == 0) part[blockIdx.x] = t;
+}
+
+// v <- lambda v, lambda <- 1  (flushes a pending thermostat scale)
+__global__ void scale_velocities_kernel(double *__restrict__ vel, const double *__restrict__ scal, int n3) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n3) vel[i] *= scal[kSlotLambda];
+}
+__global__ void reset_lambda_kernel(double *__restrict__ scal) { scal[kSlotLambda] = 1.0; }
+
+// one block: fixed-order sum of part[0..n) -> scal[slot] = scale * sum
+__global__ void reduce_partials_kernel(const double *__restrict__ part, int n, double *__restrict__ scal, int slot,
+                                       double scale) {
+    __shared__ double scratch[32];
+    double v = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) v += part[k];
+    const double t = block_sum(v, scratch);
+    if (threadIdx.x == 0) scal[slot] = scale * t;
+}
+
+// one block: KE and T from the per-block |v|^2 sums; optionally the rescale factor for T_target
+//   KE = 1/2 m sum|v|^2 / ACC ;  T = 2 KE / (kB ndof) ;  lambda = sqrt(T_target / T)
+// After a rescale the stored KE and T are those of the rescaled velocities.
+__global__ void reduce_ke_kernel(const double *__restrict__ part, int n, double *__restrict__ scal, double mass,
+                                 double ndof, int thermo, double t_target) {
+    __shared__ double scratch[32];
+    double v = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) v += part[k];
+    const double t = block_sum(v, scratch);
+    if (threadIdx.x == 0) {
+        double ke = 0.5 * mass * t / kAcc;
+        double temp = ndof > 0.0 ? 2.0 * ke / (kBoltzmann * ndof) : 0.0;
+        double lambda = 1.0;
+        if (thermo == 1 && temp > 0.0) {
+            lambda = sqrt(t_target / temp);
+            ke *= lambda * lambda;
+            temp = ndof > 0.0 ? 2.0 * ke / (kBoltzmann * ndof) : 0.0;
+        }
+        scal[kSlotKE] = ke;
+        scal[kSlotTemp] = temp;
+        scal[kSlotLambda] = lambda;
+    }
+}
+
+}  // namespace scmd

@@ -1,0 +1,120 @@
+// sc_probe.cuh -- register-only throughput probes (sc_probe_throughput): dependent FMA chains
+// with 8-way ILP per thread, one wave of resident CTAs on every SM.  Gives the measured figure
+// that bench.py prints beside the nominal ALU peak, and the SM clock held under that load.
+#pragma once
+#include "sc_device.cuh"
+
+namespace scmd {
+
+constexpr int kProbeChains = 8;
+
+template <int KIND>
+__global__ void __launch_bounds__(256) probe_kernel(double *out, long long *cycles, int iters, double seed) {
+    const long long t0 = clock64();
+    double sink = 0.0;
+    if constexpr (KIND == 0) {                       // DFMA
+        double a[kProbeChains];
+        const double b = 1.0 + seed * 1e-9, c = seed * 1e-12;
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) a[k] = seed + k + threadIdx.x;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) a[k] = fma(a[k], b, c);
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) sink += a[k];
+    } else if constexpr (KIND == 1) {                // FFMA
+        float a[kProbeChains];
+        const float b = 1.0f + float(seed) * 1e-6f, c = float(seed) * 1e-7f;
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) a[k] = float(seed) + k + threadIdx.x;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) a[k] = fmaf(a[k], b, c);
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) sink += a[k];
+    } else if constexpr (KIND == 2) {                // packed FP32x2 FMA
+        unsigned long long a[kProbeChains];
+        const float bf = 1.0f + float(seed) * 1e-6f, cf = float(seed) * 1e-7f;
+        unsigned long long b, c;
+        asm("mov.b64 %0, {%1, %1};" : "=l"(b) : "f"(bf));
+        asm("mov.b64 %0, {%1, %1};" : "=l"(c) : "f"(cf));
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) {
+            const float v = float(seed) + k + threadIdx.x;
+            asm("mov.b64 %0, {%1, %1};" : "=l"(a[k]) : "f"(v));
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k)
+                asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a[k]) : "l"(b), "l"(c));
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) {
+            float lo, hi;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a[k]));
+            sink += lo + hi;
+        }
+    } else if constexpr (KIND == 3) {                // MUFU.RSQ (binary32)
+        float a[kProbeChains];
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) a[k] = float(seed) + 1.5f + k + threadIdx.x;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) asm("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(a[k]));
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) sink += a[k];
+    } else {                                         // MUFU.RCP64H
+        double a[kProbeChains];
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) a[k] = seed + 1.5 + k + threadIdx.x;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) a[k] = rcp_seed(a[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) sink += a[k];
+    }
+    const long long t1 = clock64();
+    if (sink == 123.456) out[0] = sink;              // keep the chains alive
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+// accuracy check of the FP64 reciprocal building blocks (test helper, no context needed):
+// out[0..3] = max relative error of rcp seed, rcp_fast, rsqrt seed, rsqrt_fast over n samples
+// log-uniform in [lo, hi]; reference = IEEE division / sqrt in device code
+__global__ void reciprocal_error_kernel(double lo, double hi, int n, double *out4) {
+    __shared__ double scratch[4][32];
+    double e0 = 0, e1 = 0, e2 = 0, e3 = 0;
+    const double lr = log(hi / lo);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        // golden-ratio sequence in [0, 1)
+        double u = i * 0.6180339887498949;
+        u -= floor(u);
+        const double x = lo * exp(lr * u);
+        const double r = 1.0 / x, q = 1.0 / sqrt(x);
+        e0 = fmax(e0, fabs(rcp_seed(x) - r) / r);
+        e1 = fmax(e1, fabs(rcp_fast(x) - r) / r);
+        e2 = fmax(e2, fabs(rsqrt_seed(x) - q) / q);
+        e3 = fmax(e3, fabs(rsqrt_fast(x) - q) / q);
+    }
+    double e[4] = {e0, e1, e2, e3};
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        for (int off = 16; off > 0; off >>= 1) e[k] = fmax(e[k], __shfl_xor_sync(0xffffffffu, e[k], off));
+        if (lane == 0) scratch[k][warp] = e[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double m = 0;
+        for (int w = 0; w < (blockDim.x >> 5); ++w) m = fmax(m, scratch[threadIdx.x][w]);
+        // non-negative doubles order like their bit patterns
+        atomicMax(reinterpret_cast<unsigned long long *>(out4 + threadIdx.x),
+                  (unsigned long long)__double_as_longlong(m));
+    }
+}
+
+}  // namespace scmd

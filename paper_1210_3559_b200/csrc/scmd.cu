@@ -1,0 +1,599 @@
+// scmd.cu -- host side of libscmd: context, workspace carving, kernel selection and launches.
+// The C ABI is declared and documented in include/scmd.h.
+#include "../../include/scmd.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "sc_allpairs.cuh"
+#include "sc_device.cuh"
+#include "sc_integrate.cuh"
+#include "sc_probe.cuh"
+
+using namespace scmd;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr int kBlock = 256;          // O(N) kernels
+
+struct Carver {
+    unsigned char *base;
+    size_t off = 0;
+    explicit Carver(void *b) : base(static_cast<unsigned char *>(b)) {}
+    template <class T>
+    T *take(size_t count) {
+        off = (off + kAlign - 1) / kAlign * kAlign;
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+    size_t total() const { return (off + kAlign - 1) / kAlign * kAlign; }
+};
+
+inline int ceil_div(int64_t a, int64_t b) { return int((a + b - 1) / b); }
+
+}  // namespace
+
+struct sc_ctx {
+    sc_params p{};
+    int64_t N = 0;
+    int32_t precision = 0;
+    double skin = 0.0;
+    cudaStream_t stream = nullptr;
+    char err[512] = {0};
+    int sm_count = 148;
+
+    // device arrays (all inside the caller's workspace)
+    double4 *xs = nullptr;        // [N] (x, y, z, s')
+    double *vel = nullptr;        // [N*3]
+    double *force = nullptr;      // [N*3]
+    double *rho = nullptr;        // [N]
+    double *part_a = nullptr;     // [max CTAs] per-CTA partials, sweep 1
+    double *part_b = nullptr;     // [max CTAs] per-CTA partials, sweep 2
+    double *part_ke = nullptr;    // [ceil(N/kBlock)]
+    double *scal = nullptr;       // [kNumScalars]
+    double *stage_a = nullptr;    // [N*3] host-path staging
+    double *stage_b = nullptr;    // [N*3]
+
+    PairConsts consts{};
+    bool have_pos = false, have_vel = false;
+    bool density_valid = false, forces_valid = false, energy_valid = false;
+    bool lambda_pending = false;
+    int64_t launches = 0;
+
+    // options (0 = default)
+    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0;
+
+    // profiling
+    bool profile = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    double ms_density = 0, ms_force = 0, ms_other = 0;
+};
+
+namespace {
+
+sc_status fail(sc_ctx *c, sc_status st, const char *fmt, const char *detail = "") {
+    if (c) snprintf(c->err, sizeof(c->err), fmt, detail);
+    return st;
+}
+
+#define SC_CUDA_CHECK(ctx, call)                                                     \
+    do {                                                                             \
+        cudaError_t e_ = (call);                                                     \
+        if (e_ != cudaSuccess) return fail((ctx), SC_ERR_CUDA, #call ": %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+bool params_ok(const sc_params *p) {
+    return p && p->n > p->m && p->m > 0 && p->n <= 64 && p->eps > 0.0 && p->a > 0.0 && p->mass > 0.0 &&
+           std::isfinite(p->eps) && std::isfinite(p->a) && std::isfinite(p->c) && std::isfinite(p->mass) &&
+           std::isfinite(p->r_cut);
+}
+
+// one place that lays the workspace out; base == nullptr only measures
+size_t carve(sc_ctx *c, void *base, int64_t N) {
+    Carver w(base);
+    const size_t n = size_t(N);
+    double4 *xs = w.take<double4>(n + kTileAtoms);
+    double *vel = w.take<double>(3 * n);
+    double *force = w.take<double>(3 * n);
+    double *rho = w.take<double>(n);
+    double *pa = w.take<double>(n + 1);
+    double *pb = w.take<double>(n + 1);
+    double *pk = w.take<double>(size_t(ceil_div(N, kBlock)) + 1);
+    double *scal = w.take<double>(kNumScalars);
+    double *sa = w.take<double>(3 * n);
+    double *sb = w.take<double>(3 * n);
+    if (c && base) {
+        c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
+        c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
+    }
+    return w.total();
+}
+
+double ipow_host(double u, int k) {
+    double r = 1.0;
+    for (int t = 0; t < k; ++t) r *= u;
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------
+// all-pairs kernel selection
+// ---------------------------------------------------------------------------------------------
+struct TileChoice { int it, tpr, warps; };
+
+TileChoice choose_tile(const sc_ctx *c) {
+    const int64_t N = c->N;
+    // largest rows-per-CTA that still gives >= 4 CTAs per SM; prefer 2 rows per thread
+    const int64_t want_ctas = int64_t(4) * c->sm_count;
+    int rpc = 1;
+    while (rpc < 64 && N / (rpc * 2) >= want_ctas) rpc *= 2;
+    int it = rpc >= 2 ? 2 : 1;
+    int tpr = 32 * it / rpc;
+    if (tpr > 32) { tpr = 32; it = 1; }
+    int warps = 8;
+    // keep at least ~8 pairs per lane and tile
+    while (warps > 1 && N / (int64_t(warps) * tpr) < 8) warps /= 2;
+    if (c->opt_it) it = c->opt_it;
+    if (c->opt_tpr) tpr = c->opt_tpr;
+    if (c->opt_warps) warps = c->opt_warps;
+    return {it, tpr, warps};
+}
+
+template <int IT, int TPR, int NE, int ME>
+cudaError_t launch_allpairs_t(const AllPairsArgs &args, bool force, bool energy, int warps, int grid, cudaStream_t st) {
+    const size_t smem = allpairs_smem_bytes(IT, TPR, warps);
+    const dim3 block((warps + 1) * 32);
+    auto go = [&](auto kernel) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+        if (e != cudaSuccess) return e;
+        kernel<<<grid, block, smem, st>>>(args);
+        return cudaGetLastError();
+    };
+    if (!force) return go(allpairs64_kernel<IT, TPR, NE, ME, false, false>);
+    if (energy) return go(allpairs64_kernel<IT, TPR, NE, ME, true, true>);
+    return go(allpairs64_kernel<IT, TPR, NE, ME, true, false>);
+}
+
+template <int NE, int ME>
+cudaError_t launch_allpairs_nm(const TileChoice &tc, const AllPairsArgs &a, bool force, bool energy, int grid,
+                               cudaStream_t st) {
+#define SC_CASE(IT, TPR) \
+    if (tc.it == IT && tc.tpr == TPR) return launch_allpairs_t<IT, TPR, NE, ME>(a, force, energy, tc.warps, grid, st);
+    SC_CASE(1, 1) SC_CASE(1, 2) SC_CASE(1, 4) SC_CASE(1, 8) SC_CASE(1, 16) SC_CASE(1, 32)
+    SC_CASE(2, 1) SC_CASE(2, 2) SC_CASE(2, 4) SC_CASE(2, 8) SC_CASE(2, 16) SC_CASE(2, 32)
+    if constexpr (NE != 0) { SC_CASE(4, 1) SC_CASE(4, 2) SC_CASE(4, 4) }
+#undef SC_CASE
+    return cudaErrorInvalidConfiguration;
+}
+
+sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
+    TileChoice tc = choose_tile(c);
+    const bool fast = (c->p.n == 9 && c->p.m == 6);
+    if (!fast && tc.it > 2) tc.it = 2;
+    const int rpc = allpairs_rows_per_cta(tc.it, tc.tpr);
+    const int grid = ceil_div(c->N, rpc);
+    AllPairsArgs a{};
+    a.xs = c->xs; a.n_atoms = int(c->N); a.rho = c->rho; a.force = c->force;
+    a.partial = force ? c->part_b : c->part_a;
+    a.c = c->consts;
+    cudaError_t e = fast ? launch_allpairs_nm<9, 6>(tc, a, force, energy, grid, c->stream)
+                         : launch_allpairs_nm<0, 0>(tc, a, force, energy, grid, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "all-pairs sweep launch: %s", cudaGetErrorString(e));
+    c->launches += 1;
+    if (!force || energy) {
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
+                                                         force ? c->consts.En : -c->consts.eps_c);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return SC_OK;
+}
+
+sc_status ensure_density(sc_ctx *c) {
+    if (c->density_valid) return SC_OK;
+    sc_status st = run_sweep(c, false, false);
+    if (st == SC_OK) c->density_valid = true;
+    return st;
+}
+
+sc_status ensure_forces(sc_ctx *c, bool energy) {
+    if (c->forces_valid && (!energy || c->energy_valid)) return SC_OK;
+    if (c->profile) cudaEventRecord(c->ev[0], c->stream);
+    sc_status st = ensure_density(c);
+    if (st != SC_OK) return st;
+    if (c->profile) cudaEventRecord(c->ev[1], c->stream);
+    st = run_sweep(c, true, energy);
+    if (st != SC_OK) return st;
+    if (c->profile) cudaEventRecord(c->ev[2], c->stream);
+    c->forces_valid = true;
+    if (energy) c->energy_valid = true;
+    return SC_OK;
+}
+
+sc_status flush_lambda(sc_ctx *c) {
+    if (!c->lambda_pending) return SC_OK;
+    const int n3 = int(3 * c->N);
+    scale_velocities_kernel<<<ceil_div(n3, kBlock), kBlock, 0, c->stream>>>(c->vel, c->scal, n3);
+    reset_lambda_kernel<<<1, 1, 0, c->stream>>>(c->scal);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 2;
+    c->lambda_pending = false;
+    return SC_OK;
+}
+
+sc_status read_scalars(sc_ctx *c, double *host, int count) {
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(host, c->scal, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return SC_OK;
+}
+
+sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps) {
+    if (!c->have_pos || !c->have_vel) return fail(c, SC_ERR_STATE, "sc_step: positions and velocities must be set%s");
+    if (!(dt > 0.0) || !std::isfinite(dt) || nsteps < 0) return fail(c, SC_ERR_INVALID, "sc_step: dt must be > 0, nsteps >= 0%s");
+    int thermo = SC_THERMO_NONE;
+    if (th) {
+        thermo = th->kind;
+        if (thermo == SC_THERMO_LANGEVIN) return fail(c, SC_ERR_INVALID, "sc_step: Langevin thermostat is not implemented%s");
+        if (thermo != SC_THERMO_NONE && thermo != SC_THERMO_RESCALE) return fail(c, SC_ERR_INVALID, "sc_step: unknown thermostat kind%s");
+        if (thermo == SC_THERMO_RESCALE && !(th->T_start >= 0.0 && th->T_end >= 0.0))
+            return fail(c, SC_ERR_INVALID, "sc_step: thermostat temperatures must be >= 0%s");
+    }
+    if (nsteps == 0) return SC_OK;
+    sc_status st = ensure_forces(c, false);
+    if (st != SC_OK) return st;
+    const int N = int(c->N);
+    const int nb = ceil_div(N, kBlock);
+    const double hk = 0.5 * dt * kAcc / c->p.mass;
+    const double ndof = double(3 * c->N - 3);
+    for (int64_t k = 1; k <= nsteps; ++k) {
+        kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, nullptr, N, hk, dt);
+        c->launches += 1;
+        c->density_valid = c->forces_valid = c->energy_valid = false;
+        const bool last = (k == nsteps);
+        st = ensure_forces(c, last || c->opt_energy_every == 1);
+        if (st != SC_OK) return st;
+        kick_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk);
+        c->launches += 1;
+        if (thermo == SC_THERMO_RESCALE || last) {
+            const double target = thermo == SC_THERMO_RESCALE
+                                      ? th->T_start + (th->T_end - th->T_start) * double(k) / double(nsteps)
+                                      : 0.0;
+            reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->part_ke, nb, c->scal, c->p.mass, ndof, thermo, target);
+            c->launches += 1;
+            if (thermo == SC_THERMO_RESCALE) c->lambda_pending = true;
+        }
+    }
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    return flush_lambda(c);
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+const char *sc_version(void) { return "libscmd 0.1 (sm_100a)"; }
+
+const char *sc_last_error(const sc_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t precision, double skin) {
+    if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return 0;
+    if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
+    if (!(skin >= 0.0)) return 0;
+    return carve(nullptr, nullptr, n_atoms);
+}
+
+sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin, void *d_workspace,
+                    size_t workspace_bytes, void *cuda_stream, sc_ctx **out) {
+    if (!out) return SC_ERR_INVALID;
+    *out = nullptr;
+    if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return SC_ERR_INVALID;
+    if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return SC_ERR_INVALID;
+    if (!(skin >= 0.0) || !d_workspace) return SC_ERR_INVALID;
+    if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
+    if (precision == SC_PREC_MIXED) return SC_ERR_INVALID;     // not built yet
+    if (params->r_cut > 0.0) return SC_ERR_INVALID;            // not built yet
+    const size_t need = sc_workspace_bytes(params, n_atoms, precision, skin);
+    if (workspace_bytes < need) return SC_ERR_NOMEM;
+    int dev = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) return SC_ERR_CUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
+    sc_ctx *c = new (std::nothrow) sc_ctx();
+    if (!c) return SC_ERR_NOMEM;
+    c->p = *params; c->N = n_atoms; c->precision = precision; c->skin = skin;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    carve(c, d_workspace, n_atoms);
+    const double a_n = ipow_host(params->a, params->n), a_m = ipow_host(params->a, params->m);
+    c->consts.am = a_m;
+    c->consts.An = params->eps * params->n * a_n;
+    c->consts.Bm = params->eps * (params->c * params->m / 2.0) * a_m;
+    c->consts.En = params->eps / 2.0 * a_n;
+    c->consts.eps_c = params->eps * params->c;
+    c->consts.n = params->n; c->consts.m = params->m;
+    for (auto &e : c->ev)
+        if (cudaEventCreate(&e) != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    // scalars: zero, lambda = 1; pad the record array tail so that full-tile reads stay defined
+    if (cudaMemsetAsync(c->scal, 0, sizeof(double) * kNumScalars, c->stream) != cudaSuccess ||
+        cudaMemsetAsync(c->xs, 0, sizeof(double4) * (size_t(n_atoms) + kTileAtoms), c->stream) != cudaSuccess) {
+        delete c;
+        return SC_ERR_CUDA;
+    }
+    reset_lambda_kernel<<<1, 1, 0, c->stream>>>(c->scal);
+    if (cudaGetLastError() != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    *out = c;
+    return SC_OK;
+}
+
+sc_status sc_destroy(sc_ctx *ctx) {
+    if (!ctx) return SC_ERR_INVALID;
+    cudaStreamSynchronize(ctx->stream);
+    for (auto &e : ctx->ev)
+        if (e) cudaEventDestroy(e);
+    delete ctx;
+    return SC_OK;
+}
+
+sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
+    if (!c) return SC_ERR_INVALID;
+    auto pow2_le32 = [](int64_t v) { return v == 1 || v == 2 || v == 4 || v == 8 || v == 16 || v == 32; };
+    switch (option) {
+        case SC_OPT_ROWS_PER_THREAD:
+            if (value != 0 && value != 1 && value != 2 && value != 4) return fail(c, SC_ERR_INVALID, "rows per thread must be 0, 1, 2 or 4%s");
+            c->opt_it = int(value); break;
+        case SC_OPT_LANES_PER_ROW:
+            if (value != 0 && !pow2_le32(value)) return fail(c, SC_ERR_INVALID, "lanes per row must be a power of two <= 32%s");
+            c->opt_tpr = int(value); break;
+        case SC_OPT_WARPS_PER_CTA:
+            if (value < 0 || value > kMaxConsumerWarps) return fail(c, SC_ERR_INVALID, "warps per CTA must be 0..8%s");
+            c->opt_warps = int(value); break;
+        case SC_OPT_PERSISTENT:
+            if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "persistent must be 0, 1 or 2%s");
+            c->opt_persistent = int(value); break;
+        case SC_OPT_ENERGY_EVERY_STEP:
+            c->opt_energy_every = value ? 1 : 0; break;
+        case SC_OPT_NEIGHBOUR_CAPACITY:
+            if (value < 0) return fail(c, SC_ERR_INVALID, "neighbour capacity must be >= 0%s");
+            c->opt_kmax = int(value); break;
+        default:
+            return fail(c, SC_ERR_INVALID, "unknown option%s");
+    }
+    if (c->opt_it == 4 && c->opt_tpr > 4) return fail(c, SC_ERR_INVALID, "4 rows per thread needs lanes per row <= 4%s");
+    return SC_OK;
+}
+
+sc_status sc_set_state(sc_ctx *c, const double *d_pos, const double *d_vel) {
+    if (!c || !d_pos) return fail(c, SC_ERR_INVALID, "sc_set_state: d_pos is NULL%s");
+    const int N = int(c->N);
+    pack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(d_pos, c->xs, N);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_pos = true;
+    c->density_valid = c->forces_valid = c->energy_valid = false;
+    if (d_vel) {
+        sc_status st = flush_lambda(c);
+        if (st != SC_OK) return st;
+        SC_CUDA_CHECK(c, cudaMemcpyAsync(c->vel, d_vel, sizeof(double) * 3 * size_t(N), cudaMemcpyDeviceToDevice, c->stream));
+        c->have_vel = true;
+    }
+    return SC_OK;
+}
+
+sc_status sc_get_state(sc_ctx *c, double *d_pos, double *d_vel) {
+    if (!c) return SC_ERR_INVALID;
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_get_state: no positions set%s");
+    const int N = int(c->N);
+    if (d_pos) {
+        unpack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->xs, d_pos, N);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    if (d_vel) {
+        if (!c->have_vel) return fail(c, SC_ERR_STATE, "sc_get_state: no velocities set%s");
+        SC_CUDA_CHECK(c, cudaMemcpyAsync(d_vel, c->vel, sizeof(double) * 3 * size_t(N), cudaMemcpyDeviceToDevice, c->stream));
+    }
+    return SC_OK;
+}
+
+sc_status sc_density(sc_ctx *c, double *d_rho) {
+    if (!c || !d_rho) return fail(c, SC_ERR_INVALID, "sc_density: NULL argument%s");
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_density: no positions set%s");
+    sc_status st = ensure_density(c);
+    if (st != SC_OK) return st;
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(d_rho, c->rho, sizeof(double) * size_t(c->N), cudaMemcpyDeviceToDevice, c->stream));
+    return SC_OK;
+}
+
+sc_status sc_forces(sc_ctx *c, double *d_force) {
+    if (!c || !d_force) return fail(c, SC_ERR_INVALID, "sc_forces: NULL argument%s");
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_forces: no positions set%s");
+    sc_status st = ensure_forces(c, true);
+    if (st != SC_OK) return st;
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(d_force, c->force, sizeof(double) * 3 * size_t(c->N), cudaMemcpyDeviceToDevice, c->stream));
+    return SC_OK;
+}
+
+sc_status sc_energy(sc_ctx *c, double *h_epot) {
+    if (!c || !h_epot) return fail(c, SC_ERR_INVALID, "sc_energy: NULL argument%s");
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_energy: no positions set%s");
+    if (!c->energy_valid) { c->forces_valid = false; }
+    sc_status st = ensure_forces(c, true);
+    if (st != SC_OK) return st;
+    double s[2];
+    st = read_scalars(c, s, 2);
+    if (st != SC_OK) return st;
+    *h_epot = s[kSlotEPair] + s[kSlotEEmb];
+    if (!std::isfinite(*h_epot)) return fail(c, SC_ERR_NONFINITE, "sc_energy: potential energy is not finite (coincident atoms?)%s");
+    return SC_OK;
+}
+
+sc_status sc_kinetic(sc_ctx *c, double *h_ke, double *h_temperature) {
+    if (!c || (!h_ke && !h_temperature)) return fail(c, SC_ERR_INVALID, "sc_kinetic: NULL argument%s");
+    if (!c->have_vel) return fail(c, SC_ERR_STATE, "sc_kinetic: no velocities set%s");
+    sc_status st = flush_lambda(c);
+    if (st != SC_OK) return st;
+    const int N = int(c->N), nb = ceil_div(N, kBlock);
+    sum_v2_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->part_ke, N, 0.0, c->scal);
+    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->part_ke, nb, c->scal, c->p.mass, double(3 * c->N - 3), 0, 0.0);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 2;
+    double s[kSlotTemp + 1];
+    st = read_scalars(c, s, kSlotTemp + 1);
+    if (st != SC_OK) return st;
+    if (h_ke) *h_ke = s[kSlotKE];
+    if (h_temperature) *h_temperature = s[kSlotTemp];
+    if (!std::isfinite(s[kSlotKE])) return fail(c, SC_ERR_NONFINITE, "sc_kinetic: kinetic energy is not finite%s");
+    return SC_OK;
+}
+
+sc_status sc_step(sc_ctx *c, double dt_fs, const sc_thermostat *thermostat, int64_t nsteps) {
+    if (!c) return SC_ERR_INVALID;
+    return do_step(c, dt_fs, thermostat, nsteps);
+}
+
+sc_status sc_stats(sc_ctx *c, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int64_t *max_neighbours) {
+    if (!c) return SC_ERR_INVALID;
+    if (n_rebuilds) *n_rebuilds = 0;
+    if (n_pairs_in_cut) *n_pairs_in_cut = c->N * (c->N - 1);
+    if (max_neighbours) *max_neighbours = c->N - 1;
+    return SC_OK;
+}
+
+sc_status sc_eval_host(sc_ctx *c, const double *h_pos, double *h_force, double *h_rho, double *h_epot) {
+    if (!c || !h_pos) return fail(c, SC_ERR_INVALID, "sc_eval_host: h_pos is NULL%s");
+    const size_t n = size_t(c->N);
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_a, h_pos, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, c->stream));
+    sc_status st = sc_set_state(c, c->stage_a, nullptr);
+    if (st != SC_OK) return st;
+    st = ensure_forces(c, true);
+    if (st != SC_OK) return st;
+    if (h_force) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_force, c->force, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+    if (h_rho) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_rho, c->rho, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    double s[2];
+    st = read_scalars(c, s, 2);
+    if (st != SC_OK) return st;
+    if (h_epot) *h_epot = s[kSlotEPair] + s[kSlotEEmb];
+    if (!std::isfinite(s[0] + s[1])) return fail(c, SC_ERR_NONFINITE, "sc_eval_host: potential energy is not finite%s");
+    return SC_OK;
+}
+
+sc_status sc_step_host(sc_ctx *c, double *h_pos, double *h_vel, double dt_fs, const sc_thermostat *thermostat,
+                       int64_t nsteps, double *h_scalars) {
+    if (!c || !h_pos || !h_vel) return fail(c, SC_ERR_INVALID, "sc_step_host: NULL state pointer%s");
+    const size_t n = size_t(c->N);
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_a, h_pos, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->stage_b, h_vel, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, c->stream));
+    sc_status st = sc_set_state(c, c->stage_a, c->stage_b);
+    if (st != SC_OK) return st;
+    st = do_step(c, dt_fs, thermostat, nsteps);
+    if (st != SC_OK) return st;
+    st = ensure_forces(c, true);
+    if (st != SC_OK) return st;
+    st = sc_get_state(c, c->stage_a, nullptr);
+    if (st != SC_OK) return st;
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(h_pos, c->stage_a, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(h_vel, c->vel, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+    if (h_scalars) {
+        double ke = 0, temp = 0;
+        st = sc_kinetic(c, &ke, &temp);
+        if (st != SC_OK) return st;
+        double s[2];
+        st = read_scalars(c, s, 2);
+        if (st != SC_OK) return st;
+        h_scalars[0] = s[0] + s[1]; h_scalars[1] = ke; h_scalars[2] = temp;
+        if (!std::isfinite(h_scalars[0])) return fail(c, SC_ERR_NONFINITE, "sc_step_host: potential energy is not finite%s");
+    } else {
+        SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    }
+    return SC_OK;
+}
+
+sc_status sc_launch_count(sc_ctx *c, int64_t *n_launches) {
+    if (!c || !n_launches) return SC_ERR_INVALID;
+    *n_launches = c->launches;
+    return SC_OK;
+}
+
+sc_status sc_profile(sc_ctx *c, int32_t enable) {
+    if (!c) return SC_ERR_INVALID;
+    c->profile = enable != 0;
+    return SC_OK;
+}
+
+sc_status sc_profile_read(sc_ctx *c, double *h_ms_density, double *h_ms_force) {
+    if (!c) return SC_ERR_INVALID;
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    float a = 0.f, b = 0.f;
+    if (cudaEventElapsedTime(&a, c->ev[0], c->ev[1]) != cudaSuccess ||
+        cudaEventElapsedTime(&b, c->ev[1], c->ev[2]) != cudaSuccess)
+        return fail(c, SC_ERR_STATE, "sc_profile_read: no profiled sweep recorded%s");
+    if (h_ms_density) *h_ms_density = a;
+    if (h_ms_force) *h_ms_force = b;
+    return SC_OK;
+}
+
+sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, size_t scratch_bytes,
+                              double *h_inst_per_s, double *h_sm_clock_mhz) {
+    if (kind < 0 || kind > 4 || !d_scratch || !h_inst_per_s) return SC_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = sms * 8, block = 256;
+    if (scratch_bytes < sizeof(double) * 8 + sizeof(long long) * size_t(grid)) return SC_ERR_NOMEM;
+    double *out = static_cast<double *>(d_scratch);
+    long long *cyc = reinterpret_cast<long long *>(out + 8);
+    const int iters = (kind >= 3) ? 2048 : 16384;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return SC_ERR_CUDA;
+    auto run = [&](int it) {
+        switch (kind) {
+            case 0: probe_kernel<0><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 1: probe_kernel<1><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 2: probe_kernel<2><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 3: probe_kernel<3><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            default: probe_kernel<4><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+        }
+    };
+    run(iters / 8);   // warm-up
+    run(iters);
+    cudaEventRecord(e0, st);
+    run(iters);
+    cudaEventRecord(e1, st);
+    sc_status rc = SC_OK;
+    float ms = 0.f;
+    long long cycles0 = 0;
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess ||
+        cudaMemcpy(&cycles0, cyc, sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess)
+        rc = SC_ERR_CUDA;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (rc != SC_OK) return rc;
+    const double per_thread = double(iters) * kProbeChains * (kind == 2 ? 2.0 : 1.0);
+    *h_inst_per_s = per_thread * double(grid) * block / (double(ms) * 1e-3);
+    // a block's own span in SM cycles; 8 blocks per SM run concurrently, so span ~ kernel time
+    if (h_sm_clock_mhz) *h_sm_clock_mhz = double(cycles0) / (double(ms) * 1e3);
+    return SC_OK;
+}
+
+sc_status sc_probe_reciprocal(double lo, double hi, int32_t n_samples, void *cuda_stream, void *d_scratch,
+                              size_t scratch_bytes, double *h_err4) {
+    if (!(lo > 0.0) || !(hi > lo) || n_samples < 1 || !d_scratch || scratch_bytes < 4 * sizeof(double) || !h_err4)
+        return SC_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double *out = static_cast<double *>(d_scratch);
+    if (cudaMemsetAsync(out, 0, 4 * sizeof(double), st) != cudaSuccess) return SC_ERR_CUDA;
+    reciprocal_error_kernel<<<296, 256, 0, st>>>(lo, hi, n_samples, out);
+    if (cudaGetLastError() != cudaSuccess) return SC_ERR_CUDA;
+    if (cudaMemcpyAsync(h_err4, out, 4 * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess) return SC_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return SC_ERR_CUDA;
+    return SC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,59 @@
+"""CPU-side checks of the C ABI: libscmd.so loads and exports every symbol include/scmd.h
+declares; argument validation that needs no GPU.  No compute calls here."""
+import ctypes
+
+import pytest
+
+import paper_1210_3559_b200 as pkg
+from paper_1210_3559_b200 import build as pkg_build
+
+
+@pytest.fixture(scope="module")
+def lib():
+    pkg_build.build()
+    return pkg.load_library()
+
+
+def test_header_symbols_are_all_exported(lib):
+    names = pkg.exported_symbols()
+    must = {"sc_create", "sc_destroy", "sc_density", "sc_forces", "sc_energy", "sc_step", "sc_kinetic",
+            "sc_set_state", "sc_get_state", "sc_workspace_bytes", "sc_stats", "sc_eval_host", "sc_step_host",
+            "sc_last_error", "sc_set_option", "sc_launch_count", "sc_probe_throughput"}
+    assert must <= set(names)
+    for name in names:
+        assert hasattr(lib, name), f"{name} declared in include/scmd.h but not exported by libscmd.so"
+
+
+def test_version_string(lib):
+    assert b"libscmd" in lib.sc_version()
+
+
+def test_workspace_bytes_validation(lib):
+    P = pkg.ScParams(9, 6, 1.5707e-2, 39.432, 3.52, 58.69, 0.0)
+    n1 = lib.sc_workspace_bytes(ctypes.byref(P), 1415, pkg.SC_PREC_FP64, 0.0)
+    n2 = lib.sc_workspace_bytes(ctypes.byref(P), 65536, pkg.SC_PREC_FP64, 0.0)
+    assert 0 < n1 < n2 < 64 * 1024 * 1024
+    assert lib.sc_workspace_bytes(ctypes.byref(P), 0, pkg.SC_PREC_FP64, 0.0) == 0          # N < 1
+    assert lib.sc_workspace_bytes(ctypes.byref(P), 100, 7, 0.0) == 0                       # precision
+    assert lib.sc_workspace_bytes(ctypes.byref(P), 100, pkg.SC_PREC_FP64, -1.0) == 0       # skin < 0
+    bad = pkg.ScParams(6, 9, 1.5707e-2, 39.432, 3.52, 58.69, 0.0)                          # n <= m
+    assert lib.sc_workspace_bytes(ctypes.byref(bad), 100, pkg.SC_PREC_FP64, 0.0) == 0
+    bad = pkg.ScParams(9, 6, -1.0, 39.432, 3.52, 58.69, 0.0)                               # eps <= 0
+    assert lib.sc_workspace_bytes(ctypes.byref(bad), 100, pkg.SC_PREC_FP64, 0.0) == 0
+
+
+def test_create_rejects_bad_arguments_without_a_device(lib):
+    P = pkg.ScParams(9, 6, 1.5707e-2, 39.432, 3.52, 58.69, 0.0)
+    ctx = ctypes.c_void_p()
+    assert lib.sc_create(ctypes.byref(P), 100, 0, 0.0, None, 1 << 20, None, ctypes.byref(ctx)) == pkg.binding.SC_ERR_INVALID
+    assert lib.sc_create(ctypes.byref(P), 100, 0, 0.0, 4096 + 8, 1 << 20, None, ctypes.byref(ctx)) == pkg.binding.SC_ERR_INVALID
+    assert lib.sc_create(ctypes.byref(P), 100, 0, 0.0, 4096, 16, None, ctypes.byref(ctx)) == pkg.binding.SC_ERR_NOMEM
+    assert not ctx.value
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(pkg.ScError):
+        pkg.SuttonChen(147)
