@@ -79,7 +79,11 @@ class ClockSampler:
 
     def _pump(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.time(), line.strip()))
+
+    def mark(self):
+        """Samples taken before this call are dropped (warm-up)."""
+        self.t_mark = time.time()
 
     def stop(self) -> dict:
         if self.proc is None:
@@ -91,7 +95,10 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.lines:
+        t_mark = getattr(self, "t_mark", 0.0)
+        for stamp, line in self.lines:
+            if stamp < t_mark:
+                continue
             parts = [p.strip() for p in line.split(",")]
             if len(parts) < 7:
                 continue
@@ -214,14 +221,15 @@ def run_ours(args):
     def one_step():
         sc.sc_step(1.0, 1)
 
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()                                                # samples before mark() are dropped
     for _ in range(max(args.warmup, 3)):
         one_step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    sampler = ClockSampler(dev.index or 0)
-    if rank == 0:
-        sampler.start()
+    sampler.mark()
     launches0 = sc.sc_launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     ms_force, ms_density = [], []
@@ -300,7 +308,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="Ni65536-fcc-allpairs-fp64")

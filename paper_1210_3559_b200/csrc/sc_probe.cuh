@@ -10,7 +10,8 @@ constexpr int kProbeChains = 8;
 
 template <int KIND>
 __global__ void __launch_bounds__(256) probe_kernel(double *out, long long *cycles, int iters, double seed) {
-    const long long t0 = clock64();
+    long long t0;
+    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t0) :: "memory");
     double sink = 0.0;
     if constexpr (KIND == 0) {                       // DFMA
         double a[kProbeChains];
@@ -77,7 +78,8 @@ __global__ void __launch_bounds__(256) probe_kernel(double *out, long long *cycl
 #pragma unroll
         for (int k = 0; k < kProbeChains; ++k) sink += a[k];
     }
-    const long long t1 = clock64();
+    long long t1;
+    asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1) : "d"(sink) : "memory");   // ordered after the chains
     if (sink == 123.456) out[0] = sink;              // keep the chains alive
     if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
