@@ -9,6 +9,7 @@
 #include <new>
 
 #include "sc_allpairs.cuh"
+#include "sc_cutoff.cuh"
 #include "sc_device.cuh"
 #include "sc_integrate.cuh"
 #include "sc_probe.cuh"
@@ -59,6 +60,19 @@ struct sc_ctx {
     double *stage_a = nullptr;    // [N*3] host-path staging
     double *stage_b = nullptr;    // [N*3]
 
+    // cutoff path (r_cut > 0); all null otherwise
+    bool cutoff = false;
+    double r_list = 0.0;
+    int kmax = 0, kmax_cap = 0, npad = 0, max_dim = 1, coop_grid = 0;
+    bool list_checked = false;    // rebuild_kernel already launched for the current positions
+    double4 *xs_alt = nullptr, *xs_ref = nullptr;
+    double *vel_alt = nullptr, *blockpart = nullptr;
+    int *perm = nullptr, *perm_alt = nullptr, *cell_of = nullptr, *slot_of = nullptr, *cell_sorted = nullptr;
+    int *cell_count = nullptr, *cell_start = nullptr, *order_tmp = nullptr, *order = nullptr;
+    int *nlist = nullptr, *ncount = nullptr;
+    CellGrid *grid = nullptr;
+    unsigned long long *counters = nullptr;
+
     PairConsts consts{};
     bool have_pos = false, have_vel = false;
     bool density_valid = false, forces_valid = false, energy_valid = false;
@@ -93,8 +107,28 @@ bool params_ok(const sc_params *p) {
            std::isfinite(p->r_cut);
 }
 
+constexpr int kMaxCoopBlocks = 4096;
+
+inline int round_up(int64_t v, int64_t q) { return int((v + q - 1) / q * q); }
+
+// default neighbour-row capacity: 1.3 x the fcc number density 4 / a^3 inside the list sphere
+int default_kmax(const sc_params *p, int64_t N, double skin) {
+    const double rl = p->r_cut + skin;
+    const double est = 1.3 * (4.0 / (p->a * p->a * p->a)) * (4.0 / 3.0) * 3.14159265358979323846 * rl * rl * rl;
+    int64_t k = int64_t(est) + 1;
+    if (k > N - 1) k = N - 1;
+    if (k < 1) k = 1;
+    return round_up(k, 32);
+}
+int cutoff_max_dim(int64_t N) {
+    const int64_t cap = N / 4 + 512;
+    int d = 1;
+    while (int64_t(d + 1) * (d + 1) * (d + 1) <= cap) ++d;
+    return d;
+}
+
 // one place that lays the workspace out; base == nullptr only measures
-size_t carve(sc_ctx *c, void *base, int64_t N) {
+size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, double skin) {
     Carver w(base);
     const size_t n = size_t(N);
     double4 *xs = w.take<double4>(n + kTileAtoms);
@@ -110,6 +144,27 @@ size_t carve(sc_ctx *c, void *base, int64_t N) {
     if (c && base) {
         c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
+    }
+    if (prm->r_cut > 0.0) {
+        const int kmax = default_kmax(prm, N, skin), npad = round_up(N, 32), md = cutoff_max_dim(N);
+        const size_t ncell = size_t(md) * md * md + 2;
+        double4 *xa = w.take<double4>(n + kTileAtoms);
+        double4 *xr = w.take<double4>(n);
+        double *va = w.take<double>(3 * n);
+        double *bp = w.take<double>(9 * size_t(kMaxCoopBlocks));
+        int *perm = w.take<int>(n), *perm_alt = w.take<int>(n), *cell_of = w.take<int>(n), *slot_of = w.take<int>(n);
+        int *cell_sorted = w.take<int>(n), *order_tmp = w.take<int>(n), *order = w.take<int>(n), *ncount = w.take<int>(n);
+        int *cell_count = w.take<int>(ncell), *cell_start = w.take<int>(ncell);
+        int *nlist = w.take<int>(size_t(kmax) * size_t(npad));
+        CellGrid *grid = w.take<CellGrid>(1);
+        unsigned long long *counters = w.take<unsigned long long>(kNumCounters);
+        if (c && base) {
+            c->xs_alt = xa; c->xs_ref = xr; c->vel_alt = va; c->blockpart = bp; c->perm = perm; c->perm_alt = perm_alt;
+            c->cell_of = cell_of; c->slot_of = slot_of; c->cell_sorted = cell_sorted; c->order_tmp = order_tmp;
+            c->order = order; c->ncount = ncount; c->cell_count = cell_count; c->cell_start = cell_start;
+            c->nlist = nlist; c->grid = grid; c->counters = counters;
+            c->kmax = c->kmax_cap = kmax; c->npad = npad; c->max_dim = md;
+        }
     }
     return w.total();
 }
@@ -170,7 +225,106 @@ cudaError_t launch_allpairs_nm(const TileChoice &tc, const AllPairsArgs &a, bool
     return cudaErrorInvalidConfiguration;
 }
 
+// ---------------------------------------------------------------------------------------------
+// cutoff path: rebuild + list-driven sweeps
+// ---------------------------------------------------------------------------------------------
+sc_status ensure_list(sc_ctx *c) {
+    if (!c->cutoff || c->list_checked) return SC_OK;
+    RebuildArgs a{};
+    a.xs = c->xs; a.xs_alt = c->xs_alt; a.xs_ref = c->xs_ref; a.vel = c->vel; a.vel_alt = c->vel_alt;
+    a.perm = c->perm; a.perm_alt = c->perm_alt; a.cell_of = c->cell_of; a.slot_of = c->slot_of;
+    a.cell_sorted = c->cell_sorted; a.cell_count = c->cell_count; a.cell_start = c->cell_start;
+    a.order_tmp = c->order_tmp; a.order = c->order; a.nlist = c->nlist; a.ncount = c->ncount;
+    a.blockpart = c->blockpart; a.grid = c->grid; a.scal = c->scal; a.counters = c->counters;
+    a.n_atoms = int(c->N); a.npad = c->npad; a.kmax = c->kmax; a.max_dim = c->max_dim;
+    a.have_vel = c->have_vel ? 1 : 0;
+    a.r_list = c->r_list; a.half_skin2 = 0.25 * c->skin * c->skin;
+    void *params[] = {&a};
+    cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void *>(rebuild_kernel), dim3(c->coop_grid), dim3(256),
+                                                params, 0, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "rebuild_kernel launch: %s", cudaGetErrorString(e));
+    c->launches += 1;
+    c->list_checked = true;
+    return SC_OK;
+}
+
+int choose_tpa(const sc_ctx *c) {
+    if (c->opt_tpr) return c->opt_tpr;
+    int tpa = 1;
+    while (tpa < 32 && c->N * tpa < int64_t(c->sm_count) * 1024) tpa *= 2;
+    return tpa;
+}
+
+template <int TPA, int NE, int ME>
+cudaError_t launch_nlist_t(const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
+    const int atoms_per_block = kNlistBlock / TPA;
+    const int grid = ceil_div(a.n_atoms, atoms_per_block);
+    auto go = [&](auto kernel) -> cudaError_t {
+        kernel<<<grid, kNlistBlock, 0, st>>>(a);
+        return cudaGetLastError();
+    };
+    if (!mixed) {
+        if (!force) return go(nlist_kernel<TPA, NE, ME, false, false, false>);
+        if (energy) return go(nlist_kernel<TPA, NE, ME, true, true, false>);
+        return go(nlist_kernel<TPA, NE, ME, true, false, false>);
+    }
+    if (!force) return go(nlist_kernel<TPA, NE, ME, false, false, true>);
+    if (energy) return go(nlist_kernel<TPA, NE, ME, true, true, true>);
+    return go(nlist_kernel<TPA, NE, ME, true, false, true>);
+}
+
+template <int NE, int ME>
+cudaError_t launch_nlist_nm(int tpa, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
+    switch (tpa) {
+        case 1: return launch_nlist_t<1, NE, ME>(a, force, energy, mixed, st);
+        case 2: return launch_nlist_t<2, NE, ME>(a, force, energy, mixed, st);
+        case 4: return launch_nlist_t<4, NE, ME>(a, force, energy, mixed, st);
+        case 8: return launch_nlist_t<8, NE, ME>(a, force, energy, mixed, st);
+        case 16: return launch_nlist_t<16, NE, ME>(a, force, energy, mixed, st);
+        case 32: return launch_nlist_t<32, NE, ME>(a, force, energy, mixed, st);
+    }
+    return cudaErrorInvalidConfiguration;
+}
+
+sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
+    sc_status st = ensure_list(c);
+    if (st != SC_OK) return st;
+    const int tpa = choose_tpa(c);
+    NlistArgs a{};
+    a.xs = c->xs; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.npad = c->npad;
+    a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
+    a.pairs_in_cut = c->counters + kCntPairsInCut;
+    a.rc2 = c->p.r_cut * c->p.r_cut;
+    a.c = c->consts;
+    if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
+    const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
+    cudaError_t e = fast ? launch_nlist_nm<9, 6>(tpa, a, force, energy, mixed, c->stream)
+                         : launch_nlist_nm<0, 0>(tpa, a, force, energy, mixed, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "list sweep launch: %s", cudaGetErrorString(e));
+    c->launches += 1;
+    if (!force || energy) {
+        const int grid = ceil_div(c->N, kNlistBlock / tpa);
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
+                                                         force ? c->consts.En : -c->consts.eps_c);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return SC_OK;
+}
+
+// device flags raised by the cutoff path; call after a stream synchronisation point
+sc_status check_flags(sc_ctx *c) {
+    if (!c->cutoff) return SC_OK;
+    unsigned long long cnt[kNumCounters];
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(cnt, c->counters, sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (cnt[kCntOverflow])
+        return fail(c, SC_ERR_CAPACITY, "a neighbour row overflowed its capacity; results since then are invalid%s");
+    return SC_OK;
+}
+
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
+    if (c->cutoff) return run_sweep_cutoff(c, force, energy);
     TileChoice tc = choose_tile(c);
     const bool fast = (c->p.n == 9 && c->p.m == 6);
     if (!fast && tc.it > 2) tc.it = 2;
@@ -231,6 +385,19 @@ sc_status read_scalars(sc_ctx *c, double *host, int count) {
     return SC_OK;
 }
 
+// internal array (internal atom order) -> caller's device buffer (caller's order), width doubles per atom
+sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
+    const int N = int(c->N);
+    if (c->cutoff) {
+        scatter_by_perm_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(src, d_dst, c->perm, N, width);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+    } else {
+        SC_CUDA_CHECK(c, cudaMemcpyAsync(d_dst, src, sizeof(double) * size_t(width) * size_t(N), cudaMemcpyDeviceToDevice, c->stream));
+    }
+    return SC_OK;
+}
+
 sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps) {
     if (!c->have_pos || !c->have_vel) return fail(c, SC_ERR_STATE, "sc_step: positions and velocities must be set%s");
     if (!(dt > 0.0) || !std::isfinite(dt) || nsteps < 0) return fail(c, SC_ERR_INVALID, "sc_step: dt must be > 0, nsteps >= 0%s");
@@ -250,9 +417,11 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     const double hk = 0.5 * dt * kAcc / c->p.mass;
     const double ndof = double(3 * c->N - 3);
     for (int64_t k = 1; k <= nsteps; ++k) {
-        kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, nullptr, N, hk, dt);
+        kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, c->cutoff ? c->xs_ref : nullptr,
+                                                        N, hk, dt);
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
+        c->list_checked = false;
         const bool last = (k == nsteps);
         st = ensure_forces(c, last || c->opt_energy_every == 1);
         if (st != SC_OK) return st;
@@ -268,7 +437,9 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
         }
     }
     SC_CUDA_CHECK(c, cudaGetLastError());
-    return flush_lambda(c);
+    sc_status fl = flush_lambda(c);
+    if (fl != SC_OK) return fl;
+    return check_flags(c);          // cutoff path only: one synchronisation per sc_step call
 }
 
 }  // namespace
@@ -286,7 +457,7 @@ size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t prec
     if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return 0;
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
     if (!(skin >= 0.0)) return 0;
-    return carve(nullptr, nullptr, n_atoms);
+    return carve(nullptr, nullptr, n_atoms, params, skin);
 }
 
 sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin, void *d_workspace,
@@ -297,8 +468,7 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return SC_ERR_INVALID;
     if (!(skin >= 0.0) || !d_workspace) return SC_ERR_INVALID;
     if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
-    if (precision == SC_PREC_MIXED) return SC_ERR_INVALID;     // not built yet
-    if (params->r_cut > 0.0) return SC_ERR_INVALID;            // not built yet
+    if (precision == SC_PREC_MIXED && !(params->r_cut > 0.0)) return SC_ERR_INVALID;     // not built yet
     const size_t need = sc_workspace_bytes(params, n_atoms, precision, skin);
     if (workspace_bytes < need) return SC_ERR_NOMEM;
     int dev = 0, count = 0;
@@ -309,7 +479,7 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     c->p = *params; c->N = n_atoms; c->precision = precision; c->skin = skin;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    carve(c, d_workspace, n_atoms);
+    carve(c, d_workspace, n_atoms, params, skin);
     const double a_n = ipow_host(params->a, params->n), a_m = ipow_host(params->a, params->m);
     c->consts.am = a_m;
     c->consts.An = params->eps * params->n * a_n;
@@ -327,6 +497,27 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     }
     reset_lambda_kernel<<<1, 1, 0, c->stream>>>(c->scal);
     if (cudaGetLastError() != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    if (params->r_cut > 0.0) {
+        c->cutoff = true;
+        c->r_list = params->r_cut + skin;
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_kernel, 256, 0) != cudaSuccess || per_sm < 1) {
+            delete c;
+            return SC_ERR_CUDA;
+        }
+        if (per_sm > 4) per_sm = 4;
+        c->coop_grid = per_sm * c->sm_count;
+        const int want = ceil_div(n_atoms, 256);            // no more CTAs than there is work for
+        if (c->coop_grid > want) c->coop_grid = want;
+        if (c->coop_grid > kMaxCoopBlocks) c->coop_grid = kMaxCoopBlocks;
+        if (cudaMemsetAsync(c->counters, 0, sizeof(unsigned long long) * kNumCounters, c->stream) != cudaSuccess ||
+            cudaMemsetAsync(c->xs_alt, 0, sizeof(double4) * (size_t(n_atoms) + kTileAtoms), c->stream) != cudaSuccess) {
+            delete c;
+            return SC_ERR_CUDA;
+        }
+        iota_kernel<<<ceil_div(n_atoms, kBlock), kBlock, 0, c->stream>>>(c->perm, int(n_atoms));
+        if (cudaGetLastError() != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    }
     *out = c;
     return SC_OK;
 }
@@ -359,8 +550,16 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
         case SC_OPT_ENERGY_EVERY_STEP:
             c->opt_energy_every = value ? 1 : 0; break;
         case SC_OPT_NEIGHBOUR_CAPACITY:
-            if (value < 0) return fail(c, SC_ERR_INVALID, "neighbour capacity must be >= 0%s");
-            c->opt_kmax = int(value); break;
+            if (value < 0 || (c->cutoff && value > c->kmax_cap))
+                return fail(c, SC_ERR_INVALID, "neighbour capacity must be 0 .. the capacity the workspace was sized for%s");
+            c->opt_kmax = int(value);
+            if (c->cutoff) {
+                c->kmax = value ? int(value) : c->kmax_cap;
+                c->list_checked = false;
+                reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
+                c->density_valid = c->forces_valid = c->energy_valid = false;
+            }
+            break;
         default:
             return fail(c, SC_ERR_INVALID, "unknown option%s");
     }
@@ -376,6 +575,21 @@ sc_status sc_set_state(sc_ctx *c, const double *d_pos, const double *d_vel) {
     c->launches += 1;
     c->have_pos = true;
     c->density_valid = c->forces_valid = c->energy_valid = false;
+    if (c->cutoff) {
+        // the internal order falls back to the caller's order; velocities already held follow it
+        if (c->have_vel && !d_vel) {
+            sc_status st = flush_lambda(c);
+            if (st != SC_OK) return st;
+            scatter_by_perm_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->vel, c->vel_alt, c->perm, N, 3);
+            SC_CUDA_CHECK(c, cudaMemcpyAsync(c->vel, c->vel_alt, sizeof(double) * 3 * size_t(N), cudaMemcpyDeviceToDevice, c->stream));
+            c->launches += 1;
+        }
+        iota_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->perm, N);
+        reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 2;
+        c->list_checked = false;
+    }
     if (d_vel) {
         sc_status st = flush_lambda(c);
         if (st != SC_OK) return st;
@@ -390,13 +604,17 @@ sc_status sc_get_state(sc_ctx *c, double *d_pos, double *d_vel) {
     if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_get_state: no positions set%s");
     const int N = int(c->N);
     if (d_pos) {
-        unpack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->xs, d_pos, N);
+        if (c->cutoff) unpack_positions_perm_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->xs, d_pos, c->perm, N);
+        else unpack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->xs, d_pos, N);
         SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
     }
     if (d_vel) {
         if (!c->have_vel) return fail(c, SC_ERR_STATE, "sc_get_state: no velocities set%s");
-        SC_CUDA_CHECK(c, cudaMemcpyAsync(d_vel, c->vel, sizeof(double) * 3 * size_t(N), cudaMemcpyDeviceToDevice, c->stream));
+        sc_status st = flush_lambda(c);
+        if (st != SC_OK) return st;
+        st = copy_out(c, c->vel, d_vel, 3);
+        if (st != SC_OK) return st;
     }
     return SC_OK;
 }
@@ -406,8 +624,7 @@ sc_status sc_density(sc_ctx *c, double *d_rho) {
     if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_density: no positions set%s");
     sc_status st = ensure_density(c);
     if (st != SC_OK) return st;
-    SC_CUDA_CHECK(c, cudaMemcpyAsync(d_rho, c->rho, sizeof(double) * size_t(c->N), cudaMemcpyDeviceToDevice, c->stream));
-    return SC_OK;
+    return copy_out(c, c->rho, d_rho, 1);
 }
 
 sc_status sc_forces(sc_ctx *c, double *d_force) {
@@ -415,8 +632,7 @@ sc_status sc_forces(sc_ctx *c, double *d_force) {
     if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_forces: no positions set%s");
     sc_status st = ensure_forces(c, true);
     if (st != SC_OK) return st;
-    SC_CUDA_CHECK(c, cudaMemcpyAsync(d_force, c->force, sizeof(double) * 3 * size_t(c->N), cudaMemcpyDeviceToDevice, c->stream));
-    return SC_OK;
+    return copy_out(c, c->force, d_force, 3);
 }
 
 sc_status sc_energy(sc_ctx *c, double *h_epot) {
@@ -430,7 +646,7 @@ sc_status sc_energy(sc_ctx *c, double *h_epot) {
     if (st != SC_OK) return st;
     *h_epot = s[kSlotEPair] + s[kSlotEEmb];
     if (!std::isfinite(*h_epot)) return fail(c, SC_ERR_NONFINITE, "sc_energy: potential energy is not finite (coincident atoms?)%s");
-    return SC_OK;
+    return check_flags(c);
 }
 
 sc_status sc_kinetic(sc_ctx *c, double *h_ke, double *h_temperature) {
@@ -459,9 +675,20 @@ sc_status sc_step(sc_ctx *c, double dt_fs, const sc_thermostat *thermostat, int6
 
 sc_status sc_stats(sc_ctx *c, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int64_t *max_neighbours) {
     if (!c) return SC_ERR_INVALID;
-    if (n_rebuilds) *n_rebuilds = 0;
-    if (n_pairs_in_cut) *n_pairs_in_cut = c->N * (c->N - 1);
-    if (max_neighbours) *max_neighbours = c->N - 1;
+    if (!c->cutoff) {
+        if (n_rebuilds) *n_rebuilds = 0;
+        if (n_pairs_in_cut) *n_pairs_in_cut = c->N * (c->N - 1);
+        if (max_neighbours) *max_neighbours = c->N - 1;
+        return SC_OK;
+    }
+    unsigned long long cnt[kNumCounters];
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(cnt, c->counters, sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (n_rebuilds) *n_rebuilds = int64_t(cnt[kCntRebuilds]);
+    if (n_pairs_in_cut) *n_pairs_in_cut = int64_t(cnt[kCntPairsInCut]);
+    if (max_neighbours) *max_neighbours = int64_t(cnt[kCntMaxRow]);
+    if (cnt[kCntOverflow])
+        return fail(c, SC_ERR_CAPACITY, "a neighbour row overflowed its capacity; results since then are invalid%s");
     return SC_OK;
 }
 
@@ -473,14 +700,19 @@ sc_status sc_eval_host(sc_ctx *c, const double *h_pos, double *h_force, double *
     if (st != SC_OK) return st;
     st = ensure_forces(c, true);
     if (st != SC_OK) return st;
-    if (h_force) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_force, c->force, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
-    if (h_rho) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_rho, c->rho, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    const double *src_f = c->force, *src_r = c->rho;
+    if (c->cutoff) {                      // back to the caller's order through the staging buffers
+        if (h_force) { st = copy_out(c, c->force, c->stage_b, 3); if (st != SC_OK) return st; src_f = c->stage_b; }
+        if (h_rho) { st = copy_out(c, c->rho, c->stage_a, 1); if (st != SC_OK) return st; src_r = c->stage_a; }
+    }
+    if (h_force) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_force, src_f, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+    if (h_rho) SC_CUDA_CHECK(c, cudaMemcpyAsync(h_rho, src_r, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
     double s[2];
     st = read_scalars(c, s, 2);
     if (st != SC_OK) return st;
     if (h_epot) *h_epot = s[kSlotEPair] + s[kSlotEEmb];
     if (!std::isfinite(s[0] + s[1])) return fail(c, SC_ERR_NONFINITE, "sc_eval_host: potential energy is not finite%s");
-    return SC_OK;
+    return check_flags(c);
 }
 
 sc_status sc_step_host(sc_ctx *c, double *h_pos, double *h_vel, double dt_fs, const sc_thermostat *thermostat,
@@ -498,7 +730,9 @@ sc_status sc_step_host(sc_ctx *c, double *h_pos, double *h_vel, double dt_fs, co
     st = sc_get_state(c, c->stage_a, nullptr);
     if (st != SC_OK) return st;
     SC_CUDA_CHECK(c, cudaMemcpyAsync(h_pos, c->stage_a, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
-    SC_CUDA_CHECK(c, cudaMemcpyAsync(h_vel, c->vel, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
+    st = copy_out(c, c->vel, c->stage_b, 3);
+    if (st != SC_OK) return st;
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(h_vel, c->stage_b, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, c->stream));
     if (h_scalars) {
         double ke = 0, temp = 0;
         st = sc_kinetic(c, &ke, &temp);
