@@ -4,9 +4,11 @@
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
 
 One "step" = one pass of the whole hot path over the synthetic cluster: a velocity-Verlet MD step
-(half kick + drift, density sweep, force + energy sweep, half kick + kinetic-energy reduction)
-through libscmd's sc_step.  Default workload: BASELINE.json configs[3], the Ni65536 fcc cluster,
-all pairs, FP64 -- the configuration the metric's roofline target (N >= 65,536) is quoted on.
+(half kick + drift, [cutoff variant: skin check / cell sort / neighbour rows], density sweep, force +
+energy sweep, half kick + kinetic-energy reduction) through libscmd's sc_step.  Default workload:
+BASELINE.json configs[3], the Ni65536 fcc cluster, all pairs, FP64 -- the configuration the metric's
+roofline target (N >= 65,536) is quoted on.  Other workloads (same JSON line):
+    Ni<N>-<fcc|liquid|mackay>-<allpairs|cutoff10>-<fp64|mixed>
 Prints ONE JSON line.  N > 1 GPUs = N independent replicas
 (the paper's own use: up to 15 independent trajectories per temperature); the
 only collective is the timing reduction.
@@ -33,27 +35,49 @@ from paper_1210_3559_b200 import workloads as W  # noqa: E402
 METRIC = "pair_interactions_per_s"
 UNIT = "ordered pairs/s (both sweeps)"
 
-# FP64-pipe instructions per ordered pair in the shipped (9,6) kernels (SASS-counted)
-I_DENSITY = 11
-I_FORCE_ENERGY = 22
-# nominal B200 FP64 peak: 148 SMs x 64 lanes x 2 FLOP x 1.965 GHz
-SM_COUNT, FP64_LANES, SM_MAX_GHZ = 148, 64, 1.965
-FP64_PEAK_TFLOPS = SM_COUNT * FP64_LANES * 2 * SM_MAX_GHZ / 1e3
+# ALU instructions per ordered pair in the shipped (9,6) kernels (SASS-counted):
+# thread-level FP64-pipe instructions (FP64 path) / FMA-pipe lane operations (mixed path)
+I_DENSITY = {"fp64": 11, "mixed": 16}
+I_FORCE_ENERGY = {"fp64": 22, "mixed": 27}
+# nominal B200 ALU peaks: 148 SMs x lanes x 2 FLOP x 1.965 GHz
+SM_COUNT, SM_MAX_GHZ = 148, 1.965
+LANES = {"fp64": 64, "mixed": 128}
+PEAK_TFLOPS = {k: SM_COUNT * v * 2 * SM_MAX_GHZ / 1e3 for k, v in LANES.items()}
+DEFAULT_WORKLOAD = "Ni65536-fcc-allpairs-fp64"
+
+
+class Spec:
+    """Parsed workload name."""
+
+    def __init__(self, name: str):
+        parts = name.split("-")
+        if len(parts) != 4 or not parts[0].startswith("Ni"):
+            raise SystemExit(f"unknown workload {name}: want Ni<N>-<fcc|liquid|mackay>-<allpairs|cutoff<r>>-<fp64|mixed>")
+        self.name = name
+        self.n_atoms = int(parts[0][2:])
+        self.kind, self.pairs, self.prec = parts[1], parts[2], parts[3]
+        if self.kind not in ("fcc", "liquid", "mackay") or self.prec not in ("fp64", "mixed"):
+            raise SystemExit(f"unknown workload {name}")
+        self.r_cut = 0.0 if self.pairs == "allpairs" else float(self.pairs.replace("cutoff", ""))
+        self.skin = 1.0 if self.r_cut > 0 else 0.0                      # BASELINE.json config 4: skin 1 A
+
+    def generate(self, rank: int = 0) -> W.Workload:
+        n = self.n_atoms
+        if self.kind == "mackay":
+            assert n == 147
+            return W.config_c1(seed=1001 + rank)
+        if self.kind == "liquid":
+            return W.config_c3(seed=3001 + rank, n_atoms=n)
+        if n == 1415:
+            return W.config_c2(seed=2001 + rank)
+        if n == 65536:
+            return W.config_c4(seed=4001 + rank)
+        k = int(round(np.log2(n) / 2))
+        return W.fcc_cluster(n, 1500.0, 5000 + k + rank)                # C5 sweep member
 
 
 def make_workload(name: str, rank: int = 0) -> W.Workload:
-    if name == "Ni65536-fcc-allpairs-fp64":
-        return W.config_c4(seed=4001 + rank)
-    if name == "Ni1415-fcc-allpairs-fp64":
-        return W.config_c2(seed=2001 + rank)
-    if name == "Ni8000-liquid-allpairs-fp64":
-        return W.config_c3(seed=3001 + rank)
-    if name == "Ni147-mackay-allpairs-fp64":
-        return W.config_c1(seed=1001 + rank)
-    if name.startswith("Ni") and name.endswith("-fcc-sweep-fp64"):
-        n = int(name[2:].split("-")[0])
-        return W.fcc_cluster(n, 1500.0, 5000 + int(round(np.log2(n) / 2)) + rank)
-    raise SystemExit(f"unknown workload {name}")
+    return Spec(name).generate(rank)
 
 
 # ------------------------------------------------------------------------------------------- #
@@ -144,39 +168,61 @@ def oracle_sample_rows(n_atoms: int, target_pair_passes: float = 2.5e9) -> np.nd
     return np.unique(np.linspace(0, n_atoms - 1, nrows).astype(np.int64))
 
 
-def oracle_time_sample(w: W.Workload, rows: np.ndarray):
-    """Both sweeps of the binary64 oracle build for `rows` (all j): seconds, ordered pairs."""
+def oracle_time_sample(w: W.Workload, rows: np.ndarray, r_cut: float = 0.0, pair_fraction: float = 1.0):
+    """Both sweeps of the binary64 oracle build for `rows` (all j; with a cutoff the oracle still visits
+    every j and filters): seconds, ordered pair interactions credited (in-range ones for a cutoff)."""
     from oracle.sc_oracle import Oracle
     o = Oracle("plain")
-    P = o.params()
+    P = o.params(r_cut=r_cut)
     rho_all = np.full(w.n_atoms, 100.0)          # timing only: any positive density works as s_j input
     t0 = time.perf_counter()
     rho_rows = o.density_rows(w.pos, P, rows)
     rho_all[rows] = rho_rows
     o.forces_rows(w.pos, P, rho_all, rows)
     dt = time.perf_counter() - t0
-    return dt, float(rows.size) * (w.n_atoms - 1)
+    return dt, float(rows.size) * (w.n_atoms - 1) * pair_fraction
 
 
-def cpu_baseline(w: W.Workload) -> dict:
-    rows = oracle_sample_rows(w.n_atoms)
-    dt, pairs = oracle_time_sample(w, rows)
-    return {"value": pairs / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-            "seconds": dt,
-            "sample": f"{rows.size} evenly spaced rows i of {w.name} (all j, both sweeps), binary64 oracle build, OpenMP"}
+def in_range_fraction(w: W.Workload, r_cut: float) -> float:
+    """Share of the N(N-1) ordered pairs with r < r_cut (1 for all pairs), from a row sample."""
+    if r_cut <= 0:
+        return 1.0
+    rows = np.unique(np.linspace(0, w.n_atoms - 1, 256).astype(np.int64))
+    hits = 0
+    for i in rows:
+        d2 = ((w.pos - w.pos[i]) ** 2).sum(axis=1)
+        hits += int((d2 < r_cut * r_cut).sum()) - 1
+    return hits / (rows.size * (w.n_atoms - 1.0))
+
+
+def cpu_baseline(w: W.Workload, r_cut: float = 0.0, pair_fraction: float = 1.0, budget_s: float = 12.0) -> dict:
+    """The oracle as it stands on the host cores: whole evaluations of the workload (or, when one
+    evaluation would exceed the budget, an evenly spaced row sample of it), repeated for ~budget_s."""
+    rows = oracle_sample_rows(w.n_atoms, target_pair_passes=2.0e10)
+    total_s, total_pairs, reps = 0.0, 0.0, 0
+    while reps < 8 and (reps == 0 or total_s < budget_s):
+        dt, pairs = oracle_time_sample(w, rows, r_cut, pair_fraction)
+        total_s += dt; total_pairs += pairs; reps += 1
+    what = "all rows" if rows.size == w.n_atoms else f"{rows.size} evenly spaced rows i"
+    return {"value": total_pairs / total_s, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+            "seconds": total_s,
+            "sample": f"{reps} x ({what} of {w.name}, all j, both sweeps{', filtered at r_c' if r_cut > 0 else ''}), "
+                      "binary64 oracle build, OpenMP on all host cores"}
 
 
 def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return
-    w = make_workload(args.workload)
+    spec = Spec(args.workload)
+    w = spec.generate()
+    frac = in_range_fraction(w, spec.r_cut)
     rows = oracle_sample_rows(w.n_atoms, target_pair_passes=6e8)
     for _ in range(args.warmup):
-        oracle_time_sample(w, rows)
+        oracle_time_sample(w, rows, spec.r_cut, frac)
     total_s, total_pairs = 0.0, 0.0
     for _ in range(args.steps):
-        dt, pairs = oracle_time_sample(w, rows)
+        dt, pairs = oracle_time_sample(w, rows, spec.r_cut, frac)
         total_s += dt; total_pairs += pairs
     value = total_pairs / total_s
     sample = (f"each step = {rows.size} evenly spaced rows i of {w.name} (all j, both sweeps), "
@@ -207,13 +253,17 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     scmd.load_library()
 
-    w = make_workload(args.workload, rank)
+    spec = Spec(args.workload)
+    w = spec.generate(rank)
     N = w.n_atoms
-    pairs_per_step = float(N) * (N - 1)
-    sc = scmd.SuttonChen(N)
+    prec = scmd.SC_PREC_MIXED if spec.prec == "mixed" else scmd.SC_PREC_FP64
+    sc = scmd.SuttonChen(N, r_cut=spec.r_cut, skin=spec.skin, precision=prec)
     d_pos = torch.as_tensor(w.pos, device=dev)
     d_vel = torch.as_tensor(w.vel, device=dev)
     sc.sc_set_state(d_pos, d_vel)
+    sc.sc_energy()                                                     # first evaluation (builds the rows)
+    stats0 = sc.sc_stats()
+    pairs_per_step = float(stats0["n_pairs_in_cut"])                   # N(N-1) for all pairs
     sc.sc_profile(True)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = torch.cuda.current_stream()
@@ -246,12 +296,14 @@ def run_ours(args):
         dist.barrier()
     launches = sc.sc_launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
+    stats1 = sc.sc_stats()
     local_ms = sum(a.elapsed_time(b) for a, b in ev)
     total_ms, total_pairs = aggregate(local_ms, pairs_per_step * args.steps, world)
     value = total_pairs / (total_ms * 1e-3)
 
-    # end to end through the host-buffer entry point: upload positions, both sweeps, download
-    # forces + energy (pinned host memory), every step
+    # end to end through the host-buffer entry point: upload positions, both sweeps (cutoff: plus the
+    # cell sort and row build, since new positions invalidate the rows), download forces + energy
+    # (pinned host memory), every step
     h_pos = torch.as_tensor(w.pos).pin_memory()
     h_force = torch.empty(N, 3, dtype=torch.float64).pin_memory()
     for _ in range(2):
@@ -271,37 +323,63 @@ def run_ours(args):
         return
     t_force = statistics.mean(ms_force) * 1e-3
     t_density = statistics.mean(ms_density) * 1e-3
-    achieved = I_FORCE_ENERGY * 2.0 * pairs_per_step / t_force / 1e12
+    i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
+    achieved = i_f * 2.0 * pairs_per_step / t_force / 1e12
+    probe_kind = 0 if spec.prec == "fp64" else 2
     try:
-        dfma_rate, probe_mhz = scmd.probe_throughput(0)
-        peak_measured = dfma_rate * 2.0 / 1e12
+        rate, _ = scmd.probe_throughput(probe_kind)
+        peak_measured = rate * 2.0 / 1e12
     except Exception:
-        peak_measured, probe_mhz = None, None
+        peak_measured = None
     traffic = None
     tfile = ROOT / "profiles" / "roofline_traffic.json"
     if tfile.exists():
         traffic = json.loads(tfile.read_text()).get(args.workload, {}).get("force_sweep_dram_bytes_per_launch")
-    roofline = {"bound": "alu", "kernel": "allpairs64_kernel<force+energy>", "achieved": achieved,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no FP64 figure",
-                "peak_measured_dfma_probe": peak_measured, "probe_sm_mhz": probe_mhz,
-                "fp64_inst_per_pair": I_FORCE_ENERGY, "ms_force_sweep": t_force * 1e3,
-                "ms_density_sweep": t_density * 1e3,
-                "density_sweep_frac": I_DENSITY * 2.0 * pairs_per_step / t_density / 1e12 / FP64_PEAK_TFLOPS,
-                "both_sweeps_frac": (I_DENSITY + I_FORCE_ENERGY) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / FP64_PEAK_TFLOPS}
+    if spec.r_cut > 0:
+        kernel = f"nlist_kernel<force+energy, {spec.prec}>"
+    else:
+        kernel = ("allpairs64_kernel" if spec.prec == "fp64" else "allpairs32_kernel") + "<force+energy>"
+    pipe = "FP64" if spec.prec == "fp64" else "FP32"
+    roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                "peak_source": f"nominal: 148 SM x {LANES[spec.prec]} {pipe} lanes x 2 x 1.965 GHz (DESIGN.md section 6); "
+                               "MEASURED_PEAKS.json has no CUDA-core figure",
+                "peak_measured_fma_probe": peak_measured,
+                "alu_inst_per_pair": i_f, "ms_force_sweep": t_force * 1e3, "ms_density_sweep": t_density * 1e3,
+                "density_sweep_frac": i_d * 2.0 * pairs_per_step / t_density / 1e12 / peak,
+                "both_sweeps_frac": (i_d + i_f) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / peak}
+    if spec.r_cut > 0:
+        # the list path's memory side: the method's own bytes are records in + forces out;
+        # the neighbour indices (4 B per entry per sweep) are the data structure's cost
+        hbm_peak = 6445.6
+        try:
+            hbm_peak = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]
+        except Exception:
+            pass
+        alg_bytes = N * (32 + 8 + 24 + 32)                              # both sweeps: records, rho, forces
+        roofline["hbm"] = {"algorithmic_bytes_per_step": alg_bytes, "peak_gbs": hbm_peak,
+                           "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy)",
+                           "algorithmic_gbs": alg_bytes / (t_force + t_density) / 1e9,
+                           "frac": alg_bytes / (t_force + t_density) / 1e9 / hbm_peak,
+                           "rebuilds_in_timed_region": stats1["n_rebuilds"] - stats0["n_rebuilds"],
+                           "max_neighbours": stats1["max_neighbours"]}
+    frac_pairs = pairs_per_step / (float(N) * (N - 1)) if N > 1 else 1.0
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if spec.prec == "fp64" else "f32 pair math, f64 accumulation",
+            "data": "synthetic",
             "md_steps_per_s": world * args.steps / (total_ms * 1e-3),
             "config": {"workload": args.workload, "n_atoms": N, "pairs_per_step": pairs_per_step,
+                       "r_cut": spec.r_cut, "skin": spec.skin,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "flushed between timed steps (256 MiB memset outside the per-step events)",
-                       "step": "sc_step(dt=1 fs, nsteps=1): kick+drift, density sweep, force+energy sweep, kick+KE"},
+                       "step": "sc_step(dt=1 fs, nsteps=1): kick+drift, [skin check / rebuild,] density sweep, "
+                               "force+energy sweep, kick+KE"},
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * N,
                     "d2h_bytes_per_step": 24 * N + 16, "call": "sc_eval_host (pinned host buffers)",
                     "ms_per_call": e2e_ms / e2e_steps},
-            "roofline": roofline, "cpu_baseline": cpu_baseline(w)}
+            "roofline": roofline, "cpu_baseline": cpu_baseline(w, spec.r_cut, frac_pairs)}
     print(json.dumps(line), flush=True)
 
 
@@ -311,7 +389,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="Ni65536-fcc-allpairs-fp64")
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

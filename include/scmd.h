@@ -162,6 +162,7 @@ sc_status sc_profile_read(sc_ctx *ctx, double *h_ms_density, double *h_ms_force)
  *   thread-level instructions per second and the SM clock (MHz) held during the run.
  *   kind 0: FP64 DFMA   1: FP32 FFMA   2: packed FP32x2 FMA (counted as 2 per lane)
  *        3: MUFU.RSQ (binary32)        4: FP64 reciprocal seed (MUFU.RCP64H)
+ *        5: FP32 FADD   6: FP32 FMUL   7: packed FADD2   8: packed FMUL2 (packed: 2 per lane)
  *   bench.py prints the measured figure beside the nominal ALU peak.
  * sc_probe_reciprocal: maximum relative error, over n_samples log-uniform x in [lo, hi], of
  *   h_err4 = { rcp seed, refined 1/x, rsqrt seed, refined x^-1/2 } as used by the FP64 sweeps,

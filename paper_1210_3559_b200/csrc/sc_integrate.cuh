@@ -20,10 +20,15 @@ enum ScalarSlot {
     kNumScalars = 16
 };
 
-// pos[N*3] -> xs[N] = (x, y, z, 0)
-__global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, int N) {
+// pos[N*3] -> xs[N] = (x, y, z, 0); xf (mixed all-pairs path, else NULL) gets the split record
+__global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, FPair *__restrict__ xf,
+                                      int N) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) xs[i] = make_double4(pos[3 * size_t(i)], pos[3 * size_t(i) + 1], pos[3 * size_t(i) + 2], 0.0);
+    if (i < N) {
+        const double x = pos[3 * size_t(i)], y = pos[3 * size_t(i) + 1], z = pos[3 * size_t(i) + 2];
+        xs[i] = make_double4(x, y, z, 0.0);
+        if (xf) store_split_record(xf, i, x, y, z, 0.f);
+    }
 }
 __global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *__restrict__ pos, int N) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -37,8 +42,8 @@ __global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *
 // (hk = dt/2 * ACC / m).  ref (may be NULL): positions at the last list build; the largest squared
 // displacement from it goes to scal[kSlotMaxDisp2] through an integer atomicMax (order-free).
 __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__ vel, const double *__restrict__ force,
-                                  double *__restrict__ scal, const double4 *__restrict__ ref, int N, double hk,
-                                  double dt) {
+                                  double *__restrict__ scal, const double4 *__restrict__ ref, FPair *__restrict__ xf,
+                                  int N, double hk, double dt) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     double d2 = 0.0;
     if (i < N) {
@@ -51,6 +56,7 @@ __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__
         p.x = fma(dt, vx, p.x); p.y = fma(dt, vy, p.y); p.z = fma(dt, vz, p.z);
         vel[3 * size_t(i)] = vx; vel[3 * size_t(i) + 1] = vy; vel[3 * size_t(i) + 2] = vz;
         xs[i] = p;
+        if (xf) store_split_record(xf, i, p.x, p.y, p.z, float(p.w));
         if (ref) {
             const double4 r = ref[i];
             const double ex = p.x - r.x, ey = p.y - r.y, ez = p.z - r.z;

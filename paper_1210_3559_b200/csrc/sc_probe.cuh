@@ -57,6 +57,42 @@ __global__ void __launch_bounds__(256) probe_kernel(double *out, long long *cycl
             asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a[k]));
             sink += lo + hi;
         }
+    } else if constexpr (KIND == 5 || KIND == 6) {   // FADD / FMUL
+        float a[kProbeChains];
+        const float b = (KIND == 5) ? float(seed) * 1e-7f : 1.0f + float(seed) * 1e-7f;
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) a[k] = float(seed) + k + threadIdx.x;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) {
+                if constexpr (KIND == 5) asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b));
+                else asm volatile("mul.rn.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b));
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) sink += a[k];
+    } else if constexpr (KIND == 7 || KIND == 8) {   // packed FADD2 / FMUL2
+        unsigned long long a[kProbeChains], b;
+        const float bf = (KIND == 7) ? float(seed) * 1e-7f : 1.0f + float(seed) * 1e-7f;
+        asm("mov.b64 %0, {%1, %1};" : "=l"(b) : "f"(bf));
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) {
+            const float v = float(seed) + k + threadIdx.x;
+            asm("mov.b64 %0, {%1, %1};" : "=l"(a[k]) : "f"(v));
+        }
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int k = 0; k < kProbeChains; ++k) {
+                if constexpr (KIND == 7) asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a[k]) : "l"(b));
+                else asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(a[k]) : "l"(b));
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kProbeChains; ++k) {
+            float lo, hi;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a[k]));
+            sink += lo + hi;
+        }
     } else if constexpr (KIND == 3) {                // MUFU.RSQ (binary32)
         float a[kProbeChains];
 #pragma unroll

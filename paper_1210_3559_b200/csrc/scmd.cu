@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "sc_allpairs.cuh"
 #include "sc_cutoff.cuh"
@@ -50,6 +51,7 @@ struct sc_ctx {
 
     // device arrays (all inside the caller's workspace)
     double4 *xs = nullptr;        // [N] (x, y, z, s')
+    FPair *xf = nullptr;          // [(N + 512) / 2 + 1] packed split binary32 records (mixed all-pairs path only)
     double *vel = nullptr;        // [N*3]
     double *force = nullptr;      // [N*3]
     double *rho = nullptr;        // [N]
@@ -78,6 +80,9 @@ struct sc_ctx {
     bool density_valid = false, forces_valid = false, energy_valid = false;
     bool lambda_pending = false;
     int64_t launches = 0;
+
+    struct OccEntry { const void *fn; int warps; int per_sm; };
+    std::vector<OccEntry> occ_cache;
 
     // options (0 = default)
     int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0;
@@ -128,7 +133,7 @@ int cutoff_max_dim(int64_t N) {
 }
 
 // one place that lays the workspace out; base == nullptr only measures
-size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, double skin) {
+size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin) {
     Carver w(base);
     const size_t n = size_t(N);
     double4 *xs = w.take<double4>(n + kTileAtoms);
@@ -144,6 +149,10 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, double skin
     if (c && base) {
         c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
+    }
+    if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
+        FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
+        if (c && base) c->xf = xf;
     }
     if (prm->r_cut > 0.0) {
         const int kmax = default_kmax(prm, N, skin), npad = round_up(N, 32), md = cutoff_max_dim(N);
@@ -180,49 +189,84 @@ double ipow_host(double u, int k) {
 // ---------------------------------------------------------------------------------------------
 struct TileChoice { int it, tpr, warps; };
 
-TileChoice choose_tile(const sc_ctx *c) {
-    const int64_t N = c->N;
-    // largest rows-per-CTA that still gives >= 4 CTAs per SM; prefer 2 rows per thread
-    const int64_t want_ctas = int64_t(4) * c->sm_count;
-    int rpc = 1;
-    while (rpc < 64 && N / (rpc * 2) >= want_ctas) rpc *= 2;
-    int it = rpc >= 2 ? 2 : 1;
-    int tpr = 32 * it / rpc;
-    if (tpr > 32) { tpr = 32; it = 1; }
-    int warps = 8;
-    // keep at least ~8 pairs per lane and tile
-    while (warps > 1 && N / (int64_t(warps) * tpr) < 8) warps /= 2;
-    if (c->opt_it) it = c->opt_it;
-    if (c->opt_tpr) tpr = c->opt_tpr;
-    if (c->opt_warps) warps = c->opt_warps;
-    return {it, tpr, warps};
+template <bool MIXED, int IT, int TPR, int NE, int ME>
+const void *allpairs_fn_t(bool force, bool energy) {
+    if constexpr (MIXED) {
+        if (!force) return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, false, false>);
+        if (energy) return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, true, true>);
+        return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, true, false>);
+    } else {
+        if (!force) return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, false, false>);
+        if (energy) return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, true, true>);
+        return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, true, false>);
+    }
 }
 
-template <int IT, int TPR, int NE, int ME>
-cudaError_t launch_allpairs_t(const AllPairsArgs &args, bool force, bool energy, int warps, int grid, cudaStream_t st) {
-    const size_t smem = allpairs_smem_bytes(IT, TPR, warps);
-    const dim3 block((warps + 1) * 32);
-    auto go = [&](auto kernel) -> cudaError_t {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-        if (e != cudaSuccess) return e;
-        kernel<<<grid, block, smem, st>>>(args);
-        return cudaGetLastError();
-    };
-    if (!force) return go(allpairs64_kernel<IT, TPR, NE, ME, false, false>);
-    if (energy) return go(allpairs64_kernel<IT, TPR, NE, ME, true, true>);
-    return go(allpairs64_kernel<IT, TPR, NE, ME, true, false>);
-}
-
-template <int NE, int ME>
-cudaError_t launch_allpairs_nm(const TileChoice &tc, const AllPairsArgs &a, bool force, bool energy, int grid,
-                               cudaStream_t st) {
+template <bool MIXED, int NE, int ME>
+const void *allpairs_fn_nm(int it, int tpr, bool force, bool energy) {
 #define SC_CASE(IT, TPR) \
-    if (tc.it == IT && tc.tpr == TPR) return launch_allpairs_t<IT, TPR, NE, ME>(a, force, energy, tc.warps, grid, st);
+    if (it == IT && tpr == TPR) return allpairs_fn_t<MIXED, IT, TPR, NE, ME>(force, energy);
     SC_CASE(1, 1) SC_CASE(1, 2) SC_CASE(1, 4) SC_CASE(1, 8) SC_CASE(1, 16) SC_CASE(1, 32)
     SC_CASE(2, 1) SC_CASE(2, 2) SC_CASE(2, 4) SC_CASE(2, 8) SC_CASE(2, 16) SC_CASE(2, 32)
     if constexpr (NE != 0) { SC_CASE(4, 1) SC_CASE(4, 2) SC_CASE(4, 4) }
 #undef SC_CASE
-    return cudaErrorInvalidConfiguration;
+    return nullptr;
+}
+
+const void *allpairs_fn(const sc_ctx *c, int it, int tpr, bool force, bool energy) {
+    const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
+    if (!fast && it > 2) return nullptr;
+    if (mixed) return fast ? allpairs_fn_nm<true, 9, 6>(it, tpr, force, energy) : allpairs_fn_nm<true, 0, 0>(it, tpr, force, energy);
+    return fast ? allpairs_fn_nm<false, 9, 6>(it, tpr, force, energy) : allpairs_fn_nm<false, 0, 0>(it, tpr, force, energy);
+}
+
+// resident CTAs per SM of one instantiation at (warps + 1) * 32 threads; cached per context
+int allpairs_residency(sc_ctx *c, const void *fn, int it, int tpr, int warps) {
+    const size_t smem = allpairs_smem_bytes(it, tpr, warps);
+    for (const auto &e : c->occ_cache)
+        if (e.fn == fn && e.warps == warps) return e.per_sm;
+    int per_sm = 1;
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, (warps + 1) * 32, smem) != cudaSuccess || per_sm < 1)
+        per_sm = 1;
+    c->occ_cache.push_back({fn, warps, per_sm});
+    return per_sm;
+}
+
+// Tile shape for one sweep.  Rows per CTA = 32 / tpr * it.  Large N: CTAs run in waves of
+// sm_count * residency, and a partly filled last wave idles the chip (N = 65536 at 64 rows per CTA is
+// 3.46 waves of the force sweep: 13 % lost), so among the shapes with 2 rows per thread take the one
+// whose wave efficiency x / ceil(x) is best, preferring more rows per CTA when it is a tie.  Small N
+// (x < 1): efficiency = x, i.e. the shape with the most CTAs, down to one row per CTA.
+TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
+    const int64_t N = c->N;
+    TileChoice best{2, 1, 8};
+    if (c->opt_it && c->opt_tpr) {
+        best.it = c->opt_it; best.tpr = c->opt_tpr;
+    } else {
+        double best_eff = -1.0;
+        const int its[2] = {2, 1};
+        for (int it : its) {
+            if (c->opt_it && it != c->opt_it) continue;
+            for (int tpr = 1; tpr <= 32; tpr *= 2) {
+                if (c->opt_tpr && tpr != c->opt_tpr) continue;
+                if (it == 1 && tpr != 32 && !c->opt_it) continue;       // 1 row per thread only as the smallest shape
+                const void *fn = allpairs_fn(c, it, tpr, force, energy);
+                if (!fn) continue;
+                const int rpc = allpairs_rows_per_cta(it, tpr);
+                const double x = double(ceil_div(N, rpc)) / (double(c->sm_count) * allpairs_residency(c, fn, it, tpr, 8));
+                const double eff = x / std::ceil(x);
+                if (eff > best_eff + 0.02) { best_eff = eff; best.it = it; best.tpr = tpr; }
+            }
+        }
+        if (c->opt_it) best.it = c->opt_it;
+        if (c->opt_tpr) best.tpr = c->opt_tpr;
+    }
+    int warps = 8;
+    while (warps > 1 && N / (int64_t(warps) * best.tpr) < 8) warps /= 2;   // >= ~8 pairs per lane and row
+    if (c->opt_warps) warps = c->opt_warps;
+    best.warps = warps;
+    return best;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -325,17 +369,22 @@ sc_status check_flags(sc_ctx *c) {
 
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (c->cutoff) return run_sweep_cutoff(c, force, energy);
-    TileChoice tc = choose_tile(c);
-    const bool fast = (c->p.n == 9 && c->p.m == 6);
-    if (!fast && tc.it > 2) tc.it = 2;
+    TileChoice tc = choose_tile(c, force, energy);
+    const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);
+    if (!fn) return fail(c, SC_ERR_INVALID, "all-pairs sweep: no kernel for this tile shape%s");
     const int rpc = allpairs_rows_per_cta(tc.it, tc.tpr);
     const int grid = ceil_div(c->N, rpc);
+    const size_t smem = allpairs_smem_bytes(tc.it, tc.tpr, tc.warps);
     AllPairsArgs a{};
     a.xs = c->xs; a.n_atoms = int(c->N); a.rho = c->rho; a.force = c->force;
     a.partial = force ? c->part_b : c->part_a;
     a.c = c->consts;
-    cudaError_t e = fast ? launch_allpairs_nm<9, 6>(tc, a, force, energy, grid, c->stream)
-                         : launch_allpairs_nm<0, 0>(tc, a, force, energy, grid, c->stream);
+    AllPairs32Args a32{};
+    a32.xf = c->xf; a32.xs = c->xs; a32.n_atoms = a.n_atoms; a32.rho = a.rho; a32.force = a.force; a32.partial = a.partial;
+    a32.c = c->consts;
+    void *params[1] = {c->precision == SC_PREC_MIXED ? static_cast<void *>(&a32) : static_cast<void *>(&a)};
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+    if (e == cudaSuccess) e = cudaLaunchKernel(fn, dim3(grid), dim3((tc.warps + 1) * 32), params, smem, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "all-pairs sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     if (!force || energy) {
@@ -418,7 +467,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     const double ndof = double(3 * c->N - 3);
     for (int64_t k = 1; k <= nsteps; ++k) {
         kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, c->cutoff ? c->xs_ref : nullptr,
-                                                        N, hk, dt);
+                                                        c->xf, N, hk, dt);
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
         c->list_checked = false;
@@ -457,7 +506,7 @@ size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t prec
     if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return 0;
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
     if (!(skin >= 0.0)) return 0;
-    return carve(nullptr, nullptr, n_atoms, params, skin);
+    return carve(nullptr, nullptr, n_atoms, params, precision, skin);
 }
 
 sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin, void *d_workspace,
@@ -468,7 +517,6 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return SC_ERR_INVALID;
     if (!(skin >= 0.0) || !d_workspace) return SC_ERR_INVALID;
     if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
-    if (precision == SC_PREC_MIXED && !(params->r_cut > 0.0)) return SC_ERR_INVALID;     // not built yet
     const size_t need = sc_workspace_bytes(params, n_atoms, precision, skin);
     if (workspace_bytes < need) return SC_ERR_NOMEM;
     int dev = 0, count = 0;
@@ -479,7 +527,7 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     c->p = *params; c->N = n_atoms; c->precision = precision; c->skin = skin;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    carve(c, d_workspace, n_atoms, params, skin);
+    carve(c, d_workspace, n_atoms, params, precision, skin);
     const double a_n = ipow_host(params->a, params->n), a_m = ipow_host(params->a, params->m);
     c->consts.am = a_m;
     c->consts.An = params->eps * params->n * a_n;
@@ -491,7 +539,8 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
         if (cudaEventCreate(&e) != cudaSuccess) { delete c; return SC_ERR_CUDA; }
     // scalars: zero, lambda = 1; pad the record array tail so that full-tile reads stay defined
     if (cudaMemsetAsync(c->scal, 0, sizeof(double) * kNumScalars, c->stream) != cudaSuccess ||
-        cudaMemsetAsync(c->xs, 0, sizeof(double4) * (size_t(n_atoms) + kTileAtoms), c->stream) != cudaSuccess) {
+        cudaMemsetAsync(c->xs, 0, sizeof(double4) * (size_t(n_atoms) + kTileAtoms), c->stream) != cudaSuccess ||
+        (c->xf && cudaMemsetAsync(c->xf, 0, sizeof(FPair) * ((size_t(n_atoms) + kTileAtoms) / 2 + 1), c->stream) != cudaSuccess)) {
         delete c;
         return SC_ERR_CUDA;
     }
@@ -570,7 +619,7 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
 sc_status sc_set_state(sc_ctx *c, const double *d_pos, const double *d_vel) {
     if (!c || !d_pos) return fail(c, SC_ERR_INVALID, "sc_set_state: d_pos is NULL%s");
     const int N = int(c->N);
-    pack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(d_pos, c->xs, N);
+    pack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(d_pos, c->xs, c->xf, N);
     SC_CUDA_CHECK(c, cudaGetLastError());
     c->launches += 1;
     c->have_pos = true;
@@ -774,7 +823,7 @@ sc_status sc_profile_read(sc_ctx *c, double *h_ms_density, double *h_ms_force) {
 
 sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, size_t scratch_bytes,
                               double *h_inst_per_s, double *h_sm_clock_mhz) {
-    if (kind < 0 || kind > 4 || !d_scratch || !h_inst_per_s) return SC_ERR_INVALID;
+    if (kind < 0 || kind > 8 || !d_scratch || !h_inst_per_s) return SC_ERR_INVALID;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
@@ -783,7 +832,7 @@ sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, 
     if (scratch_bytes < sizeof(double) * 8 + sizeof(long long) * size_t(grid)) return SC_ERR_NOMEM;
     double *out = static_cast<double *>(d_scratch);
     long long *cyc = reinterpret_cast<long long *>(out + 8);
-    const int iters = (kind >= 3) ? 2048 : 16384;
+    const int iters = (kind == 3 || kind == 4) ? 2048 : 16384;
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return SC_ERR_CUDA;
     auto run = [&](int it) {
@@ -792,7 +841,11 @@ sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, 
             case 1: probe_kernel<1><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
             case 2: probe_kernel<2><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
             case 3: probe_kernel<3><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            default: probe_kernel<4><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 4: probe_kernel<4><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 5: probe_kernel<5><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 6: probe_kernel<6><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            case 7: probe_kernel<7><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
+            default: probe_kernel<8><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
         }
     };
     run(iters / 8);   // warm-up
@@ -809,7 +862,7 @@ sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, 
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     if (rc != SC_OK) return rc;
-    const double per_thread = double(iters) * kProbeChains * (kind == 2 ? 2.0 : 1.0);
+    const double per_thread = double(iters) * kProbeChains * ((kind == 2 || kind == 7 || kind == 8) ? 2.0 : 1.0);
     *h_inst_per_s = per_thread * double(grid) * block / (double(ms) * 1e-3);
     // a block's own span in SM cycles; 8 blocks per SM run concurrently, so span ~ kernel time
     if (h_sm_clock_mhz) *h_sm_clock_mhz = double(cycles0) / (double(ms) * 1e3);
