@@ -20,6 +20,16 @@
  *            v += (dt/2) ACC F/m ; r += dt v ; recompute F ; v += (dt/2) ACC F/m
  *   KE = 1/2 m sum |v|^2 / ACC ;  T = 2 KE / (kB (3N - 3))        (reading Q5)
  *   rescale thermostat after the second half kick: v *= sqrt(T_target / T)   (reading Q6)
+ *   Langevin thermostat ("Langevin thermostat with a damping constant of
+ *            10 ps^-1"; the discretisation is not stated -- reading Q18): after the second
+ *            half kick of step k the exact Ornstein-Uhlenbeck update over dt,
+ *              v <- c1 v + c2 xi,  c1 = exp(-gamma dt),  c2 = sqrt((1 - c1^2) kB T_k ACC / m),
+ *            T_k the same linear ramp as the rescale thermostat, xi standard normal per
+ *            component, drawn from the counter-based generator Philox4x32-10 (Salmon et al.,
+ *            SC'11) with key = (seed lo, seed hi) and counter = (atom index, step lo, step hi, 0),
+ *            step = step0 + k - 1; words w0..w3 -> u_t = (w_t + 1/2) 2^-32;
+ *              xi_x = sqrt(-2 ln u0) cos(2 pi u1), xi_y = sqrt(-2 ln u0) sin(2 pi u1),
+ *              xi_z = sqrt(-2 ln u2) cos(2 pi u3)                      (Box-Muller).
  *   cutoff variant (not in the paper; reading Q7): a pair contributes to
  *            rho, pair energy and force iff r2 < r_cut*r_cut, strict, where the decision
  *            value is r2 = fma(dz, dz, fma(dy, dy, dx*dx)) in binary64 with
@@ -42,7 +52,9 @@
  * Parity pins: tests/test_oracle_pins.py (closed-form dimer / triangle / tetrahedron /
  * icosahedron / cuboctahedron, mpmath brute force, F = -grad E by central differences,
  * Newton's third law, zero torque, rigid-motion invariance, homogeneity, NVE drift,
- * time reversal, bulk-limit lattice sums, SURVEY.md's independently computed values).
+ * time reversal, bulk-limit lattice sums, SURVEY.md's independently computed values;
+ * Langevin: Philox known-answer vectors, an independent Python restatement of the chain for
+ * N = 1, the gamma -> 0 and T = 0 limits, equipartition of free particles).
  * Nothing here is "parity unpinned" except absolute energies against a published
  * number -- the paper prints none.
  */
@@ -168,6 +180,36 @@ static void kinetic_real(int64_t N, const real *vel, double mass, real *ke, real
     *temp = ndof > 0 ? 2 * k / ((real)ORACLE_KB * (real)ndof) : (real)0;
 }
 
+/* Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): ten rounds of
+ *   (c0, c1, c2, c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0))
+ * with the key bumped by the Weyl constants between rounds. */
+static void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* the three standard normals of (atom, step) under `seed` -- see the header */
+static void langevin_normals(uint64_t seed, uint64_t atom, uint64_t step, double xi[3]) {
+    const uint32_t ctr[4] = {(uint32_t)atom, (uint32_t)step, (uint32_t)(step >> 32), 0u};
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t w[4];
+    philox4x32_10(ctr, key, w);
+    const double two_pi = 6.283185307179586476925286766559;
+    double u0 = ((double)w[0] + 0.5) / 4294967296.0, u1 = ((double)w[1] + 0.5) / 4294967296.0;
+    double u2 = ((double)w[2] + 0.5) / 4294967296.0, u3 = ((double)w[3] + 0.5) / 4294967296.0;
+    double ra = sqrt(-2.0 * log(u0)), rb = sqrt(-2.0 * log(u2));
+    xi[0] = ra * cos(two_pi * u1);
+    xi[1] = ra * sin(two_pi * u1);
+    xi[2] = rb * cos(two_pi * u3);
+}
+
 /* ------------------------------------------------------------------------------------ */
 /* exported C entry points (ctypes)                                                       */
 /* ------------------------------------------------------------------------------------ */
@@ -262,17 +304,21 @@ int64_t oracle_count_pairs(int64_t N, const double *pos, double r_cut) {
     return total;
 }
 
+void oracle_philox4x32_10(const uint32_t *ctr, const uint32_t *key, uint32_t *out) { philox4x32_10(ctr, key, out); }
+void oracle_langevin_normals(uint64_t seed, uint64_t atom, uint64_t step, double *xi) { langevin_normals(seed, atom, step, xi); }
+
 /*
  * nsteps of velocity-Verlet from (pos, vel), in place.
  *   thermo_kind 0: NVE.   1: rescale after the second half kick of step k (k = 1..nsteps)
  *   to T_target(k) = T_start + (T_end - T_start) * k / nsteps   (reading Q6).
+ *   2: Langevin (reading Q18; gamma in 1/fs, seed, step0 = generator step of this call's first step).
  * Traces (may be NULL), length nsteps + 1, index 0 = initial state:
  *   epot_trace[k], ekin_trace[k] after step k (after the rescale, if any).
  * pos_trace (may be NULL): (nsteps+1) * N * 3 positions.
  * The state is carried in `real` across the whole run.
  */
 int oracle_run(int64_t N, double *pos, double *vel, const oracle_params *p, double dt, int64_t nsteps,
-               int32_t thermo_kind, double T_start, double T_end,
+               int32_t thermo_kind, double T_start, double T_end, double gamma, uint64_t seed, uint64_t step0,
                double *epot_trace, double *ekin_trace, double *pos_trace) {
     size_t n3 = 3 * (size_t)(N > 0 ? N : 1);
     real *x = (real *)malloc(sizeof(real) * n3);
@@ -304,6 +350,16 @@ int oracle_run(int64_t N, double *pos, double *vel, const oracle_params *p, doub
             real target = (real)T_start + ((real)T_end - (real)T_start) * (real)k / (real)nsteps;
             real lambda = temp > 0 ? R_SQRT(target / temp) : (real)1;
             for (int64_t i = 0; i < 3 * N; ++i) v[i] *= lambda;
+            kinetic_real(N, v, p->mass, &ke, &temp);
+        } else if (thermo_kind == 2) {
+            real target = (real)T_start + ((real)T_end - (real)T_start) * (real)k / (real)nsteps;
+            real c1 = (real)exp(-gamma * dt);
+            real c2 = R_SQRT(((real)1 - c1 * c1) * (real)ORACLE_KB * target * (real)ORACLE_ACC / (real)p->mass);
+            for (int64_t i = 0; i < N; ++i) {
+                double xi[3];
+                langevin_normals(seed, (uint64_t)i, step0 + (uint64_t)(k - 1), xi);
+                for (int d = 0; d < 3; ++d) v[3 * i + d] = c1 * v[3 * i + d] + c2 * (real)xi[d];
+            }
             kinetic_real(N, v, p->mass, &ke, &temp);
         }
         if (epot_trace) epot_trace[k] = (double)(ep + ee);

@@ -68,7 +68,13 @@ class Oracle:
         L.oracle_count_pairs.argtypes = [ctypes.c_int64, _DP, ctypes.c_double]
         L.oracle_count_pairs.restype = ctypes.c_int64
         L.oracle_run.argtypes = [ctypes.c_int64, _DP, _DP, PP, ctypes.c_double, ctypes.c_int64,
-                                 ctypes.c_int32, ctypes.c_double, ctypes.c_double, _DP, _DP, _DP]
+                                 ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                 ctypes.c_uint64, ctypes.c_uint64, _DP, _DP, _DP]
+        U32P = ctypes.POINTER(ctypes.c_uint32)
+        L.oracle_philox4x32_10.argtypes = [U32P, U32P, U32P]
+        L.oracle_philox4x32_10.restype = None
+        L.oracle_langevin_normals.argtypes = [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, _DP]
+        L.oracle_langevin_normals.restype = None
 
     @staticmethod
     def params(n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0) -> OracleParams:
@@ -132,8 +138,21 @@ class Oracle:
         p = self._pos(pos)
         return int(self.lib.oracle_count_pairs(p.shape[0], _dptr(p), float(r_cut)))
 
+    def philox4x32_10(self, ctr, key) -> np.ndarray:
+        c = np.ascontiguousarray(ctr, dtype=np.uint32); k = np.ascontiguousarray(key, dtype=np.uint32)
+        out = np.zeros(4, dtype=np.uint32)
+        U32P = ctypes.POINTER(ctypes.c_uint32)
+        self.lib.oracle_philox4x32_10(c.ctypes.data_as(U32P), k.ctypes.data_as(U32P), out.ctypes.data_as(U32P))
+        return out
+
+    def langevin_normals(self, seed: int, atom: int, step: int) -> np.ndarray:
+        xi = np.zeros(3)
+        self.lib.oracle_langevin_normals(int(seed), int(atom), int(step), _dptr(xi))
+        return xi
+
     def run(self, pos, vel, params: OracleParams, dt: float, nsteps: int, thermo_kind: int = 0,
-            T_start: float = 0.0, T_end: float = 0.0, traces: bool = True, pos_trace: bool = False):
+            T_start: float = 0.0, T_end: float = 0.0, traces: bool = True, pos_trace: bool = False,
+            gamma: float = 0.0, seed: int = 0, step0: int = 0):
         """-> dict(pos, vel, epot[nsteps+1], ekin[nsteps+1], pos_trace or None)"""
         p = self._pos(pos).copy()
         v = np.ascontiguousarray(vel, dtype=np.float64).copy()
@@ -142,7 +161,8 @@ class Oracle:
         ek = np.zeros(nsteps + 1) if traces else None
         pt = np.zeros((nsteps + 1, n, 3)) if pos_trace else None
         rc = self.lib.oracle_run(n, _dptr(p), _dptr(v), ctypes.byref(params), float(dt), int(nsteps),
-                                 int(thermo_kind), float(T_start), float(T_end), _dptr(ep), _dptr(ek), _dptr(pt))
+                                 int(thermo_kind), float(T_start), float(T_end), float(gamma), int(seed), int(step0),
+                                 _dptr(ep), _dptr(ek), _dptr(pt))
         assert rc == 0
         return dict(pos=p, vel=v, epot=ep, ekin=ek, pos_trace=pt)
 
