@@ -13,8 +13,10 @@
  *           exactly as PAPER.md:127 reduces the many-body term;
  *   velocity-Verlet time stepping, dt in fs ("Verlet integrator with a
  *           time-step of 1 fs"), optionally followed by a velocity-rescale thermostat
- *           (BASELINE.json config 3; the paper's Langevin thermostat, is
- *           listed as SC_THERMO_LANGEVIN and not implemented yet).
+ *           (BASELINE.json config 3) or by the paper's Langevin thermostat ("a
+ *           Langevin thermostat with a damping constant of 10 ps^-1" = 0.01 fs^-1), discretised as
+ *           the exact Ornstein-Uhlenbeck velocity update after the second half kick (see
+ *           sc_thermostat).
  *   Parameters for nickel: eps = 1.5707e-2 eV, a = 3.52 A, c = 39.432,
  *           n = 9, m = 6.  The paper runs all pairs with no cutoff; r_cut > 0
  *           selects the cell-list / Verlet-list variant BASELINE.json adds: a pair counts in
@@ -77,11 +79,20 @@ typedef enum {
 typedef enum { SC_THERMO_NONE = 0, SC_THERMO_RESCALE = 1, SC_THERMO_LANGEVIN = 2 } sc_thermo_kind;
 
 typedef struct {
-    int32_t kind;           /* sc_thermo_kind; SC_THERMO_LANGEVIN returns SC_ERR_INVALID (next) */
-    double T_start, T_end;  /* K; step k = 1..nsteps of ONE sc_step call is rescaled, after its
-                               second half kick, to T_start + (T_end - T_start) * k / nsteps    */
-    double gamma;           /* 1/fs; Langevin only                                              */
-    uint64_t seed;          /* Langevin only                                                    */
+    int32_t kind;           /* sc_thermo_kind                                                   */
+    double T_start, T_end;  /* K; the bath temperature of step k = 1..nsteps of ONE sc_step call is
+                               T_k = T_start + (T_end - T_start) * k / nsteps.
+                               RESCALE: after the second half kick, v *= sqrt(T_k / T).
+                               LANGEVIN: after the second half kick, v <- c1 v + c2 xi with
+                               c1 = exp(-gamma dt), c2 = sqrt((1 - c1^2) kB T_k SC_ACC / mass)    */
+    double gamma;           /* 1/fs; Langevin only (10 ps^-1 = 0.01)              */
+    uint64_t seed;          /* Langevin only: xi = Box-Muller normals of Philox4x32-10 with key
+                               (seed lo, seed hi), counter (atom index in the caller's order,
+                               step lo, step hi, 0); the generator step starts at 0 at sc_create,
+                               advances by one per Langevin step and can be set with
+                               SC_OPT_LANGEVIN_STEP (resume): results do not depend on how a run
+                               is split into sc_step calls, on the precision mode's atom order
+                               or on the launch configuration                                   */
 } sc_thermostat;
 
 /* Runtime options (sc_set_option).  Values are integers; 0 always means "library default". */
@@ -92,7 +103,8 @@ typedef enum {
     SC_OPT_PERSISTENT = 4,        /* 1: whole sc_step loop in one cooperative kernel (small N);
                                      2: never; 0: choose by N                                    */
     SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
-    SC_OPT_NEIGHBOUR_CAPACITY = 6 /* K_max rows of the Verlet list (cutoff path)                */
+    SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max rows of the Verlet list (cutoff path)                */
+    SC_OPT_LANGEVIN_STEP = 7      /* generator step of the next Langevin update (>= 0)          */
 } sc_option;
 
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */

@@ -13,7 +13,7 @@ SC_OK, SC_ERR_INVALID, SC_ERR_CUDA, SC_ERR_NOMEM, SC_ERR_STATE, SC_ERR_NONFINITE
 SC_PREC_FP64, SC_PREC_MIXED = 0, 1
 SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN = 0, 1, 2
 (SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
- SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY) = range(1, 7)
+ SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY, SC_OPT_LANGEVIN_STEP) = range(1, 8)
 _STATUS_NAMES = ["SC_OK", "SC_ERR_INVALID", "SC_ERR_CUDA", "SC_ERR_NOMEM", "SC_ERR_STATE",
                  "SC_ERR_NONFINITE", "SC_ERR_CAPACITY"]
 
@@ -251,6 +251,10 @@ class SuttonChen:
 
 def rescale_thermostat(T_start: float, T_end: float) -> ScThermostat:
     return ScThermostat(SC_THERMO_RESCALE, float(T_start), float(T_end), 0.0, 0)
+
+
+def langevin_thermostat(T_start: float, T_end: float, gamma_per_fs: float, seed: int) -> ScThermostat:
+    return ScThermostat(SC_THERMO_LANGEVIN, float(T_start), float(T_end), float(gamma_per_fs), int(seed))
 
 
 def probe_throughput(kind: int):

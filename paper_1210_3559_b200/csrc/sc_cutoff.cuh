@@ -67,6 +67,7 @@ struct RebuildArgs {
     double r_list, half_skin2;
 };
 
+#ifdef SCMD_MAIN_TU
 __device__ __forceinline__ int cell_coord(double x, double o, double inv_edge, int n) {
     const double t = (x - o) * inv_edge;
     int c = t <= 0.0 ? 0 : (t >= double(n) ? n - 1 : int(t));
@@ -274,6 +275,8 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
     }
 }
 
+#endif  // SCMD_MAIN_TU
+
 // --------------------------------------------------------------------------------------------
 // list-driven sweeps
 // --------------------------------------------------------------------------------------------
@@ -461,6 +464,7 @@ __global__ void __launch_bounds__(kNlistBlock) nlist_kernel(const NlistArgs a) {
     }
 }
 
+#ifdef SCMD_MAIN_TU
 // caller's order <-> internal order at the boundary
 __global__ void scatter_by_perm_kernel(const double *__restrict__ src, double *__restrict__ dst,
                                        const int *__restrict__ perm, int N, int width) {
@@ -488,5 +492,6 @@ __global__ void reset_list_state_kernel(unsigned long long *__restrict__ counter
     scal[kSlotMaxDisp2] = 0.0;
 }
 __global__ void zero_u64_kernel(unsigned long long *p) { *p = 0ull; }
+#endif  // SCMD_MAIN_TU
 
 }  // namespace scmd

@@ -20,6 +20,7 @@ enum ScalarSlot {
     kNumScalars = 16
 };
 
+#ifdef SCMD_MAIN_TU   // the non-template kernels are compiled in scmd.cu only
 // pos[N*3] -> xs[N] = (x, y, z, 0); xf (mixed all-pairs path, else NULL) gets the split record
 __global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, FPair *__restrict__ xf,
                                       int N) {
@@ -93,6 +94,54 @@ __global__ void kick_ke_kernel(double *__restrict__ vel, const double *__restric
     if (threadIdx.x == 0) part[blockIdx.x] = t;
 }
 
+// Langevin thermostat (reading Q18 of DESIGN.md): after the second half kick the exact
+// Ornstein-Uhlenbeck update v <- c1 v + c2 xi, xi = three standard normals per (atom, step) from
+// Philox4x32-10 keyed by the seed, counter = (caller's atom index, step lo, step hi, 0).
+struct LangevinArgs {
+    double c1, c2;                  // exp(-gamma dt), sqrt((1 - c1^2) kB T ACC / m)
+    uint32_t key0, key1;            // seed lo, hi
+    uint32_t step_lo, step_hi;      // generator step
+    const int *perm;                // internal -> caller's atom index (cutoff path), else NULL
+};
+
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c.x), l0 = 0xD2511F53u * c.x;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c.z), l1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(h1 ^ c.y ^ k0, l1, h0 ^ c.w ^ k1, l0);
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return c;
+}
+__device__ __forceinline__ double unit_open(uint32_t w) { return (double(w) + 0.5) * 2.3283064365386963e-10; }  // 2^-32
+
+// second half kick + Langevin update + per-block sum of |v|^2 -> part[blockIdx.x]
+__global__ void kick_langevin_ke_kernel(double *__restrict__ vel, const double *__restrict__ force,
+                                        double *__restrict__ part, int N, double hk, const LangevinArgs lg) {
+    __shared__ double scratch[32];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double v2 = 0.0;
+    if (i < N) {
+        double vx = fma(hk, force[3 * size_t(i)], vel[3 * size_t(i)]);
+        double vy = fma(hk, force[3 * size_t(i) + 1], vel[3 * size_t(i) + 1]);
+        double vz = fma(hk, force[3 * size_t(i) + 2], vel[3 * size_t(i) + 2]);
+        const uint32_t atom = uint32_t(lg.perm ? lg.perm[i] : i);
+        const uint4 w = philox4x32_10(make_uint4(atom, lg.step_lo, lg.step_hi, 0u), lg.key0, lg.key1);
+        const double ra = sqrt(-2.0 * log(unit_open(w.x))), rb = sqrt(-2.0 * log(unit_open(w.z)));
+        double sa, ca, sb, cb;
+        sincospi(2.0 * unit_open(w.y), &sa, &ca);
+        sincospi(2.0 * unit_open(w.w), &sb, &cb);
+        vx = fma(lg.c1, vx, lg.c2 * (ra * ca));
+        vy = fma(lg.c1, vy, lg.c2 * (ra * sa));
+        vz = fma(lg.c1, vz, lg.c2 * (rb * cb));
+        vel[3 * size_t(i)] = vx; vel[3 * size_t(i) + 1] = vy; vel[3 * size_t(i) + 2] = vz;
+        v2 = fma(vz, vz, fma(vy, vy, vx * vx));
+    }
+    const double t = block_sum(v2, scratch);
+    if (threadIdx.x == 0) part[blockIdx.x] = t;
+}
+
 // per-block sum of |v|^2 without a kick (sc_kinetic)
 __global__ void sum_v2_kernel(const double *__restrict__ vel, double *__restrict__ part, int N, double lambda_apply,
                               const double *__restrict__ scal) {
@@ -148,5 +197,7 @@ __global__ void reduce_ke_kernel(const double *__restrict__ part, int n, double 
         scal[kSlotLambda] = lambda;
     }
 }
+
+#endif  // SCMD_MAIN_TU
 
 }  // namespace scmd

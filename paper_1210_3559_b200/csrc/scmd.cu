@@ -9,8 +9,8 @@
 #include <new>
 #include <vector>
 
-#include "sc_allpairs.cuh"
-#include "sc_cutoff.cuh"
+#define SCMD_MAIN_TU 1   // this translation unit compiles the non-template kernels
+#include "sc_dispatch.h"
 #include "sc_device.cuh"
 #include "sc_integrate.cuh"
 #include "sc_probe.cuh"
@@ -80,6 +80,7 @@ struct sc_ctx {
     bool density_valid = false, forces_valid = false, energy_valid = false;
     bool lambda_pending = false;
     int64_t launches = 0;
+    uint64_t langevin_step = 0;   // generator step of the next Langevin update (SC_OPT_LANGEVIN_STEP)
 
     struct OccEntry { const void *fn; int warps; int per_sm; };
     std::vector<OccEntry> occ_cache;
@@ -189,35 +190,10 @@ double ipow_host(double u, int k) {
 // ---------------------------------------------------------------------------------------------
 struct TileChoice { int it, tpr, warps; };
 
-template <bool MIXED, int IT, int TPR, int NE, int ME>
-const void *allpairs_fn_t(bool force, bool energy) {
-    if constexpr (MIXED) {
-        if (!force) return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, false, false>);
-        if (energy) return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, true, true>);
-        return reinterpret_cast<const void *>(allpairs32_kernel<IT, TPR, NE, ME, true, false>);
-    } else {
-        if (!force) return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, false, false>);
-        if (energy) return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, true, true>);
-        return reinterpret_cast<const void *>(allpairs64_kernel<IT, TPR, NE, ME, true, false>);
-    }
-}
-
-template <bool MIXED, int NE, int ME>
-const void *allpairs_fn_nm(int it, int tpr, bool force, bool energy) {
-#define SC_CASE(IT, TPR) \
-    if (it == IT && tpr == TPR) return allpairs_fn_t<MIXED, IT, TPR, NE, ME>(force, energy);
-    SC_CASE(1, 1) SC_CASE(1, 2) SC_CASE(1, 4) SC_CASE(1, 8) SC_CASE(1, 16) SC_CASE(1, 32)
-    SC_CASE(2, 1) SC_CASE(2, 2) SC_CASE(2, 4) SC_CASE(2, 8) SC_CASE(2, 16) SC_CASE(2, 32)
-    if constexpr (NE != 0) { SC_CASE(4, 1) SC_CASE(4, 2) SC_CASE(4, 4) }
-#undef SC_CASE
-    return nullptr;
-}
-
 const void *allpairs_fn(const sc_ctx *c, int it, int tpr, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    if (!fast && it > 2) return nullptr;
-    if (mixed) return fast ? allpairs_fn_nm<true, 9, 6>(it, tpr, force, energy) : allpairs_fn_nm<true, 0, 0>(it, tpr, force, energy);
-    return fast ? allpairs_fn_nm<false, 9, 6>(it, tpr, force, energy) : allpairs_fn_nm<false, 0, 0>(it, tpr, force, energy);
+    if (mixed) return fast ? allpairs32_fn_96(it, tpr, force, energy) : allpairs32_fn_generic(it, tpr, force, energy);
+    return fast ? allpairs64_fn_96(it, tpr, force, energy) : allpairs64_fn_generic(it, tpr, force, energy);
 }
 
 // resident CTAs per SM of one instantiation at (warps + 1) * 32 threads; cached per context
@@ -299,37 +275,6 @@ int choose_tpa(const sc_ctx *c) {
     return tpa;
 }
 
-template <int TPA, int NE, int ME>
-cudaError_t launch_nlist_t(const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
-    const int atoms_per_block = kNlistBlock / TPA;
-    const int grid = ceil_div(a.n_atoms, atoms_per_block);
-    auto go = [&](auto kernel) -> cudaError_t {
-        kernel<<<grid, kNlistBlock, 0, st>>>(a);
-        return cudaGetLastError();
-    };
-    if (!mixed) {
-        if (!force) return go(nlist_kernel<TPA, NE, ME, false, false, false>);
-        if (energy) return go(nlist_kernel<TPA, NE, ME, true, true, false>);
-        return go(nlist_kernel<TPA, NE, ME, true, false, false>);
-    }
-    if (!force) return go(nlist_kernel<TPA, NE, ME, false, false, true>);
-    if (energy) return go(nlist_kernel<TPA, NE, ME, true, true, true>);
-    return go(nlist_kernel<TPA, NE, ME, true, false, true>);
-}
-
-template <int NE, int ME>
-cudaError_t launch_nlist_nm(int tpa, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
-    switch (tpa) {
-        case 1: return launch_nlist_t<1, NE, ME>(a, force, energy, mixed, st);
-        case 2: return launch_nlist_t<2, NE, ME>(a, force, energy, mixed, st);
-        case 4: return launch_nlist_t<4, NE, ME>(a, force, energy, mixed, st);
-        case 8: return launch_nlist_t<8, NE, ME>(a, force, energy, mixed, st);
-        case 16: return launch_nlist_t<16, NE, ME>(a, force, energy, mixed, st);
-        case 32: return launch_nlist_t<32, NE, ME>(a, force, energy, mixed, st);
-    }
-    return cudaErrorInvalidConfiguration;
-}
-
 sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     sc_status st = ensure_list(c);
     if (st != SC_OK) return st;
@@ -342,8 +287,8 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     a.c = c->consts;
     if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    cudaError_t e = fast ? launch_nlist_nm<9, 6>(tpa, a, force, energy, mixed, c->stream)
-                         : launch_nlist_nm<0, 0>(tpa, a, force, energy, mixed, c->stream);
+    cudaError_t e = fast ? launch_nlist_96(tpa, a, force, energy, mixed, c->stream)
+                         : launch_nlist_generic(tpa, a, force, energy, mixed, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "list sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     if (!force || energy) {
@@ -453,10 +398,12 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     int thermo = SC_THERMO_NONE;
     if (th) {
         thermo = th->kind;
-        if (thermo == SC_THERMO_LANGEVIN) return fail(c, SC_ERR_INVALID, "sc_step: Langevin thermostat is not implemented%s");
-        if (thermo != SC_THERMO_NONE && thermo != SC_THERMO_RESCALE) return fail(c, SC_ERR_INVALID, "sc_step: unknown thermostat kind%s");
-        if (thermo == SC_THERMO_RESCALE && !(th->T_start >= 0.0 && th->T_end >= 0.0))
-            return fail(c, SC_ERR_INVALID, "sc_step: thermostat temperatures must be >= 0%s");
+        if (thermo != SC_THERMO_NONE && thermo != SC_THERMO_RESCALE && thermo != SC_THERMO_LANGEVIN)
+            return fail(c, SC_ERR_INVALID, "sc_step: unknown thermostat kind%s");
+        if (thermo != SC_THERMO_NONE && !(th->T_start >= 0.0 && th->T_end >= 0.0 && std::isfinite(th->T_start) && std::isfinite(th->T_end)))
+            return fail(c, SC_ERR_INVALID, "sc_step: thermostat temperatures must be finite and >= 0%s");
+        if (thermo == SC_THERMO_LANGEVIN && !(th->gamma >= 0.0 && std::isfinite(th->gamma)))
+            return fail(c, SC_ERR_INVALID, "sc_step: Langevin damping must be finite and >= 0 (1/fs)%s");
     }
     if (nsteps == 0) return SC_OK;
     sc_status st = ensure_forces(c, false);
@@ -474,7 +421,19 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
         const bool last = (k == nsteps);
         st = ensure_forces(c, last || c->opt_energy_every == 1);
         if (st != SC_OK) return st;
-        kick_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk);
+        if (thermo == SC_THERMO_LANGEVIN) {
+            const double target = th->T_start + (th->T_end - th->T_start) * double(k) / double(nsteps);
+            LangevinArgs lg{};
+            lg.c1 = std::exp(-th->gamma * dt);
+            lg.c2 = std::sqrt((1.0 - lg.c1 * lg.c1) * kBoltzmann * target * kAcc / c->p.mass);
+            lg.key0 = uint32_t(th->seed); lg.key1 = uint32_t(th->seed >> 32);
+            lg.step_lo = uint32_t(c->langevin_step); lg.step_hi = uint32_t(c->langevin_step >> 32);
+            lg.perm = c->cutoff ? c->perm : nullptr;
+            kick_langevin_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk, lg);
+            c->langevin_step += 1;
+        } else {
+            kick_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk);
+        }
         c->launches += 1;
         if (thermo == SC_THERMO_RESCALE || last) {
             const double target = thermo == SC_THERMO_RESCALE
@@ -609,6 +568,9 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
                 c->density_valid = c->forces_valid = c->energy_valid = false;
             }
             break;
+        case SC_OPT_LANGEVIN_STEP:
+            if (value < 0) return fail(c, SC_ERR_INVALID, "Langevin generator step must be >= 0%s");
+            c->langevin_step = uint64_t(value); break;
         default:
             return fail(c, SC_ERR_INVALID, "unknown option%s");
     }
