@@ -98,13 +98,20 @@ typedef struct {
 /* Runtime options (sc_set_option).  Values are integers; 0 always means "library default". */
 typedef enum {
     SC_OPT_ROWS_PER_THREAD = 1,   /* i-atoms held in registers per thread: 1, 2 or 4           */
-    SC_OPT_LANES_PER_ROW = 2,     /* lanes of a warp that share one row group: 1,2,4,8,16,32    */
+    SC_OPT_LANES_PER_ROW = 2,     /* lanes of a warp that share one row group: 1,2,4,8,16,32
+                                     (list sweeps: lanes per neighbour row, 8, 16 or 32; smaller
+                                     values are raised to 8)                                     */
     SC_OPT_WARPS_PER_CTA = 3,     /* consumer warps per CTA (they split the j range): 1..8      */
     SC_OPT_PERSISTENT = 4,        /* 1: whole sc_step loop in one cooperative kernel (small N);
                                      2: never; 0: choose by N                                    */
     SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
-    SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max rows of the Verlet list (cutoff path)                */
-    SC_OPT_LANGEVIN_STEP = 7      /* generator step of the next Langevin update (>= 0)          */
+    SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max entries per row of the Verlet list (cutoff path); rounded
+                                     down to a multiple of 32 (at least 32)                      */
+    SC_OPT_LANGEVIN_STEP = 7,     /* generator step of the next Langevin update (>= 0)          */
+    SC_OPT_CELLS_PER_RADIUS = 8,  /* cutoff path: cell edge = list radius / G, G = 1..4 (default 4);
+                                     takes effect at the next list build                         */
+    SC_OPT_ATOMS_PER_CTA = 9      /* cutoff path: consecutive atoms one CTA of the list sweeps
+                                     works through (rounded to the warp layout)                  */
 } sc_option;
 
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */

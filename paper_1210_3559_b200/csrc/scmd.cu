@@ -65,13 +65,13 @@ struct sc_ctx {
     // cutoff path (r_cut > 0); all null otherwise
     bool cutoff = false;
     double r_list = 0.0;
-    int kmax = 0, kmax_cap = 0, npad = 0, max_dim = 1, coop_grid = 0;
+    int kmax = 0, kmax_cap = 0, max_dim = 1, coop_grid = 0;
     bool list_checked = false;    // rebuild_kernel already launched for the current positions
     double4 *xs_alt = nullptr, *xs_ref = nullptr;
     double *vel_alt = nullptr, *blockpart = nullptr;
     int *perm = nullptr, *perm_alt = nullptr, *cell_of = nullptr, *slot_of = nullptr, *cell_sorted = nullptr;
     int *cell_count = nullptr, *cell_start = nullptr, *order_tmp = nullptr, *order = nullptr;
-    int *nlist = nullptr, *ncount = nullptr;
+    int *nlist = nullptr, *ncount = nullptr, *scanpart = nullptr;
     CellGrid *grid = nullptr;
     unsigned long long *counters = nullptr;
 
@@ -86,7 +86,7 @@ struct sc_ctx {
     std::vector<OccEntry> occ_cache;
 
     // options (0 = default)
-    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0;
+    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0;
 
     // profiling
     bool profile = false;
@@ -126,8 +126,10 @@ int default_kmax(const sc_params *p, int64_t N, double skin) {
     if (k < 1) k = 1;
     return round_up(k, 32);
 }
+// cell budget: fine cells of edge r_list / 4 hold ~2 atoms at metallic densities and a sphere fills half
+// of its bounding box, so ~N cells are needed; 4 N leaves room for dilute clusters
 int cutoff_max_dim(int64_t N) {
-    const int64_t cap = N / 4 + 512;
+    const int64_t cap = 4 * N + 4096;
     int d = 1;
     while (int64_t(d + 1) * (d + 1) * (d + 1) <= cap) ++d;
     return d;
@@ -156,7 +158,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         if (c && base) c->xf = xf;
     }
     if (prm->r_cut > 0.0) {
-        const int kmax = default_kmax(prm, N, skin), npad = round_up(N, 32), md = cutoff_max_dim(N);
+        const int kmax = default_kmax(prm, N, skin), md = cutoff_max_dim(N);
         const size_t ncell = size_t(md) * md * md + 2;
         double4 *xa = w.take<double4>(n + kTileAtoms);
         double4 *xr = w.take<double4>(n);
@@ -165,15 +167,16 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         int *perm = w.take<int>(n), *perm_alt = w.take<int>(n), *cell_of = w.take<int>(n), *slot_of = w.take<int>(n);
         int *cell_sorted = w.take<int>(n), *order_tmp = w.take<int>(n), *order = w.take<int>(n), *ncount = w.take<int>(n);
         int *cell_count = w.take<int>(ncell), *cell_start = w.take<int>(ncell);
-        int *nlist = w.take<int>(size_t(kmax) * size_t(npad));
+        int *nlist = w.take<int>(size_t(kmax) * n);
+        int *scanpart = w.take<int>(size_t(kMaxCoopBlocks) + 1);
         CellGrid *grid = w.take<CellGrid>(1);
         unsigned long long *counters = w.take<unsigned long long>(kNumCounters);
         if (c && base) {
             c->xs_alt = xa; c->xs_ref = xr; c->vel_alt = va; c->blockpart = bp; c->perm = perm; c->perm_alt = perm_alt;
             c->cell_of = cell_of; c->slot_of = slot_of; c->cell_sorted = cell_sorted; c->order_tmp = order_tmp;
             c->order = order; c->ncount = ncount; c->cell_count = cell_count; c->cell_start = cell_start;
-            c->nlist = nlist; c->grid = grid; c->counters = counters;
-            c->kmax = c->kmax_cap = kmax; c->npad = npad; c->max_dim = md;
+            c->nlist = nlist; c->scanpart = scanpart; c->grid = grid; c->counters = counters;
+            c->kmax = c->kmax_cap = kmax; c->max_dim = md;
         }
     }
     return w.total();
@@ -255,8 +258,9 @@ sc_status ensure_list(sc_ctx *c) {
     a.perm = c->perm; a.perm_alt = c->perm_alt; a.cell_of = c->cell_of; a.slot_of = c->slot_of;
     a.cell_sorted = c->cell_sorted; a.cell_count = c->cell_count; a.cell_start = c->cell_start;
     a.order_tmp = c->order_tmp; a.order = c->order; a.nlist = c->nlist; a.ncount = c->ncount;
-    a.blockpart = c->blockpart; a.grid = c->grid; a.scal = c->scal; a.counters = c->counters;
-    a.n_atoms = int(c->N); a.npad = c->npad; a.kmax = c->kmax; a.max_dim = c->max_dim;
+    a.blockpart = c->blockpart; a.scanpart = c->scanpart; a.grid = c->grid; a.scal = c->scal; a.counters = c->counters;
+    a.n_atoms = int(c->N); a.kmax = c->kmax; a.max_dim = c->max_dim;
+    a.fine_max = c->opt_fine ? c->opt_fine : kFineMax;
     a.have_vel = c->have_vel ? 1 : 0;
     a.r_list = c->r_list; a.half_skin2 = 0.25 * c->skin * c->skin;
     void *params[] = {&a};
@@ -268,31 +272,39 @@ sc_status ensure_list(sc_ctx *c) {
     return SC_OK;
 }
 
-int choose_tpa(const sc_ctx *c) {
-    if (c->opt_tpr) return c->opt_tpr;
-    int tpa = 1;
-    while (tpa < 32 && c->N * tpa < int64_t(c->sm_count) * 1024) tpa *= 2;
-    return tpa;
+// lanes per atom of the list sweeps: one warp per row (adjacent lanes gather adjacent records)
+int choose_lpa(const sc_ctx *c) {
+    if (c->opt_tpr) return c->opt_tpr < 8 ? 8 : c->opt_tpr;
+    return 32;
+}
+// consecutive atoms per CTA: short runs balance the SMs better than long ones keep L1 warm (measured:
+// N = 65536: 8 and 16 atoms tie, 32 and more lose 5-70 %; N = 2^20: 32 beats 8 by 7 %)
+int choose_atoms_per_cta(const sc_ctx *c, int lpa) {
+    const int step = kNlistWarps * (32 / lpa);
+    int64_t apc = c->opt_apc ? c->opt_apc : (c->N >= 262144 ? 32 : (c->N >= 4096 ? 8 : 4));
+    apc = apc / step * step;
+    return int(apc < step ? step : apc);
 }
 
 sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     sc_status st = ensure_list(c);
     if (st != SC_OK) return st;
-    const int tpa = choose_tpa(c);
+    const int lpa = choose_lpa(c);
     NlistArgs a{};
-    a.xs = c->xs; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.npad = c->npad;
+    a.xs = c->xs; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.kmax = c->kmax;
+    a.atoms_per_cta = choose_atoms_per_cta(c, lpa);
     a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
     a.pairs_in_cut = c->counters + kCntPairsInCut;
     a.rc2 = c->p.r_cut * c->p.r_cut;
     a.c = c->consts;
     if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    cudaError_t e = fast ? launch_nlist_96(tpa, a, force, energy, mixed, c->stream)
-                         : launch_nlist_generic(tpa, a, force, energy, mixed, c->stream);
+    cudaError_t e = fast ? launch_nlist_96(lpa, a, force, energy, mixed, c->stream)
+                         : launch_nlist_generic(lpa, a, force, energy, mixed, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "list sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     if (!force || energy) {
-        const int grid = ceil_div(c->N, kNlistBlock / tpa);
+        const int grid = ceil_div(c->N, a.atoms_per_cta);
         reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
                                                          force ? c->consts.En : -c->consts.eps_c);
         SC_CUDA_CHECK(c, cudaGetLastError());
@@ -562,7 +574,7 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
                 return fail(c, SC_ERR_INVALID, "neighbour capacity must be 0 .. the capacity the workspace was sized for%s");
             c->opt_kmax = int(value);
             if (c->cutoff) {
-                c->kmax = value ? int(value) : c->kmax_cap;
+                c->kmax = value ? (value < 32 ? 32 : int(value) / 32 * 32) : c->kmax_cap;   // rows are padded to 32
                 c->list_checked = false;
                 reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
                 c->density_valid = c->forces_valid = c->energy_valid = false;
@@ -571,6 +583,18 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
         case SC_OPT_LANGEVIN_STEP:
             if (value < 0) return fail(c, SC_ERR_INVALID, "Langevin generator step must be >= 0%s");
             c->langevin_step = uint64_t(value); break;
+        case SC_OPT_CELLS_PER_RADIUS:
+            if (value < 0 || value > kFineMax) return fail(c, SC_ERR_INVALID, "cells per list radius must be 0..4%s");
+            c->opt_fine = int(value);
+            if (c->cutoff) {
+                c->list_checked = false;
+                reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
+                c->density_valid = c->forces_valid = c->energy_valid = false;
+            }
+            break;
+        case SC_OPT_ATOMS_PER_CTA:
+            if (value < 0 || value > 4096) return fail(c, SC_ERR_INVALID, "atoms per CTA must be 0..4096%s");
+            c->opt_apc = int(value); break;
         default:
             return fail(c, SC_ERR_INVALID, "unknown option%s");
     }

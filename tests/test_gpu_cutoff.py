@@ -75,7 +75,7 @@ def test_c3_ni8000_liquid_rc10(scmd, oracle_ld, precision):
     check(scmd, oracle_ld, w.pos, 10.0, precision=precision)
 
 
-@pytest.mark.parametrize("tpa", [1, 2, 4, 8, 16, 32])
+@pytest.mark.parametrize("tpa", [4, 8, 16, 32])
 @pytest.mark.parametrize("precision", [0, 1])
 def test_lanes_per_atom_ragged(scmd, oracle_ld, tpa, precision):
     """Every lanes-per-atom family on N = 2607 (not a multiple of 32 or of the atoms per CTA)."""
