@@ -1,0 +1,340 @@
+// sc_small.cuh -- the whole velocity-Verlet loop of sc_step in ONE cooperative launch, for clusters
+// small enough that a step is bound by launch latency rather than by the FP64 pipe (the paper's own
+// production size, Ni2057 for 6.5e7 steps; BASELINE.json configs 1 and 2).
+//
+// The multi-launch path needs 6-7 dependent launches per step (~40-50 us at N <= 2000, of which the
+// pair arithmetic is < 5 us).  Here the grid stays resident and the phases of a step are separated
+// by grid-wide barriers instead of launch boundaries:
+//
+//   A  owners: v <- lambda v; v += hk F; x += dt v                     (rows of this CTA only)
+//      ---- grid barrier 1: all positions of the step are in global memory ----
+//   B  every CTA stages all N records into shared memory; sweep 1 for its own rows:
+//      rho_i, s'_i = eps (c m / 2) a^m rho_i^-1/2 -> sprime[i]
+//      ---- grid barrier 2: all s' are in global memory ----
+//   C  stage the s' (8 bytes per atom); sweep 2 for its own rows: F_i and sum_j r^-n
+//   D  owners: v += hk F [Langevin update]; |v|^2
+//      rescale thermostat only: ---- grid barrier 3 ----, every CTA forms the same kinetic energy
+//      from the per-CTA partials in a fixed order and scales its own velocities.
+//
+// Decomposition: a CTA owns `rows` consecutive atoms; JL (a power of two) threads share one row and
+// stride the j range; their partial sums meet in a shuffle tree (and across warps through shared
+// memory when JL > 32), always in the same order: results are bit-reproducible.  The row's first
+// thread ("owner") keeps v and F of its atom in registers for the whole call.
+#pragma once
+#include "sc_allpairs.cuh"
+#include "sc_device.cuh"
+#include "sc_integrate.cuh"
+
+namespace scmd {
+
+constexpr int kSmallThreads = 512;
+constexpr int kSmallMaxAtoms = 6144;         // N * 32 B of records must fit in shared memory
+
+struct SmallStepArgs {
+    double4 *xs;            // [N] (x, y, z, s'): the state at entry and at exit
+    double4 *xs_b;          // [N] second buffer: step k works in (k odd ? xs_b : xs), so that a CTA already in
+                            //     phase A of step k + 1 never overwrites records another CTA still stages
+    double *vel, *force, *rho;
+    double *part_emb, *part_pair, *part_ke;   // [gridDim.x]
+    double *sprime;         // [N] s' of the current step, contiguous (phase C re-stages only these 8 bytes per atom)
+    unsigned long long *barrier;      // grid barrier counter; grows by gridDim.x per barrier
+    unsigned long long barrier_base;  // its value when this launch starts (the host keeps count)
+    double *scal;
+    int n_atoms, rows, jl;  // rows per CTA; threads per row (power of two, rows * jl <= kSmallThreads)
+    long long nsteps;
+    double hk, dt, mass, ndof;
+    int thermo;             // sc_thermo_kind
+    double T_start, T_end;
+    double lg_c1, lg_pre;   // Langevin: c1 = exp(-gamma dt); c2_k = sqrt(lg_pre * T_k * ACC / mass), lg_pre = (1 - c1^2) kB
+    uint32_t key0, key1;
+    unsigned long long lg_step0;
+    PairConsts c;
+};
+
+inline size_t small_step_smem_bytes(int n_atoms) {
+    return size_t(n_atoms) * sizeof(double4) + (kSmallThreads / 32) * 4 * sizeof(double) + kSmallThreads * sizeof(double);
+}
+
+#ifdef SCMD_MAIN_TU
+__device__ __forceinline__ double4 load_record_cg(const double4 *p) {    // L2 (coherent) load, bypasses L1
+    double4 r;
+    asm volatile("ld.global.cg.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+    return r;
+}
+
+// sum over the JL threads of a row; valid in the row's first thread.  JL <= 32: shuffle tree inside the
+// warp; JL > 32: shuffle tree per warp, then the row's first thread adds the per-warp values in order.
+template <int NV>
+__device__ __forceinline__ void row_reduce(double (&v)[NV], int jl, int q, double *warp_red) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int width = jl < 32 ? jl : 32;
+    for (int off = width >> 1; off > 0; off >>= 1)
+#pragma unroll
+        for (int c = 0; c < NV; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], off);
+    if (jl > 32) {                                          // block-uniform
+        __syncthreads();
+        if (lane == 0)
+#pragma unroll
+            for (int c = 0; c < NV; ++c) warp_red[warp * 4 + c] = v[c];
+        __syncthreads();
+        if (q == 0) {
+            const int nw = jl >> 5;
+#pragma unroll
+            for (int c = 0; c < NV; ++c) {
+                double s = 0.0;
+                for (int w = 0; w < nw; ++w) s += warp_red[(warp + w) * 4 + c];
+                v[c] = s;
+            }
+        }
+    }
+}
+
+// fixed-order sum of one value per row over the rows of the CTA; result valid in thread 0
+__device__ __forceinline__ double rows_sum(double mine, bool owner, int r, int nrows, double *rowval) {
+    __syncthreads();
+    if (owner) rowval[r] = mine;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int k = 0; k < nrows; ++k) s += rowval[k];
+    return s;
+}
+
+// fixed-order sum of part[0..n) by warp 0 (every CTA gets the same bits); valid in all lanes of warp 0
+__device__ __forceinline__ double warp0_sum_partials(const double *part, int n) {
+    const int lane = threadIdx.x & 31;
+    double s = 0.0;
+    for (int k = lane; k < n; k += 32) s += __ldcg(part + k);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    return s;
+}
+
+// Grid-wide barrier on a monotonically increasing counter (all CTAs are resident: cooperative launch).
+// Release: every thread's writes -> bar.sync -> thread 0: fence + atomic add.  Acquire: thread 0 spins on
+// an acquire load until all CTAs of this generation have arrived -> bar.sync.
+__device__ __forceinline__ void grid_barrier(unsigned long long *counter, unsigned long long target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(counter, 1ull);
+        unsigned long long seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(counter) : "memory");
+        } while (seen < target);
+    }
+    __syncthreads();
+}
+
+// one term of sweep 1: r^-m (self == true: the reciprocal is replaced by 0, so the term is exactly 0)
+template <int ME>
+__device__ __forceinline__ double small_density_term(const double4 &pi, const double4 &p, bool self, int m_exp) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    r2 = self ? 1.0 : r2;
+    if constexpr (ME > 0 && ME % 2 == 0) {
+        const double w = self ? 0.0 : rcp_fast(r2);
+        return ipow_c<ME / 2>(w);
+    } else {
+        const double y = self ? 0.0 : rsqrt_fast(r2);
+        return (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+    }
+}
+
+// one term of sweep 2 added into (fx, fy, fz, sum r^-n)
+template <int NE, int ME>
+__device__ __forceinline__ void small_force_term(const double4 &pi, const double4 &p, bool self, double An, int n_exp,
+                                                 int m_exp, double (&acc)[4]) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    r2 = self ? 1.0 : r2;
+    const double y = self ? 0.0 : rsqrt_fast(r2);          // self: every power below is exactly 0
+    const double w = y * y;
+    const double ss = pi.w + p.w;
+    double coef, pn;
+    if constexpr (NE == 9 && ME == 6) {
+        const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
+        coef = w4 * fma(An, y3, -ss);
+        pn = w4 * y;
+    } else {
+        const double pm = (ME > 0) ? ipow_c<ME>(y) : ipow_rt(y, m_exp);
+        pn = (NE > 0) ? ipow_c<NE>(y) : ipow_rt(y, n_exp);
+        coef = w * fma(An, pn, -ss * pm);
+    }
+    acc[0] = fma(coef, dx, acc[0]);
+    acc[1] = fma(coef, dy, acc[1]);
+    acc[2] = fma(coef, dz, acc[2]);
+    acc[3] += pn;
+}
+
+template <int NE, int ME>
+__global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const SmallStepArgs a) {
+    unsigned long long bar_target = a.barrier_base;
+    auto grid_sync = [&]() { bar_target += gridDim.x; grid_barrier(a.barrier, bar_target); };
+    extern __shared__ __align__(32) unsigned char smem_raw[];
+    const int N = a.n_atoms;
+    double4 *sm = reinterpret_cast<double4 *>(smem_raw);
+    double *warp_red = reinterpret_cast<double *>(sm + N);
+    double *rowval = warp_red + (kSmallThreads / 32) * 4;
+    __shared__ double s_lambda;
+
+    const int t = threadIdx.x, JL = a.jl;
+    const int r = t / JL, q = t % JL;
+    const int row0 = blockIdx.x * a.rows;
+    const int nrows = min(a.rows, N - row0);
+    const int i = row0 + r;
+    const bool rowlive = r < nrows;
+    const bool owner = rowlive && q == 0;
+    const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
+    const double An = a.c.An;
+
+    double vx = 0, vy = 0, vz = 0, fx = 0, fy = 0, fz = 0, my_rho = 0;
+    if (owner) {
+        vx = a.vel[3 * size_t(i)]; vy = a.vel[3 * size_t(i) + 1]; vz = a.vel[3 * size_t(i) + 2];
+        fx = a.force[3 * size_t(i)]; fy = a.force[3 * size_t(i) + 1]; fz = a.force[3 * size_t(i) + 2];
+    }
+    double lambda = a.scal[kSlotLambda];                   // a scale left pending by an earlier call
+    double e_emb = 0.0, e_pair = 0.0, ke_sum = 0.0;        // thread 0: this CTA's partials of the last step
+    double ke_final = 0.0, temp_final = 0.0;
+
+    double px = 0, py = 0, pz = 0, sp = 0;                 // owner: position and s' of its atom
+    auto stage = [&](const double4 *cur) {
+        __syncthreads();                                    // everyone is done with the previous contents
+        for (int j = t; j < N; j += kSmallThreads) sm[j] = load_record_cg(cur + j);
+        __syncthreads();
+    };
+
+    for (long long k = 1; k <= a.nsteps; ++k) {
+        double4 *cur = (k & 1) ? a.xs_b : a.xs;
+        // ---- A: first half kick + drift ----
+        if (owner) {
+            vx *= lambda; vy *= lambda; vz *= lambda;
+            vx = fma(a.hk, fx, vx); vy = fma(a.hk, fy, vy); vz = fma(a.hk, fz, vz);
+            double4 p = sm[i];                              // staged in phase C of the previous step
+            if (k == 1) p = load_record_cg(a.xs + i);
+            p.x = fma(a.dt, vx, p.x); p.y = fma(a.dt, vy, p.y); p.z = fma(a.dt, vz, p.z);
+            px = p.x; py = p.y; pz = p.z;
+            cur[i] = p;
+        }
+        lambda = 1.0;
+        grid_sync();
+
+        // ---- B: sweep 1 ----
+        stage(cur);
+        {
+            double acc[1] = {0.0};
+            if (rowlive) {
+                const double4 pi = sm[i];
+                double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;   // 4 independent chains; summed in a fixed order
+                int j = q;
+                for (; j + 3 * JL < N; j += 4 * JL) {
+                    t0 += small_density_term<ME>(pi, sm[j], j == i, m_exp);              // self term excluded by index
+                    t1 += small_density_term<ME>(pi, sm[j + JL], j + JL == i, m_exp);
+                    t2 += small_density_term<ME>(pi, sm[j + 2 * JL], j + 2 * JL == i, m_exp);
+                    t3 += small_density_term<ME>(pi, sm[j + 3 * JL], j + 3 * JL == i, m_exp);
+                }
+                for (; j < N; j += JL) t0 += small_density_term<ME>(pi, sm[j], j == i, m_exp);
+                acc[0] = (t0 + t1) + (t2 + t3);
+            }
+            row_reduce<1>(acc, JL, q, warp_red);
+            double root = 0.0;
+            if (owner) {
+                my_rho = a.c.am * acc[0];
+                root = my_rho > 0.0 ? sqrt(my_rho) : 0.0;                    // reading Q9
+                sp = my_rho > 0.0 ? a.c.Bm / root : 0.0;
+                a.sprime[i] = sp;
+            }
+            if (k == a.nsteps) e_emb = rows_sum(root, owner, r, nrows, rowval);
+        }
+        grid_sync();
+
+        // ---- C: sweep 2 (positions are still staged; fetch the s' of this step) ----
+        for (int j = t; j < N; j += kSmallThreads) sm[j].w = __ldcg(a.sprime + j);
+        __syncthreads();
+        {
+            double acc[4] = {0.0, 0.0, 0.0, 0.0};
+            if (rowlive) {
+                const double4 pi = sm[i];
+                double b[4] = {0.0, 0.0, 0.0, 0.0};               // second chain
+                int j = q;
+                for (; j + JL < N; j += 2 * JL) {
+                    small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
+                    small_force_term<NE, ME>(pi, sm[j + JL], j + JL == i, An, n_exp, m_exp, b);
+                }
+                if (j < N) small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[c] += b[c];
+            }
+            row_reduce<4>(acc, JL, q, warp_red);
+            // ---- D: second half kick (+ Langevin), |v|^2 ----
+            double v2 = 0.0;
+            if (owner) {
+                fx = acc[0]; fy = acc[1]; fz = acc[2];
+                vx = fma(a.hk, fx, vx); vy = fma(a.hk, fy, vy); vz = fma(a.hk, fz, vz);
+                if (a.thermo == 2) {
+                    const double target = a.T_start + (a.T_end - a.T_start) * double(k) / double(a.nsteps);
+                    const double c2 = sqrt(a.lg_pre * target * kAcc / a.mass);
+                    const unsigned long long step = a.lg_step0 + (unsigned long long)(k - 1);
+                    const uint4 wd = philox4x32_10(make_uint4(uint32_t(i), uint32_t(step), uint32_t(step >> 32), 0u), a.key0, a.key1);
+                    const double ra = sqrt(-2.0 * log(unit_open(wd.x))), rb = sqrt(-2.0 * log(unit_open(wd.z)));
+                    double sa, ca, sb, cb;
+                    sincospi(2.0 * unit_open(wd.y), &sa, &ca);
+                    sincospi(2.0 * unit_open(wd.w), &sb, &cb);
+                    vx = fma(a.lg_c1, vx, c2 * (ra * ca));
+                    vy = fma(a.lg_c1, vy, c2 * (ra * sa));
+                    vz = fma(a.lg_c1, vz, c2 * (rb * cb));
+                }
+                v2 = fma(vz, vz, fma(vy, vy, vx * vx));
+            }
+            const bool last = (k == a.nsteps);
+            if (last) e_pair = rows_sum(acc[3], owner, r, nrows, rowval);
+            if (a.thermo == 1 || last) {
+                ke_sum = rows_sum(v2, owner, r, nrows, rowval);
+                if (t == 0) a.part_ke[blockIdx.x] = ke_sum;
+                grid_sync();
+                // every CTA forms the same total (same order, same bits)
+                if (t < 32) {
+                    const double tot = warp0_sum_partials(a.part_ke, int(gridDim.x));
+                    if (t == 0) {
+                        double ke = 0.5 * a.mass * tot / kAcc;
+                        double temp = a.ndof > 0.0 ? 2.0 * ke / (kBoltzmann * a.ndof) : 0.0;
+                        double lam = 1.0;
+                        if (a.thermo == 1 && temp > 0.0) {
+                            const double target = a.T_start + (a.T_end - a.T_start) * double(k) / double(a.nsteps);
+                            lam = sqrt(target / temp);
+                            ke *= lam * lam;
+                            temp = a.ndof > 0.0 ? 2.0 * ke / (kBoltzmann * a.ndof) : 0.0;
+                        }
+                        s_lambda = lam; ke_final = ke; temp_final = temp;
+                    }
+                }
+                __syncthreads();
+                lambda = s_lambda;
+            }
+        }
+    }
+
+    // ---- epilogue: state back to global memory, scalars ----
+    if (owner) {
+        a.vel[3 * size_t(i)] = vx * lambda; a.vel[3 * size_t(i) + 1] = vy * lambda; a.vel[3 * size_t(i) + 2] = vz * lambda;
+        a.force[3 * size_t(i)] = fx; a.force[3 * size_t(i) + 1] = fy; a.force[3 * size_t(i) + 2] = fz;
+        a.rho[i] = my_rho;
+        a.xs[i] = make_double4(px, py, pz, sp);             // after the last barrier: nobody stages any more
+    }
+    if (t == 0) { a.part_emb[blockIdx.x] = e_emb; a.part_pair[blockIdx.x] = e_pair; }
+    grid_sync();
+    if (blockIdx.x == 0 && t < 32) {
+        const double emb = warp0_sum_partials(a.part_emb, int(gridDim.x));
+        const double pair = warp0_sum_partials(a.part_pair, int(gridDim.x));
+        if (t == 0) {
+            a.scal[kSlotEEmb] = -a.c.eps_c * emb;
+            a.scal[kSlotEPair] = a.c.En * pair;
+            a.scal[kSlotKE] = ke_final;
+            a.scal[kSlotTemp] = temp_final;
+            a.scal[kSlotLambda] = 1.0;
+        }
+    }
+}
+#endif  // SCMD_MAIN_TU
+
+}  // namespace scmd

@@ -14,6 +14,7 @@
 #include "sc_device.cuh"
 #include "sc_integrate.cuh"
 #include "sc_probe.cuh"
+#include "sc_small.cuh"
 
 using namespace scmd;
 
@@ -51,6 +52,10 @@ struct sc_ctx {
 
     // device arrays (all inside the caller's workspace)
     double4 *xs = nullptr;        // [N] (x, y, z, s')
+    double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
+    unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
+    unsigned long long small_barrier_count = 0;
+    double4 *xs_b = nullptr;      // [N] second record buffer of the one-launch step loop (small all-pairs clusters)
     FPair *xf = nullptr;          // [(N + 512) / 2 + 1] packed split binary32 records (mixed all-pairs path only)
     double *vel = nullptr;        // [N*3]
     double *force = nullptr;      // [N*3]
@@ -65,7 +70,7 @@ struct sc_ctx {
     // cutoff path (r_cut > 0); all null otherwise
     bool cutoff = false;
     double r_list = 0.0;
-    int kmax = 0, kmax_cap = 0, max_dim = 1, coop_grid = 0;
+    int kmax = 0, kmax_cap = 0, max_dim = 1, coop_grid = 0, small_ctas = 0;
     bool list_checked = false;    // rebuild_kernel already launched for the current positions
     double4 *xs_alt = nullptr, *xs_ref = nullptr;
     double *vel_alt = nullptr, *blockpart = nullptr;
@@ -145,13 +150,19 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
     double *rho = w.take<double>(n);
     double *pa = w.take<double>(n + 1);
     double *pb = w.take<double>(n + 1);
-    double *pk = w.take<double>(size_t(ceil_div(N, kBlock)) + 1);
+    double *pk = w.take<double>(size_t(ceil_div(N, kBlock)) + 1 + 1024);   // also the per-CTA partials of the one-launch loop
     double *scal = w.take<double>(kNumScalars);
     double *sa = w.take<double>(3 * n);
     double *sb = w.take<double>(3 * n);
     if (c && base) {
         c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
+    }
+    if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms) {
+        double4 *xb = w.take<double4>(n);
+        double *spr = w.take<double>(n);
+        unsigned long long *bar = w.take<unsigned long long>(2);
+        if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
     }
     if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
         FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
@@ -404,6 +415,63 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
     return SC_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// one-launch step loop (sc_small.cuh): small all-pairs FP64 clusters
+// ---------------------------------------------------------------------------------------------
+constexpr int64_t kSmallDefaultMaxAtoms = kSmallMaxAtoms;   // measured: the loop beats the multi-launch path up to its capacity
+
+bool small_path_wanted(const sc_ctx *c) {
+    if (c->cutoff || c->precision != SC_PREC_FP64 || !c->xs_b || c->opt_persistent == 2 || c->profile) return false;
+    if (c->N > kSmallMaxAtoms) return false;
+    return c->opt_persistent == 1 || c->N <= kSmallDefaultMaxAtoms;
+}
+
+sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int thermo, int64_t nsteps) {
+    const bool fast = (c->p.n == 9 && c->p.m == 6);
+    const void *fn = fast ? reinterpret_cast<const void *>(small_step_kernel<9, 6>)
+                          : reinterpret_cast<const void *>(small_step_kernel<0, 0>);
+    const int N = int(c->N);
+    const size_t smem = small_step_smem_bytes(N);
+    if (c->small_ctas == 0) {
+        int per_sm = 0;
+        SC_CUDA_CHECK(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+        SC_CUDA_CHECK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kSmallThreads, smem));
+        if (per_sm < 1) return fail(c, SC_ERR_CUDA, "one-launch step loop: kernel does not fit on an SM%s");
+        c->small_ctas = c->sm_count;                    // one CTA per SM: the barrier cost grows with the CTA count
+    }
+    SmallStepArgs a{};
+    a.xs = c->xs; a.xs_b = c->xs_b; a.vel = c->vel; a.force = c->force; a.rho = c->rho;
+    a.part_emb = c->part_a; a.part_pair = c->part_b; a.part_ke = c->part_ke; a.scal = c->scal;
+    a.sprime = c->sprime; a.barrier = c->small_barrier; a.barrier_base = c->small_barrier_count;
+    a.n_atoms = N;
+    a.rows = ceil_div(N, c->small_ctas);
+    const int grid = ceil_div(N, a.rows);
+    int jl = 1;
+    while (jl * 2 * a.rows <= kSmallThreads && jl < 512) jl *= 2;
+    a.jl = jl;
+    a.nsteps = nsteps; a.hk = 0.5 * dt * kAcc / c->p.mass; a.dt = dt; a.mass = c->p.mass; a.ndof = double(3 * c->N - 3);
+    a.thermo = thermo;
+    if (th) { a.T_start = th->T_start; a.T_end = th->T_end; }
+    if (thermo == SC_THERMO_LANGEVIN) {
+        a.lg_c1 = std::exp(-th->gamma * dt);
+        a.lg_pre = (1.0 - a.lg_c1 * a.lg_c1) * kBoltzmann;
+        a.key0 = uint32_t(th->seed); a.key1 = uint32_t(th->seed >> 32);
+        a.lg_step0 = c->langevin_step;
+    }
+    a.c = c->consts;
+    void *params[] = {&a};
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kSmallThreads), params, smem, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "one-launch step loop: %s", cudaGetErrorString(e));
+    c->launches += 1;
+    // barriers of this launch: 2 per step, a third on rescale steps and on the last step, one in the epilogue
+    const uint64_t nbar = 2 * uint64_t(nsteps) + (thermo == SC_THERMO_RESCALE ? uint64_t(nsteps) : 1) + 1;
+    c->small_barrier_count += nbar * uint64_t(grid);
+    if (thermo == SC_THERMO_LANGEVIN) c->langevin_step += uint64_t(nsteps);
+    c->lambda_pending = false;                           // consumed (and the last scale applied) by the kernel
+    c->density_valid = c->forces_valid = c->energy_valid = true;
+    return SC_OK;
+}
+
 sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps) {
     if (!c->have_pos || !c->have_vel) return fail(c, SC_ERR_STATE, "sc_step: positions and velocities must be set%s");
     if (!(dt > 0.0) || !std::isfinite(dt) || nsteps < 0) return fail(c, SC_ERR_INVALID, "sc_step: dt must be > 0, nsteps >= 0%s");
@@ -420,6 +488,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     if (nsteps == 0) return SC_OK;
     sc_status st = ensure_forces(c, false);
     if (st != SC_OK) return st;
+    if (small_path_wanted(c)) return run_small_steps(c, dt, th, thermo, nsteps);
     const int N = int(c->N);
     const int nb = ceil_div(N, kBlock);
     const double hk = 0.5 * dt * kAcc / c->p.mass;
@@ -517,6 +586,10 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     }
     reset_lambda_kernel<<<1, 1, 0, c->stream>>>(c->scal);
     if (cudaGetLastError() != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    if (c->small_barrier && cudaMemsetAsync(c->small_barrier, 0, 2 * sizeof(unsigned long long), c->stream) != cudaSuccess) {
+        delete c;
+        return SC_ERR_CUDA;
+    }
     if (params->r_cut > 0.0) {
         c->cutoff = true;
         c->r_list = params->r_cut + skin;
