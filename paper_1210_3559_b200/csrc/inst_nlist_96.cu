@@ -4,10 +4,11 @@
 namespace scmd {
 namespace {
 template <int LPA>
-cudaError_t launch(const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
-    const int grid = (a.n_atoms + a.atoms_per_cta - 1) / a.atoms_per_cta;
+cudaError_t launch(int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
+    const int n_pairs = (a.n_atoms + 1) / 2;
+    const int grid = (n_pairs + a.pairs_per_cta - 1) / a.pairs_per_cta;
     auto go = [&](auto kernel) -> cudaError_t {
-        kernel<<<grid, kNlistBlock, 0, st>>>(a);
+        kernel<<<grid, block, 0, st>>>(a);
         return cudaGetLastError();
     };
     if (!mixed) {
@@ -21,11 +22,11 @@ cudaError_t launch(const NlistArgs &a, bool force, bool energy, bool mixed, cuda
 }
 }  // namespace
 
-cudaError_t launch_nlist_96(int lpa, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
+cudaError_t launch_nlist_96(int lpa, int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st) {
     switch (lpa) {
-        case 8: return launch<8>(a, force, energy, mixed, st);
-        case 16: return launch<16>(a, force, energy, mixed, st);
-        case 32: return launch<32>(a, force, energy, mixed, st);
+        case 8: return launch<8>(block, a, force, energy, mixed, st);
+        case 16: return launch<16>(block, a, force, energy, mixed, st);
+        case 32: return launch<32>(block, a, force, energy, mixed, st);
     }
     return cudaErrorInvalidConfiguration;
 }

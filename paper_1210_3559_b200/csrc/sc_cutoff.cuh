@@ -76,7 +76,7 @@ struct RebuildArgs {
     int *cell_of, *slot_of, *cell_sorted;
     int *cell_count, *cell_start;   // [ncell_max + 1]
     int *order_tmp, *order;
-    int *nlist, *ncount;            // rows: nlist[k * kmax + e], ascending j, padded with n_atoms to a multiple of 32
+    int *nlist, *ncount;            // pair rows: nlist[g * 2 kmax + e], g = k / 2; padded with n_atoms to a multiple of 32
     double *blockpart;              // [9 * gridDim.x]
     int *scanpart;                  // [gridDim.x + 1]
     CellGrid *grid;
@@ -290,52 +290,94 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
     if (gtid == 0) a.xs[N] = make_double4(kFarAway, kFarAway, kFarAway, 0.0);   // the dummy record
     grid.sync();
 
-    // ---- P8: neighbour rows, one warp per atom ----
+    // ---- P8: neighbour rows, one warp per PAIR of consecutive atoms (k0 = 2g, k1 = 2g + 1) ----
+    // The row of a pair is the union of the two atoms' neighbourhoods (they sit in the same or in
+    // adjacent fine cells, so the union is ~1.2x one neighbourhood): the sweeps fetch every record once
+    // for two rows i.  Capacity of a pair row: 2 * kmax entries.
     const double rl2 = a.r_list * a.r_list;
     const double rl2_cells = rl2 * g.inv_edge * g.inv_edge;           // (list radius / edge)^2
     const int G = g.fine;
     const unsigned lt_mask = (1u << lane) - 1u;
-    int my_max = 0;
+    const int cap = 2 * a.kmax;
+    int my_max = 0;                                                    // longest single-atom neighbourhood
+    bool my_overflow = false;
     const int gwarp = gtid >> 5, nwarps = gsize >> 5;
-    for (int k = gwarp; k < N; k += nwarps) {
-        const double4 p = a.xs[k];
-        const int c = a.cell_sorted[k];
-        const int cx = c % g.nx, cy = (c / g.nx) % g.ny, cz = c / (g.nx * g.ny);
-        int *row = a.nlist + size_t(k) * a.kmax;
-        int cnt = 0;
-        for (int zz = max(cz - G, 0); zz <= min(cz + G, g.nz - 1); ++zz) {
-            const int adz = max(abs(zz - cz) - 1, 0);
-            for (int yy = max(cy - G, 0); yy <= min(cy + G, g.ny - 1); ++yy) {
-                const int ady = max(abs(yy - cy) - 1, 0);
-                // cells of this row whose nearest point can be inside the list sphere
-                const double rem = rl2_cells - double(adz * adz + ady * ady);
-                if (!(rem > 0.0)) continue;
-                const int mx = min(G, int(sqrt(rem)) + 1);
-                const int rowc = (zz * g.ny + yy) * g.nx;
-                const int jb = a.cell_start[rowc + max(cx - mx, 0)], je = a.cell_start[rowc + min(cx + mx, g.nx - 1) + 1];
-                for (int j0 = jb; j0 < je; j0 += 32) {
-                    const int j = j0 + lane;
-                    bool ok = false;
-                    if (j < je) {
-                        const double4 q = a.xs[j];
-                        const double dx = p.x - q.x, dy = p.y - q.y, dz = p.z - q.z;
-                        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                        ok = (r2 < rl2) && (j != k);
-                    }
-                    const unsigned m = __ballot_sync(0xffffffffu, ok);
-                    const int at = cnt + __popc(m & lt_mask);
-                    if (ok && at < a.kmax) row[at] = j;
-                    cnt += __popc(m);
+    const int npairs = (N + 1) >> 1;
+    for (int gp = gwarp; gp < npairs; gp += nwarps) {
+        const int k0 = 2 * gp, k1 = k0 + 1;
+        const bool has1 = k1 < N;
+        const double4 p0 = a.xs[k0];
+        const double4 p1 = a.xs[has1 ? k1 : N];                        // odd N: the dummy record, never in range
+        const int c0 = a.cell_sorted[k0], c1 = has1 ? a.cell_sorted[k1] : c0;
+        const int cx0 = c0 % g.nx, cy0 = (c0 / g.nx) % g.ny, cz0 = c0 / (g.nx * g.ny);
+        const int cx1 = c1 % g.nx, cy1 = (c1 / g.nx) % g.ny, cz1 = c1 / (g.nx * g.ny);
+        int *row = a.nlist + size_t(gp) * cap;
+        int cnt = 0, cnt0 = 0, cnt1 = 0;
+        // x-range of cells of the row (yy, zz) that can hold a neighbour of an atom in cell (cx, cy, cz)
+        auto xrange = [&](int cx, int cy, int cz, int yy, int zz, int &lo, int &hi) -> bool {
+            const int adz = max(abs(zz - cz) - 1, 0), ady = max(abs(yy - cy) - 1, 0);
+            if (abs(zz - cz) > G || abs(yy - cy) > G) return false;
+            const double rem = rl2_cells - double(adz * adz + ady * ady);
+            if (!(rem > 0.0)) return false;
+            const int mx = min(G, int(sqrt(rem)) + 1);
+            lo = max(cx - mx, 0); hi = min(cx + mx, g.nx - 1);
+            return true;
+        };
+        auto scan = [&](int jb, int je) {
+            for (int j0 = jb; j0 < je; j0 += 32) {
+                const int j = j0 + lane;
+                bool in0 = false, in1 = false;
+                if (j < je) {
+                    const double4 q = a.xs[j];
+                    const double ax = p0.x - q.x, ay = p0.y - q.y, az = p0.z - q.z;
+                    const double bx = p1.x - q.x, by = p1.y - q.y, bz = p1.z - q.z;
+                    in0 = fma(az, az, fma(ay, ay, ax * ax)) < rl2;
+                    in1 = fma(bz, bz, fma(by, by, bx * bx)) < rl2;
                 }
+                const bool ok = in0 || in1;                             // includes k0 and k1 themselves: excluded
+                const unsigned m = __ballot_sync(0xffffffffu, ok);      // by index in the sweeps
+                const int at = cnt + __popc(m & lt_mask);
+                if (ok && at < cap) row[at] = j;
+                cnt += __popc(m);
+                cnt0 += __popc(__ballot_sync(0xffffffffu, in0 && j != k0));
+                cnt1 += __popc(__ballot_sync(0xffffffffu, in1 && j != k1));
+            }
+        };
+        const bool near = abs(cx0 - cx1) <= 2 * G && abs(cy0 - cy1) <= 2 * G && abs(cz0 - cz1) <= 2 * G;
+        if (near) {
+            // one pass over the bounding box of the two stencils, each row of cells once
+            for (int zz = max(min(cz0, cz1) - G, 0); zz <= min(max(cz0, cz1) + G, g.nz - 1); ++zz)
+                for (int yy = max(min(cy0, cy1) - G, 0); yy <= min(max(cy0, cy1) + G, g.ny - 1); ++yy) {
+                    int lo0, hi0, lo1, hi1;
+                    const bool v0 = xrange(cx0, cy0, cz0, yy, zz, lo0, hi0);
+                    const bool v1 = has1 && xrange(cx1, cy1, cz1, yy, zz, lo1, hi1);
+                    if (!v0 && !v1) continue;
+                    const int lo = v0 ? (v1 ? min(lo0, lo1) : lo0) : lo1;
+                    const int hi = v0 ? (v1 ? max(hi0, hi1) : hi0) : hi1;
+                    const int rowc = (zz * g.ny + yy) * g.nx;
+                    scan(a.cell_start[rowc + lo], a.cell_start[rowc + hi + 1]);
+                }
+        } else {
+            // the stencils are disjoint (the pair straddles the end of a row of cells): one pass each
+            for (int which = 0; which < 2; ++which) {
+                const int cx = which ? cx1 : cx0, cy = which ? cy1 : cy0, cz = which ? cz1 : cz0;
+                for (int zz = max(cz - G, 0); zz <= min(cz + G, g.nz - 1); ++zz)
+                    for (int yy = max(cy - G, 0); yy <= min(cy + G, g.ny - 1); ++yy) {
+                        int lo, hi;
+                        if (!xrange(cx, cy, cz, yy, zz, lo, hi)) continue;
+                        const int rowc = (zz * g.ny + yy) * g.nx;
+                        scan(a.cell_start[rowc + lo], a.cell_start[rowc + hi + 1]);
+                    }
             }
         }
-        const int kept = min(cnt, a.kmax);
-        const int padded = min((kept + 31) & ~31, a.kmax);
+        const int kept = min(cnt, cap);
+        const int padded = min((kept + 31) & ~31, cap);
         if (kept + lane < padded) row[kept + lane] = N;                 // pad with the dummy record
-        if (lane == 0) a.ncount[k] = kept;
-        my_max = max(my_max, cnt);
+        if (lane == 0) a.ncount[gp] = kept;
+        my_max = max(my_max, max(cnt0, cnt1));
+        my_overflow = my_overflow || cnt > cap;
     }
-    if (lane == 0 && my_max > a.kmax) atomicExch(&a.counters[kCntOverflow], 1ull);
+    if (lane == 0 && (my_overflow || my_max > a.kmax)) atomicExch(&a.counters[kCntOverflow], 1ull);
     // counters[kCntMaxRow] is reset below by the one thread that also bumps the build count; a max
     // across the grid needs the reset to happen first, so it lives in its own slot pair:
     if (lane == 0) atomicMax(&a.counters[kNumCounters - 1], (unsigned long long)my_max);
@@ -356,10 +398,10 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
 // --------------------------------------------------------------------------------------------
 struct NlistArgs {
     double4 *xs;              // [N + 1] (x, y, z, s'), internal order; xs[N] = the dummy record at infinity
-    const int *nlist;         // [N][kmax] rows, padded with N to a multiple of 32
-    const int *ncount;        // [N]
+    const int *nlist;         // [ceil(N/2)][2 * kmax] pair rows, padded with N to a multiple of 32
+    const int *ncount;        // [ceil(N/2)]
     int n_atoms, kmax;
-    int atoms_per_cta;        // consecutive atoms one CTA works through (multiple of 4 * 32 / LPA)
+    int pairs_per_cta;        // consecutive atom pairs one CTA works through (multiple of warps * 32 / LPA)
     double *rho;              // [N]    sweep 1
     double *force;            // [N*3]  sweep 2
     double *partial;          // [gridDim.x]
@@ -368,9 +410,7 @@ struct NlistArgs {
     PairConsts c;
 };
 
-constexpr int kNlistBlock = 128;
-constexpr int kNlistWarps = kNlistBlock / 32;
-constexpr int kMixedChunk = 8;      // binary32 partial sums are flushed into binary64 every 8 row entries
+constexpr int kNlistMaxBlock = 256;   // threads per CTA of the list sweeps: 32 * warps, chosen by the host
 
 // one 32-byte record with a single 256-bit load (SASS LDG.E.ENL2.256): one L1 wavefront per line touched
 __device__ __forceinline__ double4 load_record(const double4 *p) {
@@ -379,163 +419,187 @@ __device__ __forceinline__ double4 load_record(const double4 *p) {
     return r;
 }
 
-// LPA lanes per atom (32 / LPA atoms per warp at a time).  A CTA works through atoms_per_cta consecutive
-// atoms of the internal (cell) order, its warps interleaved, so that the records its gathers touch stay
-// in L1.
+// One row entry against one of the two atoms of the pair: the strict binary64 test r^2 < r_c^2 (reading
+// Q7), then the pair terms of the all-pairs sweeps.  `other` is false for the atom's own record (the
+// self term is excluded by index).  BRANCH-FREE: an entry that fails the test runs the same
+// instructions on r^2 := 1 with its reciprocal (square root) replaced by 0, so every term it adds is an
+// exact 0.  (A warp almost never has 32 failing lanes, so a branch would save nothing, and without
+// branches the compiler interleaves the 8 independent chains of a batch: 4 entries x 2 atoms.)
+// MIXED: pair arithmetic in binary32 on the converted binary64 difference, partial sums in f[]
+// (flushed into acc[] by the caller after every batch).
+template <int NE, int ME, bool FORCE, bool ENERGY, bool MIXED>
+__device__ __forceinline__ void nlist_term(const double4 &pi, const double4 &p, bool other, double rc2, double An,
+                                           int n_exp, int m_exp, double (&acc)[4], float (&f)[4], int &npairs) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = (r2 < rc2) && other;
+    if constexpr (!FORCE) npairs += in ? 1 : 0;
+    if constexpr (!MIXED) {
+        const double r2m = in ? r2 : 1.0;
+        if constexpr (!FORCE) {
+            if constexpr (ME > 0 && ME % 2 == 0) {
+                double w = rcp_fast(r2m);
+                w = in ? w : 0.0;
+                if constexpr (ME == 6) acc[0] = fma(w * w, w, acc[0]);
+                else acc[0] += ipow_c<ME / 2>(w);
+            } else {
+                double y = rsqrt_fast(r2m);
+                y = in ? y : 0.0;
+                acc[0] += (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+            }
+        } else {
+            double y = rsqrt_fast(r2m);
+            y = in ? y : 0.0;
+            const double w = y * y;
+            const double ss = pi.w + p.w;
+            double coef;
+            if constexpr (NE == 9 && ME == 6) {
+                const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
+                coef = w4 * fma(An, y3, -ss);
+                if constexpr (ENERGY) acc[3] = fma(w4, y, acc[3]);
+            } else {
+                const double pm = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+                const double pn = (NE > 0) ? ipow_c<(NE > 0 ? NE : 1)>(y) : ipow_rt(y, n_exp);
+                coef = w * fma(An, pn, -ss * pm);
+                if constexpr (ENERGY) acc[3] += pn;
+            }
+            acc[0] = fma(coef, dx, acc[0]);
+            acc[1] = fma(coef, dy, acc[1]);
+            acc[2] = fma(coef, dz, acc[2]);
+        }
+    } else {
+        // masked differences: a far-away record must not turn 0 * inf into NaN in binary32
+        const float fx = in ? float(dx) : 0.f, fy = in ? float(dy) : 0.f, fz = in ? float(dz) : 0.f;
+        const float q2 = in ? fmaf(fz, fz, fmaf(fy, fy, fx * fx)) : 1.0f;
+        if constexpr (!FORCE) {
+            if constexpr (ME > 0 && ME % 2 == 0) {
+                float w = rcp_fast_f(q2);
+                w = in ? w : 0.f;
+                if constexpr (ME == 6) f[0] = fmaf(w * w, w, f[0]);
+                else f[0] += ipow_cf<ME / 2>(w);
+            } else {
+                float y = rsqrt_fast_f(q2);
+                y = in ? y : 0.f;
+                f[0] += (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+            }
+        } else {
+            const float Anf = float(An);
+            float y = rsqrt_fast_f(q2);
+            y = in ? y : 0.f;
+            const float w = y * y;
+            const float ss = float(pi.w) + float(p.w);
+            float coef;
+            if constexpr (NE == 9 && ME == 6) {
+                const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+                coef = w4 * fmaf(Anf, y3, -ss);
+                if constexpr (ENERGY) f[3] = fmaf(w4, y, f[3]);
+            } else {
+                const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+                const float pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+                coef = w * fmaf(Anf, pn, -ss * pm);
+                if constexpr (ENERGY) f[3] += pn;
+            }
+            f[0] = fmaf(coef, fx, f[0]);
+            f[1] = fmaf(coef, fy, f[1]);
+            f[2] = fmaf(coef, fz, f[2]);
+        }
+    }
+}
+
+// LPA lanes per atom PAIR (32 / LPA pairs per warp at a time).  A CTA works through pairs_per_cta
+// consecutive pairs of the internal (cell) order, its warps interleaved, so that the records its
+// gathers touch stay in L1.  Every fetched record serves both atoms of the pair.
 template <int LPA, int NE, int ME, bool FORCE, bool ENERGY, bool MIXED>
-__global__ void __launch_bounds__(kNlistBlock) nlist_kernel(const NlistArgs a) {
-    constexpr int AW = 32 / LPA;                         // atoms per warp
+__global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a) {
+    constexpr int AW = 32 / LPA;                         // pairs per warp
     __shared__ double scratch[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int g = lane / LPA, q = lane % LPA;            // group g of the warp takes one atom, q strides its row
-    const int N = a.n_atoms;
+    const int g = lane / LPA, q = lane % LPA;            // group g of the warp takes one pair, q strides its row
+    const int N = a.n_atoms, NP = (N + 1) >> 1;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An, rc2 = a.rc2;
-    const float Anf = float(An);
+    const size_t stride = 2 * size_t(a.kmax);
     double contrib = 0.0;
     int npairs = 0;
 
-    const int base = blockIdx.x * a.atoms_per_cta;
-    const int end = min(N, base + a.atoms_per_cta);
-    for (int i0 = base + warp * AW; i0 < end; i0 += kNlistWarps * AW) {
-        const int i = i0 + g;
-        const bool live = i < end;
-        const int ii = live ? i : N;                     // idle groups sit on the dummy record, empty row
-        const double4 pi = a.xs[ii];
-        const int cnt = live ? a.ncount[i] : 0;
+    const int base = blockIdx.x * a.pairs_per_cta;
+    const int end = min(NP, base + a.pairs_per_cta);
+    const int nwarps = blockDim.x >> 5;
+    for (int g0 = base + warp * AW; g0 < end; g0 += nwarps * AW) {
+        const int gp = g0 + g;
+        const bool live = gp < end;
+        const int i0 = live ? 2 * gp : N, i1 = (live && 2 * gp + 1 < N) ? 2 * gp + 1 : N;   // N = the dummy record
+        const double4 pa = a.xs[i0], pb = a.xs[i1];
+        const int cnt = live ? a.ncount[gp] : 0;
         const int niter = (cnt + LPA - 1) / LPA;         // rows are padded to a multiple of 32 >= LPA
-        const int *row = a.nlist + size_t(live ? i : 0) * a.kmax + q;
-        const float sif = float(pi.w);
-        double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+        const int *row = a.nlist + size_t(live ? gp : 0) * stride + q;
+        double acc0[4] = {0.0, 0.0, 0.0, 0.0}, acc1[4] = {0.0, 0.0, 0.0, 0.0};
+        float f0[4] = {0.f, 0.f, 0.f, 0.f}, f1[4] = {0.f, 0.f, 0.f, 0.f};
 
-        if constexpr (!MIXED) {
-            auto pair = [&](const double4 &p) {
-                const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                if (r2 < rc2) {
-                    if constexpr (!FORCE) {
-                        ++npairs;
-                        if constexpr (ME > 0 && ME % 2 == 0) {
-                            const double w = rcp_fast(r2);
-                            if constexpr (ME == 6) acc0 = fma(w * w, w, acc0);
-                            else acc0 += ipow_c<ME / 2>(w);
-                        } else if constexpr (ME > 0) {
-                            acc0 += ipow_c<ME>(rsqrt_fast(r2));
-                        } else {
-                            acc0 += ipow_rt(rsqrt_fast(r2), m_exp);
-                        }
-                    } else {
-                        const double y = rsqrt_fast(r2);
-                        const double w = y * y;
-                        const double ss = pi.w + p.w;
-                        double coef;
-                        if constexpr (NE == 9 && ME == 6) {
-                            const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
-                            coef = w4 * fma(An, y3, -ss);
-                            if constexpr (ENERGY) acc3 = fma(w4, y, acc3);
-                        } else {
-                            const double pm = (ME > 0) ? ipow_c<ME>(y) : ipow_rt(y, m_exp);
-                            const double pn = (NE > 0) ? ipow_c<NE>(y) : ipow_rt(y, n_exp);
-                            coef = w * fma(An, pn, -ss * pm);
-                            if constexpr (ENERGY) acc3 += pn;
-                        }
-                        acc0 = fma(coef, dx, acc0);
-                        acc1 = fma(coef, dy, acc1);
-                        acc2 = fma(coef, dz, acc2);
-                    }
-                }
-            };
-            int t = 0;
-            for (; t + 3 < niter; t += 4) {                // 4 independent gathers in flight
-                const int j0 = row[t * LPA], j1 = row[(t + 1) * LPA], j2 = row[(t + 2) * LPA], j3 = row[(t + 3) * LPA];
-                const double4 p0 = load_record(a.xs + j0), p1 = load_record(a.xs + j1);
-                const double4 p2 = load_record(a.xs + j2), p3 = load_record(a.xs + j3);
-                pair(p0); pair(p1); pair(p2); pair(p3);
-            }
-            for (; t < niter; ++t) pair(load_record(a.xs + row[t * LPA]));
-        } else {
-            float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
-            auto pair = [&](const double4 &p) {
-                const double dxd = pi.x - p.x, dyd = pi.y - p.y, dzd = pi.z - p.z;
-                const double r2d = fma(dzd, dzd, fma(dyd, dyd, dxd * dxd));
-                if (r2d < rc2) {                                   // membership decided in binary64 (Q7)
-                    const float dx = float(dxd), dy = float(dyd), dz = float(dzd);
-                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    if constexpr (!FORCE) {
-                        ++npairs;
-                        if constexpr (ME > 0 && ME % 2 == 0) {
-                            const float w = rcp_fast_f(r2);
-                            if constexpr (ME == 6) f0 = fmaf(w * w, w, f0);
-                            else f0 += ipow_cf<ME / 2>(w);
-                        } else if constexpr (ME > 0) {
-                            f0 += ipow_cf<ME>(rsqrt_fast_f(r2));
-                        } else {
-                            f0 += ipow_rtf(rsqrt_fast_f(r2), m_exp);
-                        }
-                    } else {
-                        const float y = rsqrt_fast_f(r2);
-                        const float w = y * y;
-                        const float ss = sif + float(p.w);
-                        float coef;
-                        if constexpr (NE == 9 && ME == 6) {
-                            const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
-                            coef = w4 * fmaf(Anf, y3, -ss);
-                            if constexpr (ENERGY) f3 = fmaf(w4, y, f3);
-                        } else {
-                            const float pm = (ME > 0) ? ipow_cf<ME>(y) : ipow_rtf(y, m_exp);
-                            const float pn = (NE > 0) ? ipow_cf<NE>(y) : ipow_rtf(y, n_exp);
-                            coef = w * fmaf(Anf, pn, -ss * pm);
-                            if constexpr (ENERGY) f3 += pn;
-                        }
-                        f0 = fmaf(coef, dx, f0);
-                        f1 = fmaf(coef, dy, f1);
-                        f2 = fmaf(coef, dz, f2);
-                    }
-                }
-            };
-            auto flush = [&]() {
-                acc0 += double(f0); f0 = 0.f;
-                if constexpr (FORCE) {
-                    acc1 += double(f1); acc2 += double(f2); f1 = f2 = 0.f;
-                    if constexpr (ENERGY) { acc3 += double(f3); f3 = 0.f; }
-                }
-            };
-            int t = 0;
-            for (; t + kMixedChunk - 1 < niter; t += kMixedChunk) {
-                int j[kMixedChunk];
+        auto entry = [&](int j, const double4 &p) {
+            nlist_term<NE, ME, FORCE, ENERGY, MIXED>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, f0, npairs);
+            nlist_term<NE, ME, FORCE, ENERGY, MIXED>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, f1, npairs);
+        };
+        auto flush = [&]() {
+            if constexpr (MIXED) {
 #pragma unroll
-                for (int u = 0; u < kMixedChunk; ++u) j[u] = row[(t + u) * LPA];
-#pragma unroll
-                for (int u = 0; u < kMixedChunk; u += 4) {
-                    const double4 p0 = load_record(a.xs + j[u]), p1 = load_record(a.xs + j[u + 1]);
-                    const double4 p2 = load_record(a.xs + j[u + 2]), p3 = load_record(a.xs + j[u + 3]);
-                    pair(p0); pair(p1); pair(p2); pair(p3);
+                for (int c = 0; c < 4; ++c) {
+                    acc0[c] += double(f0[c]); acc1[c] += double(f1[c]);
+                    f0[c] = 0.f; f1[c] = 0.f;
                 }
-                flush();
             }
-            for (; t < niter; ++t) pair(load_record(a.xs + row[t * LPA]));
+        };
+        // Software pipeline over batches of CH entries per lane: while batch t is in the FP64 pipe the
+        // records of batch t + 1 (indices fetched an iteration earlier) and the indices of batch t + 2
+        // (streamed from HBM) are in flight.  Slots beyond the row read the dummy record.
+        constexpr int CH = 4;
+        const int nbatch = (niter + CH - 1) / CH;
+        auto load_idx = [&](int b, int (&jj)[CH]) {
+#pragma unroll
+            for (int u = 0; u < CH; ++u) {
+                const int it = b * CH + u;
+                jj[u] = it < niter ? row[it * LPA] : N;
+            }
+        };
+        int jc[CH], j1[CH], j2[CH];
+        double4 pc[CH], pn[CH];
+        load_idx(0, jc);
+        load_idx(1, j1);
+#pragma unroll
+        for (int u = 0; u < CH; ++u) pc[u] = load_record(a.xs + jc[u]);
+        for (int b = 0; b < nbatch; ++b) {
+            load_idx(b + 2, j2);
+#pragma unroll
+            for (int u = 0; u < CH; ++u) pn[u] = load_record(a.xs + j1[u]);
+#pragma unroll
+            for (int u = 0; u < CH; ++u) entry(jc[u], pc[u]);
             flush();
+#pragma unroll
+            for (int u = 0; u < CH; ++u) { jc[u] = j1[u]; j1[u] = j2[u]; pc[u] = pn[u]; }
         }
 
-        // ---- reduce over the LPA lanes of the atom (fixed order) ----
-        acc0 = group_sum<LPA>(acc0);
-        if constexpr (FORCE) {
-            acc1 = group_sum<LPA>(acc1);
-            acc2 = group_sum<LPA>(acc2);
-            if constexpr (ENERGY) acc3 = group_sum<LPA>(acc3);
-        }
+        // ---- reduce over the LPA lanes of the pair (fixed order) ----
+        constexpr int NV = FORCE ? (ENERGY ? 4 : 3) : 1;
+#pragma unroll
+        for (int c = 0; c < NV; ++c) { acc0[c] = group_sum<LPA>(acc0[c]); acc1[c] = group_sum<LPA>(acc1[c]); }
         if (live && q == 0) {
-            if constexpr (!FORCE) {
-                const double rho = a.c.am * acc0;
-                a.rho[i] = rho;
-                const double root = rho > 0.0 ? sqrt(rho) : 0.0;           // reading Q9
-                a.xs[i].w = rho > 0.0 ? a.c.Bm / root : 0.0;
-                contrib += root;
-            } else {
-                a.force[3 * size_t(i)] = acc0;
-                a.force[3 * size_t(i) + 1] = acc1;
-                a.force[3 * size_t(i) + 2] = acc2;
-                contrib += acc3;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int i = h ? i1 : i0;
+                const double *acc = h ? acc1 : acc0;
+                if (i >= N) continue;
+                if constexpr (!FORCE) {
+                    const double rho = a.c.am * acc[0];
+                    a.rho[i] = rho;
+                    const double root = rho > 0.0 ? sqrt(rho) : 0.0;       // reading Q9
+                    a.xs[i].w = rho > 0.0 ? a.c.Bm / root : 0.0;
+                    contrib += root;
+                } else {
+                    a.force[3 * size_t(i)] = acc[0];
+                    a.force[3 * size_t(i) + 1] = acc[1];
+                    a.force[3 * size_t(i) + 2] = acc[2];
+                    contrib += acc[3];
+                }
             }
         }
     }

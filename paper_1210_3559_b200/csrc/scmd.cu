@@ -178,7 +178,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         int *perm = w.take<int>(n), *perm_alt = w.take<int>(n), *cell_of = w.take<int>(n), *slot_of = w.take<int>(n);
         int *cell_sorted = w.take<int>(n), *order_tmp = w.take<int>(n), *order = w.take<int>(n), *ncount = w.take<int>(n);
         int *cell_count = w.take<int>(ncell), *cell_start = w.take<int>(ncell);
-        int *nlist = w.take<int>(size_t(kmax) * n);
+        int *nlist = w.take<int>(size_t(kmax) * (n + 1));      // ceil(N / 2) pair rows of 2 kmax entries
         int *scanpart = w.take<int>(size_t(kMaxCoopBlocks) + 1);
         CellGrid *grid = w.take<CellGrid>(1);
         unsigned long long *counters = w.take<unsigned long long>(kNumCounters);
@@ -288,13 +288,14 @@ int choose_lpa(const sc_ctx *c) {
     if (c->opt_tpr) return c->opt_tpr < 8 ? 8 : c->opt_tpr;
     return 32;
 }
-// consecutive atoms per CTA: short runs balance the SMs better than long ones keep L1 warm (measured:
-// N = 65536: 8 and 16 atoms tie, 32 and more lose 5-70 %; N = 2^20: 32 beats 8 by 7 %)
-int choose_atoms_per_cta(const sc_ctx *c, int lpa) {
-    const int step = kNlistWarps * (32 / lpa);
-    int64_t apc = c->opt_apc ? c->opt_apc : (c->N >= 262144 ? 32 : (c->N >= 4096 ? 8 : 4));
-    apc = apc / step * step;
-    return int(apc < step ? step : apc);
+// list sweeps: warps per CTA and consecutive atom pairs per CTA.  The warps of a CTA work on adjacent
+// pairs at the same time, so the records they gather are the same L1 lines.
+int choose_nlist_warps(const sc_ctx *c) { return c->opt_warps ? c->opt_warps : 4; }
+int choose_pairs_per_cta(const sc_ctx *c, int lpa, int warps) {
+    const int step = warps * (32 / lpa);
+    int64_t ppc = c->opt_apc ? (c->opt_apc + 1) / 2 : (c->N >= 262144 ? 32 : 2 * step);   // measured
+    ppc = ppc / step * step;
+    return int(ppc < step ? step : ppc);
 }
 
 sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
@@ -303,19 +304,20 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     const int lpa = choose_lpa(c);
     NlistArgs a{};
     a.xs = c->xs; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.kmax = c->kmax;
-    a.atoms_per_cta = choose_atoms_per_cta(c, lpa);
+    const int warps = choose_nlist_warps(c);
+    a.pairs_per_cta = choose_pairs_per_cta(c, lpa, warps);
     a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
     a.pairs_in_cut = c->counters + kCntPairsInCut;
     a.rc2 = c->p.r_cut * c->p.r_cut;
     a.c = c->consts;
     if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    cudaError_t e = fast ? launch_nlist_96(lpa, a, force, energy, mixed, c->stream)
-                         : launch_nlist_generic(lpa, a, force, energy, mixed, c->stream);
+    cudaError_t e = fast ? launch_nlist_96(lpa, warps * 32, a, force, energy, mixed, c->stream)
+                         : launch_nlist_generic(lpa, warps * 32, a, force, energy, mixed, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "list sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     if (!force || energy) {
-        const int grid = ceil_div(c->N, a.atoms_per_cta);
+        const int grid = ceil_div((c->N + 1) / 2, a.pairs_per_cta);
         reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
                                                          force ? c->consts.En : -c->consts.eps_c);
         SC_CUDA_CHECK(c, cudaGetLastError());
@@ -635,7 +637,8 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
             if (value != 0 && !pow2_le32(value)) return fail(c, SC_ERR_INVALID, "lanes per row must be a power of two <= 32%s");
             c->opt_tpr = int(value); break;
         case SC_OPT_WARPS_PER_CTA:
-            if (value < 0 || value > kMaxConsumerWarps) return fail(c, SC_ERR_INVALID, "warps per CTA must be 0..8%s");
+            if (value < 0 || value > (c->cutoff ? kNlistMaxBlock / 32 : kMaxConsumerWarps))
+                return fail(c, SC_ERR_INVALID, "warps per CTA must be 0..8%s");
             c->opt_warps = int(value); break;
         case SC_OPT_PERSISTENT:
             if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "persistent must be 0, 1 or 2%s");
