@@ -602,7 +602,7 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
         }
         if (per_sm > 4) per_sm = 4;
         c->coop_grid = per_sm * c->sm_count;
-        const int want = ceil_div(n_atoms, 256);            // no more CTAs than there is work for
+        const int want = ceil_div(n_atoms, 16);             // neighbour rows are built one warp per atom pair
         if (c->coop_grid > want) c->coop_grid = want;
         if (c->coop_grid > kMaxCoopBlocks) c->coop_grid = kMaxCoopBlocks;
         if (cudaMemsetAsync(c->counters, 0, sizeof(unsigned long long) * kNumCounters, c->stream) != cudaSuccess ||
