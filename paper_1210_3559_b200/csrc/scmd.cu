@@ -223,16 +223,30 @@ int allpairs_residency(sc_ctx *c, const void *fn, int it, int tpr, int warps) {
     return per_sm;
 }
 
-// Tile shape for one sweep.  Rows per CTA = 32 / tpr * it.  Large N: CTAs run in waves of
-// sm_count * residency, and a partly filled last wave idles the chip (N = 65536 at 64 rows per CTA is
-// 3.46 waves of the force sweep: 13 % lost), so among the shapes with 2 rows per thread take the one
-// whose wave efficiency x / ceil(x) is best, preferring more rows per CTA when it is a tie.  Small N
-// (x < 1): efficiency = x, i.e. the shape with the most CTAs, down to one row per CTA.
+// Tile shape for one sweep.  Rows per CTA = 32 / tpr * it.
+//  * N >= 7104 (measured sweep over it x tpr x warps at N = 8000 ... 262144): 4 consumer warps per
+//    CTA and the largest row block among 64 (4 rows per thread, 2 lanes per row), 32 (4, 4), 16 (2, 4) that
+//    still gives >= 6 CTAs per SM; 4 rows per thread put 16 independent pair chains in flight per thread, which
+//    the FP64 pipe needs more than it needs resident warps (3-8 % over 2 rows per thread and 8 warps);
+//  * smaller N: CTAs run in waves of sm_count * residency, and a partly filled last wave idles the chip, so among
+//    the shapes with 2 rows per thread take the one whose wave efficiency x / ceil(x) is best, preferring more
+//    rows per CTA when it is a tie (x < 1: efficiency = x, i.e. the shape with the most CTAs, down to one row
+//    per CTA), discounted for the lanes that split j inside a warp.
 TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
     const int64_t N = c->N;
     TileChoice best{2, 1, 8};
+    int warps_pref = 0;
     if (c->opt_it && c->opt_tpr) {
         best.it = c->opt_it; best.tpr = c->opt_tpr;
+    } else if (!c->opt_it && !c->opt_tpr && N >= 3 * 16 * int64_t(c->sm_count) &&
+               (c->precision != SC_PREC_MIXED || N >= 6 * 64 * int64_t(c->sm_count))) {
+        static const int shapes[3][2] = {{4, 2}, {4, 4}, {2, 4}};
+        best.it = 2; best.tpr = 4;
+        for (const auto &sh : shapes) {
+            if (!allpairs_fn(c, sh[0], sh[1], force, energy)) continue;
+            if (ceil_div(N, allpairs_rows_per_cta(sh[0], sh[1])) >= 6 * c->sm_count) { best.it = sh[0]; best.tpr = sh[1]; break; }
+        }
+        warps_pref = 4;
     } else {
         double best_eff = -1.0;
         const int its[2] = {2, 1};
@@ -245,14 +259,17 @@ TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
                 if (!fn) continue;
                 const int rpc = allpairs_rows_per_cta(it, tpr);
                 const double x = double(ceil_div(N, rpc)) / (double(c->sm_count) * allpairs_residency(c, fn, it, tpr, 8));
-                const double eff = x / std::ceil(x);
+                // lanes that split j inside a warp cost shared-memory bandwidth and epilogue shuffles (measured)
+                static const double lanes64[6] = {1.0, 1.0, 0.97, 0.90, 0.75, 0.6}, lanes32[6] = {1.0, 0.92, 0.75, 0.5, 0.35, 0.25};
+                const int lg = tpr == 1 ? 0 : tpr == 2 ? 1 : tpr == 4 ? 2 : tpr == 8 ? 3 : tpr == 16 ? 4 : 5;
+                const double eff = x / std::ceil(x) * (c->precision == SC_PREC_MIXED ? lanes32[lg] : lanes64[lg]);
                 if (eff > best_eff + 0.02) { best_eff = eff; best.it = it; best.tpr = tpr; }
             }
         }
         if (c->opt_it) best.it = c->opt_it;
         if (c->opt_tpr) best.tpr = c->opt_tpr;
     }
-    int warps = 8;
+    int warps = warps_pref ? warps_pref : 8;
     while (warps > 1 && N / (int64_t(warps) * best.tpr) < 8) warps /= 2;   // >= ~8 pairs per lane and row
     if (c->opt_warps) warps = c->opt_warps;
     best.warps = warps;
