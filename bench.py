@@ -264,9 +264,9 @@ def run_ours(args):
     sc.sc_energy()                                                     # first evaluation (builds the rows)
     stats0 = sc.sc_stats()
     pairs_per_step = float(stats0["n_pairs_in_cut"])                   # N(N-1) for all pairs
-    # small all-pairs FP64 clusters run the whole sc_step loop in one cooperative launch (csrc/sc_small.cuh):
+    # small all-pairs clusters run the whole sc_step loop in one cooperative launch (csrc/sc_small.cuh):
     # there a bench step is one sc_step call of MD_PER_CALL MD steps and the roofline kernel is the loop itself
-    one_launch = spec.r_cut <= 0 and spec.prec == "fp64" and N <= 6144
+    one_launch = spec.r_cut <= 0 and N <= 6144
     md_per_call = 100 if one_launch else 1
     if not one_launch:
         sc.sc_profile(True)

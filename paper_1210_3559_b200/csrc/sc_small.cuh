@@ -35,6 +35,7 @@ struct SmallStepArgs {
     double4 *xs_b;          // [N] second buffer: step k works in (k odd ? xs_b : xs), so that a CTA already in
                             //     phase A of step k + 1 never overwrites records another CTA still stages
     double *vel, *force, *rho;
+    FPair *xf;              // MIXED: the packed records of the multi-launch sweeps, refreshed at exit (may be NULL)
     double *part_emb, *part_pair, *part_ke;   // [gridDim.x]
     double *sprime;         // [N] s' of the current step, contiguous (phase C re-stages only these 8 bytes per atom)
     unsigned long long *barrier;      // grid barrier counter; grows by gridDim.x per barrier
@@ -167,13 +168,63 @@ __device__ __forceinline__ void small_force_term(const double4 &pi, const double
     acc[3] += pn;
 }
 
+// ---- mixed precision (binary32 pair arithmetic on split coordinates, binary64 accumulation) ----
+// staged record: x = xh + xl with xh = fl32(x), xl = fl32(x - xh), so that (xh_i - xh_j) + (xl_i - xl_j) keeps the
+// accuracy of a binary64 subtraction to within binary32 rounding of the DIFFERENCE (as in allpairs32_kernel)
+struct __align__(32) SmallRecF { float xh, yh, zh, s, xl, yl, zl, pad; };
+static_assert(sizeof(SmallRecF) == sizeof(double4), "same staging footprint in both precisions");
+__device__ __forceinline__ SmallRecF split_record(const double4 &p) {
+    SmallRecF r;
+    r.xh = float(p.x); r.yh = float(p.y); r.zh = float(p.z); r.s = float(p.w);
+    r.xl = float(p.x - double(r.xh)); r.yl = float(p.y - double(r.yh)); r.zl = float(p.z - double(r.zh)); r.pad = 0.f;
+    return r;
+}
+template <int ME>
+__device__ __forceinline__ float small_density_term_f(const SmallRecF &pi, const SmallRecF &p, bool self, int m_exp) {
+    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
+    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    r2 = self ? 1.0f : r2;
+    if constexpr (ME > 0 && ME % 2 == 0) {
+        const float w = self ? 0.f : rcp_fast_f(r2);
+        return ipow_cf<ME / 2>(w);
+    } else {
+        const float y = self ? 0.f : rsqrt_fast_f(r2);
+        return (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+    }
+}
 template <int NE, int ME>
+__device__ __forceinline__ void small_force_term_f(const SmallRecF &pi, const SmallRecF &p, bool self, float Anf, int n_exp,
+                                                   int m_exp, float (&acc)[4]) {
+    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
+    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    r2 = self ? 1.0f : r2;
+    const float y = self ? 0.f : rsqrt_fast_f(r2);
+    const float w = y * y;
+    const float ss = pi.s + p.s;
+    float coef, pn;
+    if constexpr (NE == 9 && ME == 6) {
+        const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+        coef = w4 * fmaf(Anf, y3, -ss);
+        pn = w4 * y;
+    } else {
+        const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+        pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+        coef = w * fmaf(Anf, pn, -ss * pm);
+    }
+    acc[0] = fmaf(coef, dx, acc[0]);
+    acc[1] = fmaf(coef, dy, acc[1]);
+    acc[2] = fmaf(coef, dz, acc[2]);
+    acc[3] += pn;
+}
+
+template <int NE, int ME, bool MIXED>
 __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const SmallStepArgs a) {
     unsigned long long bar_target = a.barrier_base;
     auto grid_sync = [&]() { bar_target += gridDim.x; grid_barrier(a.barrier, bar_target); };
     extern __shared__ __align__(32) unsigned char smem_raw[];
     const int N = a.n_atoms;
     double4 *sm = reinterpret_cast<double4 *>(smem_raw);
+    SmallRecF *smf = reinterpret_cast<SmallRecF *>(smem_raw);          // MIXED: the same bytes hold split binary32 records
     double *warp_red = reinterpret_cast<double *>(sm + N);
     double *rowval = warp_red + (kSmallThreads / 32) * 4;
     __shared__ double s_lambda;
@@ -187,6 +238,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
     const bool owner = rowlive && q == 0;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
+    const float Anf = float(An);
 
     double vx = 0, vy = 0, vz = 0, fx = 0, fy = 0, fz = 0, my_rho = 0;
     if (owner) {
@@ -198,9 +250,17 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
     double ke_final = 0.0, temp_final = 0.0;
 
     double px = 0, py = 0, pz = 0, sp = 0;                 // owner: position and s' of its atom
+    if (owner) {
+        const double4 p = load_record_cg(a.xs + i);
+        px = p.x; py = p.y; pz = p.z; sp = p.w;
+    }
     auto stage = [&](const double4 *cur) {
         __syncthreads();                                    // everyone is done with the previous contents
-        for (int j = t; j < N; j += kSmallThreads) sm[j] = load_record_cg(cur + j);
+        for (int j = t; j < N; j += kSmallThreads) {
+            const double4 p = load_record_cg(cur + j);
+            if constexpr (MIXED) smf[j] = split_record(p);
+            else sm[j] = p;
+        }
         __syncthreads();
     };
 
@@ -210,11 +270,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         if (owner) {
             vx *= lambda; vy *= lambda; vz *= lambda;
             vx = fma(a.hk, fx, vx); vy = fma(a.hk, fy, vy); vz = fma(a.hk, fz, vz);
-            double4 p = sm[i];                              // staged in phase C of the previous step
-            if (k == 1) p = load_record_cg(a.xs + i);
-            p.x = fma(a.dt, vx, p.x); p.y = fma(a.dt, vy, p.y); p.z = fma(a.dt, vz, p.z);
-            px = p.x; py = p.y; pz = p.z;
-            cur[i] = p;
+            px = fma(a.dt, vx, px); py = fma(a.dt, vy, py); pz = fma(a.dt, vz, pz);
+            cur[i] = make_double4(px, py, pz, sp);
         }
         lambda = 1.0;
         grid_sync();
@@ -223,7 +280,20 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         stage(cur);
         {
             double acc[1] = {0.0};
-            if (rowlive) {
+            if (rowlive && MIXED) {
+                const SmallRecF pi = smf[i];
+                int j = q;
+                while (j < N) {                                   // binary32 partial sums over <= 8 terms, then binary64
+                    float t0 = 0.f, t1 = 0.f;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (j < N) t0 += small_density_term_f<ME>(pi, smf[j], j == i, m_exp);
+                        if (j + JL < N) t1 += small_density_term_f<ME>(pi, smf[j + JL], j + JL == i, m_exp);
+                        j += 2 * JL;
+                    }
+                    acc[0] += double(t0 + t1);
+                }
+            } else if (rowlive) {
                 const double4 pi = sm[i];
                 double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;   // 4 independent chains; summed in a fixed order
                 int j = q;
@@ -249,11 +319,28 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         grid_sync();
 
         // ---- C: sweep 2 (positions are still staged; fetch the s' of this step) ----
-        for (int j = t; j < N; j += kSmallThreads) sm[j].w = __ldcg(a.sprime + j);
+        for (int j = t; j < N; j += kSmallThreads) {
+            if constexpr (MIXED) smf[j].s = float(__ldcg(a.sprime + j));
+            else sm[j].w = __ldcg(a.sprime + j);
+        }
         __syncthreads();
         {
             double acc[4] = {0.0, 0.0, 0.0, 0.0};
-            if (rowlive) {
+            if (rowlive && MIXED) {
+                const SmallRecF pi = smf[i];
+                int j = q;
+                while (j < N) {
+                    float fa[4] = {0.f, 0.f, 0.f, 0.f}, fb[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (j < N) small_force_term_f<NE, ME>(pi, smf[j], j == i, Anf, n_exp, m_exp, fa);
+                        if (j + JL < N) small_force_term_f<NE, ME>(pi, smf[j + JL], j + JL == i, Anf, n_exp, m_exp, fb);
+                        j += 2 * JL;
+                    }
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) acc[c] += double(fa[c] + fb[c]);
+                }
+            } else if (rowlive) {
                 const double4 pi = sm[i];
                 double b[4] = {0.0, 0.0, 0.0, 0.0};               // second chain
                 int j = q;
@@ -320,6 +407,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         a.force[3 * size_t(i)] = fx; a.force[3 * size_t(i) + 1] = fy; a.force[3 * size_t(i) + 2] = fz;
         a.rho[i] = my_rho;
         a.xs[i] = make_double4(px, py, pz, sp);             // after the last barrier: nobody stages any more
+        if (a.xf) store_split_record(a.xf, i, px, py, pz, float(sp));
     }
     if (t == 0) { a.part_emb[blockIdx.x] = e_emb; a.part_pair[blockIdx.x] = e_pair; }
     grid_sync();

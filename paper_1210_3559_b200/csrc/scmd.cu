@@ -440,15 +440,18 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
 constexpr int64_t kSmallDefaultMaxAtoms = kSmallMaxAtoms;   // measured: the loop beats the multi-launch path up to its capacity
 
 bool small_path_wanted(const sc_ctx *c) {
-    if (c->cutoff || c->precision != SC_PREC_FP64 || !c->xs_b || c->opt_persistent == 2 || c->profile) return false;
+    if (c->cutoff || !c->xs_b || c->opt_persistent == 2 || c->profile) return false;
     if (c->N > kSmallMaxAtoms) return false;
     return c->opt_persistent == 1 || c->N <= kSmallDefaultMaxAtoms;
 }
 
 sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int thermo, int64_t nsteps) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
-    const void *fn = fast ? reinterpret_cast<const void *>(small_step_kernel<9, 6>)
-                          : reinterpret_cast<const void *>(small_step_kernel<0, 0>);
+    const bool mixed = c->precision == SC_PREC_MIXED;
+    const void *fn = mixed ? (fast ? reinterpret_cast<const void *>(small_step_kernel<9, 6, true>)
+                                   : reinterpret_cast<const void *>(small_step_kernel<0, 0, true>))
+                           : (fast ? reinterpret_cast<const void *>(small_step_kernel<9, 6, false>)
+                                   : reinterpret_cast<const void *>(small_step_kernel<0, 0, false>));
     const int N = int(c->N);
     const size_t smem = small_step_smem_bytes(N);
     if (c->small_ctas == 0) {
@@ -459,7 +462,7 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
         c->small_ctas = c->sm_count;                    // one CTA per SM: the barrier cost grows with the CTA count
     }
     SmallStepArgs a{};
-    a.xs = c->xs; a.xs_b = c->xs_b; a.vel = c->vel; a.force = c->force; a.rho = c->rho;
+    a.xs = c->xs; a.xs_b = c->xs_b; a.xf = c->xf; a.vel = c->vel; a.force = c->force; a.rho = c->rho;
     a.part_emb = c->part_a; a.part_pair = c->part_b; a.part_ke = c->part_ke; a.scal = c->scal;
     a.sprime = c->sprime; a.barrier = c->small_barrier; a.barrier_base = c->small_barrier_count;
     a.n_atoms = N;
