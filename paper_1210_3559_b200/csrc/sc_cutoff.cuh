@@ -297,6 +297,15 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
     const double rl2 = a.r_list * a.r_list;
     const double rl2_cells = rl2 * g.inv_edge * g.inv_edge;           // (list radius / edge)^2
     const int G = g.fine;
+    // reach[ady][adz]: how many cells along x a neighbour can be away in a row of cells whose nearest points
+    // are (ady, adz) cells away in y, z (-1: the row is out of reach)
+    __shared__ int reach[kFineMax + 1][kFineMax + 1];
+    if (tid < (kFineMax + 1) * (kFineMax + 1)) {
+        const int ady = tid / (kFineMax + 1), adz = tid % (kFineMax + 1);
+        const double rem = rl2_cells - double(adz * adz + ady * ady);
+        reach[ady][adz] = rem > 0.0 ? min(G, int(sqrt(rem)) + 1) : -1;
+    }
+    __syncthreads();
     const unsigned lt_mask = (1u << lane) - 1u;
     const int cap = 2 * a.kmax;
     int my_max = 0;                                                    // longest single-atom neighbourhood
@@ -315,11 +324,9 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
         int cnt = 0, cnt0 = 0, cnt1 = 0;
         // x-range of cells of the row (yy, zz) that can hold a neighbour of an atom in cell (cx, cy, cz)
         auto xrange = [&](int cx, int cy, int cz, int yy, int zz, int &lo, int &hi) -> bool {
-            const int adz = max(abs(zz - cz) - 1, 0), ady = max(abs(yy - cy) - 1, 0);
             if (abs(zz - cz) > G || abs(yy - cy) > G) return false;
-            const double rem = rl2_cells - double(adz * adz + ady * ady);
-            if (!(rem > 0.0)) return false;
-            const int mx = min(G, int(sqrt(rem)) + 1);
+            const int mx = reach[max(abs(yy - cy) - 1, 0)][max(abs(zz - cz) - 1, 0)];
+            if (mx < 0) return false;
             lo = max(cx - mx, 0); hi = min(cx + mx, g.nx - 1);
             return true;
         };
@@ -339,8 +346,8 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
                 const int at = cnt + __popc(m & lt_mask);
                 if (ok && at < cap) row[at] = j;
                 cnt += __popc(m);
-                cnt0 += __popc(__ballot_sync(0xffffffffu, in0 && j != k0));
-                cnt1 += __popc(__ballot_sync(0xffffffffu, in1 && j != k1));
+                cnt0 += (in0 && j != k0) ? 1 : 0;                       // per lane; summed over the warp below
+                cnt1 += (in1 && j != k1) ? 1 : 0;
             }
         };
         const bool near = abs(cx0 - cx1) <= 2 * G && abs(cy0 - cy1) <= 2 * G && abs(cz0 - cz1) <= 2 * G;
@@ -369,6 +376,11 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
                         scan(a.cell_start[rowc + lo], a.cell_start[rowc + hi + 1]);
                     }
             }
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            cnt0 += __shfl_xor_sync(0xffffffffu, cnt0, off);
+            cnt1 += __shfl_xor_sync(0xffffffffu, cnt1, off);
         }
         const int kept = min(cnt, cap);
         const int padded = min((kept + 31) & ~31, cap);
