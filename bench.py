@@ -64,8 +64,10 @@ class Spec:
     def generate(self, rank: int = 0) -> W.Workload:
         n = self.n_atoms
         if self.kind == "mackay":
-            assert n == 147
-            return W.config_c1(seed=1001 + rank)
+            if n == 147:
+                return W.config_c1(seed=1001 + rank)
+            shells = {309: 4, 561: 5, 923: 6, 1415: 7, 2057: 8}[n]          # 8 shells: the paper's Ni2057
+            return W.mackay_cluster(shells, 1000.0, 1001 + rank)
         if self.kind == "liquid":
             return W.config_c3(seed=3001 + rank, n_atoms=n)
         if n == 1415:

@@ -225,6 +225,15 @@ def config_c1(seed: int = 1001) -> Workload:
     return Workload("Ni147-mackay", pos, vel, 1000.0, seed)
 
 
+def mackay_cluster(n_shells: int, temperature: float, seed: int) -> Workload:
+    """Mackay icosahedron with n_shells shells (10 s^2 + 2 atoms per shell: 147, 309, 561, 923, 1415, 2057
+    atoms for 3..8 shells), Maxwell-Boltzmann velocities.  8 shells = the paper's Ni2057."""
+    rng = np.random.default_rng(seed)
+    pos = mackay_icosahedron(n_shells, 2.49)
+    vel = maxwell_boltzmann(rng, pos.shape[0], temperature)
+    return Workload(f"Ni{pos.shape[0]}-mackay", pos, vel, temperature, seed)
+
+
 def config_c2(seed: int = 2001) -> Workload:
     """C2: Ni1415 fcc N-nearest sites, jitter +-0.05 A, 2000 K."""
     return fcc_cluster(1415, 2000.0, seed, name="Ni1415-fcc")
