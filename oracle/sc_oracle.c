@@ -55,6 +55,8 @@
  * time reversal, bulk-limit lattice sums, SURVEY.md's independently computed values;
  * Langevin: Philox known-answer vectors, an independent Python restatement of the chain for
  * N = 1, the gamma -> 0 and T = 0 limits, equipartition of free particles).
+ * RDF counts: fcc coordination shells 12, 6, 24, 12, 24, 8, 48, the 13-atom icosahedron, the total
+ * n_ref (N - 1), numpy brute force.
  * Nothing here is "parity unpinned" except absolute energies against a published
  * number -- the paper prints none.
  */
@@ -302,6 +304,48 @@ int64_t oracle_count_pairs(int64_t N, const double *pos, double r_cut) {
         for (int64_t j = 0; j < N; ++j)
             if (j != i && pair_in_range(pos + 3 * i, pos + 3 * j, r_cut)) ++total;
     return total;
+}
+
+/*
+ * Radial distribution histogram of the central atoms (Eq. (11) and the procedure below
+ * it): "the atoms located within 3 A of the cluster center of mass were selected.  For these atoms the RDF
+ * was calculated with a distance bin of 0.4 A".  This routine produces the part of g(r) = rho(r) / rho_bar
+ * that is a count: counts[b] = number of ordered pairs (i, j), j != i, i a reference atom, with
+ * b = floor(r_ij / bin_width), b < n_bins.  Reference atoms: |r_i - centre|^2 < r_select^2, strict.
+ *   centre == NULL: the centre of mass (equal masses: the mean position, long double accumulation).
+ * Where floating point decides an integer, the precision is fixed (as for the cutoff, reading Q7):
+ *   d = x_i - x_j in binary64; r2 = fma(dz, dz, fma(dy, dy, dx*dx)); r = sqrt(r2) (correctly rounded);
+ *   b = (int64) floor(r * (1.0 / bin_width)); the selection uses the same r2 form against r_select*r_select.
+ * The normalisation to g(r) (division by n_ref * 4 pi r^2 dr * rho_bar; the paper does not say which volume
+ * defines rho_bar for a finite cluster -- reading Q19) is arithmetic on these counts and is left to the caller.
+ * Returns the number of reference atoms; centre_out (may be NULL) receives the centre used.
+ */
+int64_t oracle_rdf_counts(int64_t N, const double *pos, const double *centre, double r_select, double bin_width,
+                          int64_t n_bins, int64_t *counts, double *centre_out) {
+    double c[3];
+    if (centre) { c[0] = centre[0]; c[1] = centre[1]; c[2] = centre[2]; }
+    else {
+        long double s[3] = {0, 0, 0};
+        for (int64_t i = 0; i < N; ++i) for (int d = 0; d < 3; ++d) s[d] += pos[3 * i + d];
+        for (int d = 0; d < 3; ++d) c[d] = (double)(s[d] / (long double)N);
+    }
+    if (centre_out) { centre_out[0] = c[0]; centre_out[1] = c[1]; centre_out[2] = c[2]; }
+    for (int64_t b = 0; b < n_bins; ++b) counts[b] = 0;
+    const double inv_bin = 1.0 / bin_width, rs2 = r_select * r_select;
+    int64_t n_ref = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        const double ex = pos[3 * i] - c[0], ey = pos[3 * i + 1] - c[1], ez = pos[3 * i + 2] - c[2];
+        if (!(fma(ez, ez, fma(ey, ey, ex * ex)) < rs2)) continue;
+        ++n_ref;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            const double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+            const double r = sqrt(fma(dz, dz, fma(dy, dy, dx * dx)));
+            const double fb = floor(r * inv_bin);
+            if (fb < (double)n_bins) counts[(int64_t)fb] += 1;
+        }
+    }
+    return n_ref;
 }
 
 void oracle_philox4x32_10(const uint32_t *ctr, const uint32_t *key, uint32_t *out) { philox4x32_10(ctr, key, out); }

@@ -70,6 +70,8 @@ class Oracle:
         L.oracle_run.argtypes = [ctypes.c_int64, _DP, _DP, PP, ctypes.c_double, ctypes.c_int64,
                                  ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                  ctypes.c_uint64, ctypes.c_uint64, _DP, _DP, _DP]
+        L.oracle_rdf_counts.argtypes = [ctypes.c_int64, _DP, _DP, ctypes.c_double, ctypes.c_double, ctypes.c_int64, _IP, _DP]
+        L.oracle_rdf_counts.restype = ctypes.c_int64
         U32P = ctypes.POINTER(ctypes.c_uint32)
         L.oracle_philox4x32_10.argtypes = [U32P, U32P, U32P]
         L.oracle_philox4x32_10.restype = None
@@ -137,6 +139,16 @@ class Oracle:
     def count_pairs(self, pos, r_cut: float) -> int:
         p = self._pos(pos)
         return int(self.lib.oracle_count_pairs(p.shape[0], _dptr(p), float(r_cut)))
+
+    def rdf_counts(self, pos, r_select: float, bin_width: float, n_bins: int, centre=None):
+        """-> (counts[n_bins] int64, n_ref, centre used)."""
+        p = self._pos(pos)
+        counts = np.zeros(int(n_bins), dtype=np.int64)
+        cen = None if centre is None else np.ascontiguousarray(centre, dtype=np.float64)
+        out = np.zeros(3)
+        n_ref = self.lib.oracle_rdf_counts(p.shape[0], _dptr(p), _dptr(cen), float(r_select), float(bin_width),
+                                           int(n_bins), counts.ctypes.data_as(_IP), _dptr(out))
+        return counts, int(n_ref), out
 
     def philox4x32_10(self, ctr, key) -> np.ndarray:
         c = np.ascontiguousarray(ctr, dtype=np.uint32); k = np.ascontiguousarray(key, dtype=np.uint32)
