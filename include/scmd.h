@@ -155,6 +155,23 @@ sc_status sc_step(sc_ctx *ctx, double dt_fs, const sc_thermostat *thermostat, in
 sc_status sc_stats(sc_ctx *ctx, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int64_t *max_neighbours);
 
 /*
+ * Radial-distribution counts of the central atoms (Eq. (11) g(r) = rho(r) / rho_bar: "the
+ * atoms located within 3 A of the cluster center of mass were selected.  For these atoms the RDF was
+ * calculated with a distance bin of 0.4 A").  Reference atoms i: |r_i - centre|^2 < r_select^2 (strict);
+ * h_counts[b] (host, n_bins entries, 1 <= n_bins <= 4096) = number of ordered pairs (i, j), j != i, with
+ * floor(r_ij / bin_width) = b; pairs beyond the last bin are dropped.  The counts are bit-exact (binary64
+ * differences, r^2 by fused multiply-add, correctly rounded square root, one multiplication by 1 / bin_width).
+ *   h_centre       host, 3 doubles, or NULL = the centre of mass (mean position) computed on the device
+ *   h_n_ref        receives the number of reference atoms (may be NULL)
+ *   h_centre_used  receives the centre used (host, 3 doubles; may be NULL)
+ * The division by n_ref * 4 pi r^2 dr * rho_bar that turns counts into g(r) is left to the caller (the paper
+ * does not say which volume defines rho_bar of a finite cluster).  Works on the current positions in any
+ * precision mode and with or without a cutoff; synchronises the stream.
+ */
+sc_status sc_rdf(sc_ctx *ctx, const double *h_centre, double r_select, double bin_width, int32_t n_bins,
+                 int64_t *h_counts, int64_t *h_n_ref, double *h_centre_used);
+
+/*
  * Host-buffer entry points (the end-to-end path): copies are part of the call.
  * sc_eval_host: upload h_pos[N*3], run both sweeps, download h_force[N*3], h_rho[N] (either
  *   may be NULL) and the potential energy *h_epot (may be NULL).

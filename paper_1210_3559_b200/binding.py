@@ -81,6 +81,7 @@ def load_library() -> ctypes.CDLL:
         "sc_stats": (i32, [vp, IP, IP, IP]),
         "sc_eval_host": (i32, [vp, vp, vp, vp, DP]),
         "sc_step_host": (i32, [vp, vp, vp, dbl, TP, i64, DP]),
+        "sc_rdf": (i32, [vp, DP, dbl, dbl, i32, IP, IP, DP]),
         "sc_launch_count": (i32, [vp, IP]),
         "sc_profile": (i32, [vp, i32]),
         "sc_profile_read": (i32, [vp, DP, DP]),
@@ -235,6 +236,20 @@ class SuttonChen:
         self._check(self.lib.sc_step_host(self._ctx, _host_ptr(h_pos, n3, "h_pos"), _host_ptr(h_vel, n3, "h_vel"),
                                           float(dt_fs), th, int(nsteps), s), "sc_step_host")
         return dict(epot=s[0], ekin=s[1], temperature=s[2])
+
+    def sc_rdf(self, r_select: float, bin_width: float, n_bins: int, centre=None):
+        """-> (counts[n_bins] numpy int64, n_ref, centre used); see sc_rdf in include/scmd.h."""
+        import numpy as np
+        counts = np.zeros(int(n_bins), dtype=np.int64)
+        n_ref = ctypes.c_int64()
+        used = (ctypes.c_double * 3)()
+        cen = None
+        if centre is not None:
+            cen = (ctypes.c_double * 3)(*[float(v) for v in centre])
+        self._check(self.lib.sc_rdf(self._ctx, cen, float(r_select), float(bin_width), int(n_bins),
+                                    counts.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), ctypes.byref(n_ref), used),
+                    "sc_rdf")
+        return counts, n_ref.value, np.array(list(used))
 
     def sc_launch_count(self) -> int:
         v = ctypes.c_int64()

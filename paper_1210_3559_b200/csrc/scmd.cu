@@ -15,6 +15,7 @@
 #include "sc_integrate.cuh"
 #include "sc_probe.cuh"
 #include "sc_small.cuh"
+#include "sc_analysis.cuh"
 
 using namespace scmd;
 
@@ -52,6 +53,9 @@ struct sc_ctx {
 
     // device arrays (all inside the caller's workspace)
     double4 *xs = nullptr;        // [N] (x, y, z, s')
+    unsigned long long *rdf_counts = nullptr;   // [kRdfMaxBins + 1] histogram; the last word is the reference-atom count
+    int *rdf_refs = nullptr;      // [N] reference atoms of sc_rdf
+    double *rdf_meta = nullptr;   // [4] centre
     double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
     unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
     unsigned long long small_barrier_count = 0;
@@ -154,9 +158,13 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
     double *scal = w.take<double>(kNumScalars);
     double *sa = w.take<double>(3 * n);
     double *sb = w.take<double>(3 * n);
+    unsigned long long *rc = w.take<unsigned long long>(kRdfMaxBins + 2);
+    int *rr = w.take<int>(n);
+    double *rm = w.take<double>(4);
     if (c && base) {
         c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
+        c->rdf_counts = rc; c->rdf_refs = rr; c->rdf_meta = rm;
     }
     if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms) {
         double4 *xb = w.take<double4>(n);
@@ -820,6 +828,43 @@ sc_status sc_stats(sc_ctx *c, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int6
     if (max_neighbours) *max_neighbours = int64_t(cnt[kCntMaxRow]);
     if (cnt[kCntOverflow])
         return fail(c, SC_ERR_CAPACITY, "a neighbour row overflowed its capacity; results since then are invalid%s");
+    return SC_OK;
+}
+
+sc_status sc_rdf(sc_ctx *c, const double *h_centre, double r_select, double bin_width, int32_t n_bins,
+                 int64_t *h_counts, int64_t *h_n_ref, double *h_centre_used) {
+    if (!c) return SC_ERR_INVALID;
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_rdf: no positions set%s");
+    if (!h_counts || n_bins < 1 || n_bins > kRdfMaxBins || !(r_select > 0.0) || !(bin_width > 0.0) ||
+        !std::isfinite(r_select) || !std::isfinite(bin_width))
+        return fail(c, SC_ERR_INVALID, "sc_rdf: need h_counts, 1 <= n_bins <= 4096, r_select > 0, bin_width > 0%s");
+    const int N = int(c->N);
+    SC_CUDA_CHECK(c, cudaMemsetAsync(c->rdf_counts, 0, sizeof(unsigned long long) * (kRdfMaxBins + 2), c->stream));
+    if (h_centre) {
+        if (!std::isfinite(h_centre[0]) || !std::isfinite(h_centre[1]) || !std::isfinite(h_centre[2]))
+            return fail(c, SC_ERR_INVALID, "sc_rdf: centre must be finite%s");
+        SC_CUDA_CHECK(c, cudaMemcpyAsync(c->rdf_meta, h_centre, 3 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));             // h_centre is pageable caller memory
+    } else {
+        rdf_centre_kernel<<<1, 1024, 0, c->stream>>>(c->xs, N, c->rdf_meta);
+        c->launches += 1;
+    }
+    unsigned int *n_ref = reinterpret_cast<unsigned int *>(c->rdf_counts + kRdfMaxBins);
+    rdf_select_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(c->xs, N, c->rdf_meta, r_select * r_select, c->rdf_refs, n_ref);
+    rdf_count_kernel<<<ceil_div(N, kRdfBlock), kRdfBlock, 0, c->stream>>>(c->xs, N, c->rdf_refs, n_ref, 1.0 / bin_width,
+                                                                           int(n_bins), c->rdf_counts);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 2;
+    std::vector<unsigned long long> host(size_t(n_bins) + 0);
+    unsigned long long nref_word = 0;
+    double centre[3];
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(host.data(), c->rdf_counts, sizeof(unsigned long long) * size_t(n_bins), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(&nref_word, c->rdf_counts + kRdfMaxBins, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(centre, c->rdf_meta, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    for (int b = 0; b < n_bins; ++b) h_counts[b] = int64_t(host[size_t(b)]);
+    if (h_n_ref) *h_n_ref = int64_t(nref_word & 0xffffffffull);
+    if (h_centre_used) { h_centre_used[0] = centre[0]; h_centre_used[1] = centre[1]; h_centre_used[2] = centre[2]; }
     return SC_OK;
 }
 
