@@ -17,8 +17,9 @@
 //      from the per-CTA partials in a fixed order and scales its own velocities.
 //
 // Decomposition: a CTA owns `rows` consecutive atoms; JL (a power of two) threads share one row and
-// stride the j range; their partial sums meet in a shuffle tree (and across warps through shared
-// memory when JL > 32), always in the same order: results are bit-reproducible.  The row's first
+// stride the j range; a warp holds 32 / lq rows (lq threads of each), so its shared-memory loads are
+// broadcast across rows; partial sums meet in a shuffle tree (and across the warps of a row through
+// shared memory), always in the same order: results are bit-reproducible.  The row's first
 // thread ("owner") keeps v and F of its atom in registers for the whole call.
 #pragma once
 #include "sc_allpairs.cuh"
@@ -41,7 +42,10 @@ struct SmallStepArgs {
     unsigned long long *barrier;      // grid barrier counter; grows by gridDim.x per barrier
     unsigned long long barrier_base;  // its value when this launch starts (the host keeps count)
     double *scal;
-    int n_atoms, rows, jl;  // rows per CTA; threads per row (power of two, rows * jl <= kSmallThreads)
+    int n_atoms, rows, jl;  // rows per CTA; threads per row (power of two)
+    int lq;                 // threads of a row inside one warp (power of two, <= min(jl, 32)): a warp holds 32 / lq rows, so a
+                            //   shared-memory load of 32 lanes touches lq records (broadcast across the rows);
+                            //   round_up(rows, 32 / lq) * jl <= kSmallThreads
     long long nsteps;
     double hk, dt, mass, ndof;
     int thermo;             // sc_thermo_kind
@@ -53,7 +57,7 @@ struct SmallStepArgs {
 };
 
 inline size_t small_step_smem_bytes(int n_atoms) {
-    return size_t(n_atoms) * sizeof(double4) + (kSmallThreads / 32) * 4 * sizeof(double) + kSmallThreads * sizeof(double);
+    return size_t(n_atoms) * sizeof(double4) + (kSmallThreads / 32) * 8 * 4 * sizeof(double) + kSmallThreads * sizeof(double);
 }
 
 #ifdef SCMD_MAIN_TU
@@ -63,27 +67,28 @@ __device__ __forceinline__ double4 load_record_cg(const double4 *p) {    // L2 (
     return r;
 }
 
-// sum over the JL threads of a row; valid in the row's first thread.  JL <= 32: shuffle tree inside the
-// warp; JL > 32: shuffle tree per warp, then the row's first thread adds the per-warp values in order.
+// sum over the JL threads of a row; valid in the row's first thread.  The lq threads of a row inside a warp meet in
+// a shuffle tree; when the row spans jl / lq warps, its first thread adds the per-warp values in order.
+constexpr int kSmallMaxRowsPerWarp = 8;
 template <int NV>
-__device__ __forceinline__ void row_reduce(double (&v)[NV], int jl, int q, double *warp_red) {
+__device__ __forceinline__ void row_reduce(double (&v)[NV], int jl, int lq, int q, double *warp_red) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int width = jl < 32 ? jl : 32;
-    for (int off = width >> 1; off > 0; off >>= 1)
+    for (int off = lq >> 1; off > 0; off >>= 1)
 #pragma unroll
         for (int c = 0; c < NV; ++c) v[c] += __shfl_xor_sync(0xffffffffu, v[c], off);
-    if (jl > 32) {                                          // block-uniform
+    if (jl > lq) {                                          // block-uniform
+        const int rl = lane / lq;                           // row of this lane inside the warp
         __syncthreads();
-        if (lane == 0)
+        if (lane % lq == 0)
 #pragma unroll
-            for (int c = 0; c < NV; ++c) warp_red[warp * 4 + c] = v[c];
+            for (int c = 0; c < NV; ++c) warp_red[(warp * kSmallMaxRowsPerWarp + rl) * 4 + c] = v[c];
         __syncthreads();
-        if (q == 0) {
-            const int nw = jl >> 5;
+        if (q == 0) {                                       // first warp of the row's group, first lane of the row
+            const int nw = jl / lq;
 #pragma unroll
             for (int c = 0; c < NV; ++c) {
                 double s = 0.0;
-                for (int w = 0; w < nw; ++w) s += warp_red[(warp + w) * 4 + c];
+                for (int w = 0; w < nw; ++w) s += warp_red[((warp + w) * kSmallMaxRowsPerWarp + rl) * 4 + c];
                 v[c] = s;
             }
         }
@@ -226,11 +231,15 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
     double4 *sm = reinterpret_cast<double4 *>(smem_raw);
     SmallRecF *smf = reinterpret_cast<SmallRecF *>(smem_raw);          // MIXED: the same bytes hold split binary32 records
     double *warp_red = reinterpret_cast<double *>(sm + N);
-    double *rowval = warp_red + (kSmallThreads / 32) * 4;
+    double *rowval = warp_red + (kSmallThreads / 32) * kSmallMaxRowsPerWarp * 4;
     __shared__ double s_lambda;
 
-    const int t = threadIdx.x, JL = a.jl;
-    const int r = t / JL, q = t % JL;
+    // thread -> (row r of this CTA, q of the row's JL threads): a warp holds RPW = 32 / lq rows (lq consecutive q each);
+    // a group of JL / lq consecutive warps covers the JL threads of its RPW rows
+    const int t = threadIdx.x, JL = a.jl, LQ = a.lq;
+    const int rpw = 32 / LQ, wpg = JL / LQ;
+    const int r = ((t >> 5) / wpg) * rpw + (t & 31) / LQ;
+    const int q = ((t >> 5) % wpg) * LQ + (t & 31) % LQ;
     const int row0 = blockIdx.x * a.rows;
     const int nrows = min(a.rows, N - row0);
     const int i = row0 + r;
@@ -306,7 +315,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
                 for (; j < N; j += JL) t0 += small_density_term<ME>(pi, sm[j], j == i, m_exp);
                 acc[0] = (t0 + t1) + (t2 + t3);
             }
-            row_reduce<1>(acc, JL, q, warp_red);
+            row_reduce<1>(acc, JL, LQ, q, warp_red);
             double root = 0.0;
             if (owner) {
                 my_rho = a.c.am * acc[0];
@@ -352,7 +361,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
 #pragma unroll
                 for (int c = 0; c < 4; ++c) acc[c] += b[c];
             }
-            row_reduce<4>(acc, JL, q, warp_red);
+            row_reduce<4>(acc, JL, LQ, q, warp_red);
             // ---- D: second half kick (+ Langevin), |v|^2 ----
             double v2 = 0.0;
             if (owner) {

@@ -476,9 +476,22 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
     a.n_atoms = N;
     a.rows = ceil_div(N, c->small_ctas);
     const int grid = ceil_div(N, a.rows);
-    int jl = 1;
-    while (jl * 2 * a.rows <= kSmallThreads && jl < 512) jl *= 2;
+    // rows per warp (1, 2 or 4): more rows per warp = fewer shared-memory wavefronts per pair (the 32 lanes of a
+    // load touch 32 / rpw records), at the price of padding the row count to a multiple of rpw
+    int rpw = c->opt_tpr ? 32 / c->opt_tpr : (a.rows >= 12 ? 8 : (a.rows >= 2 ? 2 : 1));   // measured: 8 rows per warp +4 % at N >= 2057
+    if (rpw > kSmallMaxRowsPerWarp) rpw = kSmallMaxRowsPerWarp;
+    if (rpw < 1) rpw = 1;
+    int jl = 1, rows_p = 0;
+    for (;; rpw /= 2) {
+        rows_p = (a.rows + rpw - 1) / rpw * rpw;
+        jl = 1;
+        while (jl * 2 * rows_p <= kSmallThreads && jl < 512) jl *= 2;
+        if (rows_p * jl <= kSmallThreads && jl * rpw >= 32) break;   // a warp must be filled by rpw rows x (32 / rpw) lanes
+        if (rpw == 1) break;
+    }
     a.jl = jl;
+    a.lq = jl < 32 / rpw ? jl : 32 / rpw;
+    if (32 / a.lq > kSmallMaxRowsPerWarp) return fail(c, SC_ERR_INVALID, "one-launch step loop: more than 8 rows per warp%s");
     a.nsteps = nsteps; a.hk = 0.5 * dt * kAcc / c->p.mass; a.dt = dt; a.mass = c->p.mass; a.ndof = double(3 * c->N - 3);
     a.thermo = thermo;
     if (th) { a.T_start = th->T_start; a.T_end = th->T_end; }
