@@ -36,8 +36,11 @@
 //
 // nlist_kernel: LPA lanes (32 by default) walk one row, gather the 32-byte record of j, apply the
 // strict binary64 test r^2 < r_c^2 (reading Q7: same decision value as the oracle) and accumulate
-// the same pair terms as the all-pairs sweeps.  MIXED: pair arithmetic in binary32 on the converted
-// binary64 difference, accumulated in binary32 over a short chunk and flushed into binary64.
+// the same pair terms as the all-pairs sweeps.  MIXED: the rows gather split binary32 records (x = xh + xl)
+// and the whole pair term runs in binary32 -- no conversion, no binary64 instruction -- except that an entry
+// whose binary32 r^2 lies within 2e-6 r_c^2 of the cutoff takes its set-membership decision from the binary64
+// records (reading Q7: membership is the oracle's, bit for bit); partial sums are flushed into binary64 after
+// every batch.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -60,6 +63,7 @@ enum CounterSlot {
 constexpr int kFineMax = 4;      // G_max: fine cells per list radius (the grid falls back to coarser cells
                                  // when the fine grid would exceed the cell budget)
 constexpr double kFarAway = 1.0e150;   // coordinates of the dummy record that pads every neighbour row
+constexpr float kFarAwayF = 1.0e18f;   // ... of its binary32 twin (its r^2 = 3e36 stays finite)
 
 struct CellGrid {          // written by CTA 0 in P1, read by everyone afterwards
     double ox, oy, oz;     // origin
@@ -71,6 +75,7 @@ struct CellGrid {          // written by CTA 0 in P1, read by everyone afterward
 
 struct RebuildArgs {
     double4 *xs, *xs_alt, *xs_ref;
+    RecF *xfr;                      // mixed list sweeps: split binary32 records in internal order (else NULL)
     double *vel, *vel_alt;          // vel may be unset (have_vel == 0): then not permuted
     int *perm, *perm_alt;
     int *cell_of, *slot_of, *cell_sorted;
@@ -280,6 +285,7 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
         const double4 p = a.xs_alt[k];
         a.xs[k] = p;
         a.xs_ref[k] = p;
+        if (a.xfr) a.xfr[k] = split_record(p);
         a.perm[k] = a.perm_alt[k];
         if (a.have_vel) {
             a.vel[3 * size_t(k)] = a.vel_alt[3 * size_t(k)];
@@ -287,7 +293,10 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
             a.vel[3 * size_t(k) + 2] = a.vel_alt[3 * size_t(k) + 2];
         }
     }
-    if (gtid == 0) a.xs[N] = make_double4(kFarAway, kFarAway, kFarAway, 0.0);   // the dummy record
+    if (gtid == 0) {                                                             // the dummy records
+        a.xs[N] = make_double4(kFarAway, kFarAway, kFarAway, 0.0);
+        if (a.xfr) a.xfr[N] = RecF{kFarAwayF, kFarAwayF, kFarAwayF, 0.f, 0.f, 0.f, 0.f, 0.f};
+    }
     grid.sync();
 
     // ---- P8: neighbour rows, one warp per PAIR of consecutive atoms (k0 = 2g, k1 = 2g + 1) ----
@@ -410,6 +419,7 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
 // --------------------------------------------------------------------------------------------
 struct NlistArgs {
     double4 *xs;              // [N + 1] (x, y, z, s'), internal order; xs[N] = the dummy record at infinity
+    RecF *xfr;                // MIXED: [N + 1] split binary32 records (same order, same dummy); sweep 1 stores fl32(s') here
     const int *nlist;         // [ceil(N/2)][2 * kmax] pair rows, padded with N to a multiple of 32
     const int *ncount;        // [ceil(N/2)]
     int n_atoms, kmax;
@@ -439,14 +449,14 @@ __device__ __forceinline__ double4 load_record(const double4 *p) {
 // branches the compiler interleaves the 8 independent chains of a batch: 4 entries x 2 atoms.)
 // MIXED: pair arithmetic in binary32 on the converted binary64 difference, partial sums in f[]
 // (flushed into acc[] by the caller after every batch).
-template <int NE, int ME, bool FORCE, bool ENERGY, bool MIXED>
+template <int NE, int ME, bool FORCE, bool ENERGY>
 __device__ __forceinline__ void nlist_term(const double4 &pi, const double4 &p, bool other, double rc2, double An,
-                                           int n_exp, int m_exp, double (&acc)[4], float (&f)[4], int &npairs) {
+                                           int n_exp, int m_exp, double (&acc)[4], int &npairs) {
     const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     const bool in = (r2 < rc2) && other;
     if constexpr (!FORCE) npairs += in ? 1 : 0;
-    if constexpr (!MIXED) {
+    {
         const double r2m = in ? r2 : 1.0;
         if constexpr (!FORCE) {
             if constexpr (ME > 0 && ME % 2 == 0) {
@@ -479,42 +489,63 @@ __device__ __forceinline__ void nlist_term(const double4 &pi, const double4 &p, 
             acc[1] = fma(coef, dy, acc[1]);
             acc[2] = fma(coef, dz, acc[2]);
         }
-    } else {
-        // masked differences: a far-away record must not turn 0 * inf into NaN in binary32
-        const float fx = in ? float(dx) : 0.f, fy = in ? float(dy) : 0.f, fz = in ? float(dz) : 0.f;
-        const float q2 = in ? fmaf(fz, fz, fmaf(fy, fy, fx * fx)) : 1.0f;
-        if constexpr (!FORCE) {
-            if constexpr (ME > 0 && ME % 2 == 0) {
-                float w = rcp_fast_f(q2);
-                w = in ? w : 0.f;
-                if constexpr (ME == 6) f[0] = fmaf(w * w, w, f[0]);
-                else f[0] += ipow_cf<ME / 2>(w);
-            } else {
-                float y = rsqrt_fast_f(q2);
-                y = in ? y : 0.f;
-                f[0] += (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
-            }
+    }
+}
+
+// MIXED: the same term in binary32 on split records (no binary64 instruction, no conversion on the common path).
+// Set membership must equal the oracle's binary64 decision (reading Q7): the binary32 r^2 decides unless it lies
+// within 2e-6 r_c^2 of the cutoff (its own error is < 4e-7 relative), in which case the binary64 records are
+// fetched and the decision is taken exactly as in the FP64 path.  The hot loop only raises a flag for such an
+// entry (~3 in a million); a lane whose flag is up recomputes its share of the row with exact decisions.
+struct PairGeomF { float fx, fy, fz, q2; };
+__device__ __forceinline__ PairGeomF nlist_geom_f(const RecF &pi, const RecF &p) {
+    PairGeomF g;
+    g.fx = (pi.xh - p.xh) + (pi.xl - p.xl); g.fy = (pi.yh - p.yh) + (pi.yl - p.yl); g.fz = (pi.zh - p.zh) + (pi.zl - p.zl);
+    g.q2 = fmaf(g.fz, g.fz, fmaf(g.fy, g.fy, g.fx * g.fx));
+    return g;
+}
+__device__ __forceinline__ bool nlist_exact_in_range(const double4 *xs, int i, int j, double rc2) {
+    const double4 a = xs[i], b = xs[j];
+    const double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+    return fma(dz, dz, fma(dy, dy, dx * dx)) < rc2;
+}
+template <int NE, int ME, bool FORCE, bool ENERGY>
+__device__ __forceinline__ void nlist_term_f(const RecF &pi, const RecF &p, PairGeomF g, bool in, float Anf, int n_exp,
+                                             int m_exp, float (&f)[4], int &npairs) {
+    if constexpr (!FORCE) npairs += in ? 1 : 0;
+    const float q2 = in ? g.q2 : 1.0f;
+    if constexpr (!FORCE) {
+        if constexpr (ME > 0 && ME % 2 == 0) {
+            float w = rcp_fast_f(q2);
+            w = in ? w : 0.f;
+            if constexpr (ME == 6) f[0] = fmaf(w * w, w, f[0]);
+            else f[0] += ipow_cf<ME / 2>(w);
         } else {
-            const float Anf = float(An);
             float y = rsqrt_fast_f(q2);
             y = in ? y : 0.f;
-            const float w = y * y;
-            const float ss = float(pi.w) + float(p.w);
-            float coef;
-            if constexpr (NE == 9 && ME == 6) {
-                const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
-                coef = w4 * fmaf(Anf, y3, -ss);
-                if constexpr (ENERGY) f[3] = fmaf(w4, y, f[3]);
-            } else {
-                const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
-                const float pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
-                coef = w * fmaf(Anf, pn, -ss * pm);
-                if constexpr (ENERGY) f[3] += pn;
-            }
-            f[0] = fmaf(coef, fx, f[0]);
-            f[1] = fmaf(coef, fy, f[1]);
-            f[2] = fmaf(coef, fz, f[2]);
+            f[0] += (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
         }
+    } else {
+        // a far-away record must not turn 0 * inf into NaN
+        const float fx = in ? g.fx : 0.f, fy = in ? g.fy : 0.f, fz = in ? g.fz : 0.f;
+        float y = rsqrt_fast_f(q2);
+        y = in ? y : 0.f;
+        const float w = y * y;
+        const float ss = pi.s + p.s;
+        float coef;
+        if constexpr (NE == 9 && ME == 6) {
+            const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+            coef = w4 * fmaf(Anf, y3, -ss);
+            if constexpr (ENERGY) f[3] = fmaf(w4, y, f[3]);
+        } else {
+            const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+            const float pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+            coef = w * fmaf(Anf, pn, -ss * pm);
+            if constexpr (ENERGY) f[3] += pn;
+        }
+        f[0] = fmaf(coef, fx, f[0]);
+        f[1] = fmaf(coef, fy, f[1]);
+        f[2] = fmaf(coef, fz, f[2]);
     }
 }
 
@@ -530,6 +561,7 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
     const int N = a.n_atoms, NP = (N + 1) >> 1;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An, rc2 = a.rc2;
+    const float Anf = float(An), rc2f = float(rc2), band = 2.0e-6f * rc2f;
     const size_t stride = 2 * size_t(a.kmax);
     double contrib = 0.0;
     int npairs = 0;
@@ -541,16 +573,30 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
         const int gp = g0 + g;
         const bool live = gp < end;
         const int i0 = live ? 2 * gp : N, i1 = (live && 2 * gp + 1 < N) ? 2 * gp + 1 : N;   // N = the dummy record
-        const double4 pa = a.xs[i0], pb = a.xs[i1];
+        // records: binary64 (x, y, z, s') or, MIXED, their split binary32 twins -- both 32 bytes, fetched alike
+        const double4 *recs = MIXED ? reinterpret_cast<const double4 *>(a.xfr) : a.xs;
+        const double4 pa = recs[i0], pb = recs[i1];
         const int cnt = live ? a.ncount[gp] : 0;
         const int niter = (cnt + LPA - 1) / LPA;         // rows are padded to a multiple of 32 >= LPA
         const int *row = a.nlist + size_t(live ? gp : 0) * stride + q;
         double acc0[4] = {0.0, 0.0, 0.0, 0.0}, acc1[4] = {0.0, 0.0, 0.0, 0.0};
         float f0[4] = {0.f, 0.f, 0.f, 0.f}, f1[4] = {0.f, 0.f, 0.f, 0.f};
+        int np_row = 0;
+        bool unsure = false;
 
         auto entry = [&](int j, const double4 &p) {
-            nlist_term<NE, ME, FORCE, ENERGY, MIXED>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, f0, npairs);
-            nlist_term<NE, ME, FORCE, ENERGY, MIXED>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, f1, npairs);
+            if constexpr (MIXED) {
+                // binary32 decision; entries too close to the cutoff to trust it only raise `unsure`
+                const RecF &fa = reinterpret_cast<const RecF &>(pa), &fb = reinterpret_cast<const RecF &>(pb);
+                const RecF &fp = reinterpret_cast<const RecF &>(p);
+                const PairGeomF ga = nlist_geom_f(fa, fp), gb = nlist_geom_f(fb, fp);
+                unsure = unsure || fabsf(ga.q2 - rc2f) <= band || fabsf(gb.q2 - rc2f) <= band;
+                nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, ga, ga.q2 < rc2f && j != i0, Anf, n_exp, m_exp, f0, np_row);
+                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, np_row);
+            } else {
+                nlist_term<NE, ME, FORCE, ENERGY>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, np_row);
+                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, np_row);
+            }
         };
         auto flush = [&]() {
             if constexpr (MIXED) {
@@ -578,17 +624,41 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
         load_idx(0, jc);
         load_idx(1, j1);
 #pragma unroll
-        for (int u = 0; u < CH; ++u) pc[u] = load_record(a.xs + jc[u]);
+        for (int u = 0; u < CH; ++u) pc[u] = load_record(recs + jc[u]);
         for (int b = 0; b < nbatch; ++b) {
             load_idx(b + 2, j2);
 #pragma unroll
-            for (int u = 0; u < CH; ++u) pn[u] = load_record(a.xs + j1[u]);
+            for (int u = 0; u < CH; ++u) pn[u] = load_record(recs + j1[u]);
 #pragma unroll
             for (int u = 0; u < CH; ++u) entry(jc[u], pc[u]);
             flush();
 #pragma unroll
             for (int u = 0; u < CH; ++u) { jc[u] = j1[u]; j1[u] = j2[u]; pc[u] = pn[u]; }
         }
+
+        if constexpr (MIXED) {
+            if (unsure) {
+                // Rare (~3 entries in a million): this lane met an entry whose binary32 r^2 is within 2e-6 r_c^2 of the
+                // cutoff.  Its partial sums are recomputed with every decision taken from the binary64 records, exactly
+                // as the FP64 path takes it (reading Q7: set membership is the oracle's).
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { acc0[c] = 0.0; acc1[c] = 0.0; f0[c] = 0.f; f1[c] = 0.f; }
+                np_row = 0;
+                const RecF &fa = reinterpret_cast<const RecF &>(pa), &fb = reinterpret_cast<const RecF &>(pb);
+                for (int it = 0; it < niter; ++it) {
+                    const int j = row[it * LPA];
+                    const double4 p = load_record(recs + j);
+                    const RecF &fp = reinterpret_cast<const RecF &>(p);
+                    const bool in0 = j != i0 && nlist_exact_in_range(a.xs, i0, j, rc2);
+                    const bool in1 = j != i1 && nlist_exact_in_range(a.xs, i1, j, rc2);
+                    nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, nlist_geom_f(fa, fp), in0, Anf, n_exp, m_exp, f0, np_row);
+                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, np_row);
+                    if ((it & 3) == 3) flush();                  // same flush points as the fast loop
+                }
+                flush();
+            }
+        }
+        npairs += np_row;
 
         // ---- reduce over the LPA lanes of the pair (fixed order) ----
         constexpr int NV = FORCE ? (ENERGY ? 4 : 3) : 1;
@@ -604,7 +674,9 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                     const double rho = a.c.am * acc[0];
                     a.rho[i] = rho;
                     const double root = rho > 0.0 ? sqrt(rho) : 0.0;       // reading Q9
-                    a.xs[i].w = rho > 0.0 ? a.c.Bm / root : 0.0;
+                    const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;
+                    a.xs[i].w = sp;
+                    if constexpr (MIXED) a.xfr[i].s = float(sp);
                     contrib += root;
                 } else {
                     a.force[3 * size_t(i)] = acc[0];

@@ -22,13 +22,14 @@ enum ScalarSlot {
 
 #ifdef SCMD_MAIN_TU   // the non-template kernels are compiled in scmd.cu only
 // pos[N*3] -> xs[N] = (x, y, z, 0); xf (mixed all-pairs path, else NULL) gets the split record
-__global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, FPair *__restrict__ xf,
+__global__ void pack_positions_kernel(const double *__restrict__ pos, double4 *__restrict__ xs, FPair *__restrict__ xf, RecF *__restrict__ xfr,
                                       int N) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < N) {
         const double x = pos[3 * size_t(i)], y = pos[3 * size_t(i) + 1], z = pos[3 * size_t(i) + 2];
         xs[i] = make_double4(x, y, z, 0.0);
         if (xf) store_split_record(xf, i, x, y, z, 0.f);
+        if (xfr) xfr[i] = split_record(make_double4(x, y, z, 0.0));     // mixed list sweeps
     }
 }
 __global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *__restrict__ pos, int N) {
@@ -43,7 +44,7 @@ __global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *
 // (hk = dt/2 * ACC / m).  ref (may be NULL): positions at the last list build; the largest squared
 // displacement from it goes to scal[kSlotMaxDisp2] through an integer atomicMax (order-free).
 __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__ vel, const double *__restrict__ force,
-                                  double *__restrict__ scal, const double4 *__restrict__ ref, FPair *__restrict__ xf,
+                                  double *__restrict__ scal, const double4 *__restrict__ ref, FPair *__restrict__ xf, RecF *__restrict__ xfr,
                                   int N, double hk, double dt) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     double d2 = 0.0;
@@ -58,6 +59,7 @@ __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__
         vel[3 * size_t(i)] = vx; vel[3 * size_t(i) + 1] = vy; vel[3 * size_t(i) + 2] = vz;
         xs[i] = p;
         if (xf) store_split_record(xf, i, p.x, p.y, p.z, float(p.w));
+        if (xfr) xfr[i] = split_record(p);
         if (ref) {
             const double4 r = ref[i];
             const double ex = p.x - r.x, ey = p.y - r.y, ez = p.z - r.z;

@@ -176,14 +176,7 @@ __device__ __forceinline__ void small_force_term(const double4 &pi, const double
 // ---- mixed precision (binary32 pair arithmetic on split coordinates, binary64 accumulation) ----
 // staged record: x = xh + xl with xh = fl32(x), xl = fl32(x - xh), so that (xh_i - xh_j) + (xl_i - xl_j) keeps the
 // accuracy of a binary64 subtraction to within binary32 rounding of the DIFFERENCE (as in allpairs32_kernel)
-struct __align__(32) SmallRecF { float xh, yh, zh, s, xl, yl, zl, pad; };
-static_assert(sizeof(SmallRecF) == sizeof(double4), "same staging footprint in both precisions");
-__device__ __forceinline__ SmallRecF split_record(const double4 &p) {
-    SmallRecF r;
-    r.xh = float(p.x); r.yh = float(p.y); r.zh = float(p.z); r.s = float(p.w);
-    r.xl = float(p.x - double(r.xh)); r.yl = float(p.y - double(r.yh)); r.zl = float(p.z - double(r.zh)); r.pad = 0.f;
-    return r;
-}
+using SmallRecF = RecF;
 template <int ME>
 __device__ __forceinline__ float small_density_term_f(const SmallRecF &pi, const SmallRecF &p, bool self, int m_exp) {
     const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);

@@ -60,6 +60,7 @@ struct sc_ctx {
     unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
     unsigned long long small_barrier_count = 0;
     double4 *xs_b = nullptr;      // [N] second record buffer of the one-launch step loop (small all-pairs clusters)
+    RecF *xfr = nullptr;          // [N + 1] split binary32 records (mixed list sweeps only)
     FPair *xf = nullptr;          // [(N + 512) / 2 + 1] packed split binary32 records (mixed all-pairs path only)
     double *vel = nullptr;        // [N*3]
     double *force = nullptr;      // [N*3]
@@ -180,6 +181,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         const int kmax = default_kmax(prm, N, skin), md = cutoff_max_dim(N);
         const size_t ncell = size_t(md) * md * md + 2;
         double4 *xa = w.take<double4>(n + kTileAtoms);
+        RecF *xfr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;
         double4 *xr = w.take<double4>(n);
         double *va = w.take<double>(3 * n);
         double *bp = w.take<double>(9 * size_t(kMaxCoopBlocks));
@@ -191,7 +193,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         CellGrid *grid = w.take<CellGrid>(1);
         unsigned long long *counters = w.take<unsigned long long>(kNumCounters);
         if (c && base) {
-            c->xs_alt = xa; c->xs_ref = xr; c->vel_alt = va; c->blockpart = bp; c->perm = perm; c->perm_alt = perm_alt;
+            c->xs_alt = xa; c->xfr = xfr; c->xs_ref = xr; c->vel_alt = va; c->blockpart = bp; c->perm = perm; c->perm_alt = perm_alt;
             c->cell_of = cell_of; c->slot_of = slot_of; c->cell_sorted = cell_sorted; c->order_tmp = order_tmp;
             c->order = order; c->ncount = ncount; c->cell_count = cell_count; c->cell_start = cell_start;
             c->nlist = nlist; c->scanpart = scanpart; c->grid = grid; c->counters = counters;
@@ -290,7 +292,7 @@ TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
 sc_status ensure_list(sc_ctx *c) {
     if (!c->cutoff || c->list_checked) return SC_OK;
     RebuildArgs a{};
-    a.xs = c->xs; a.xs_alt = c->xs_alt; a.xs_ref = c->xs_ref; a.vel = c->vel; a.vel_alt = c->vel_alt;
+    a.xs = c->xs; a.xs_alt = c->xs_alt; a.xs_ref = c->xs_ref; a.xfr = c->xfr; a.vel = c->vel; a.vel_alt = c->vel_alt;
     a.perm = c->perm; a.perm_alt = c->perm_alt; a.cell_of = c->cell_of; a.slot_of = c->slot_of;
     a.cell_sorted = c->cell_sorted; a.cell_count = c->cell_count; a.cell_start = c->cell_start;
     a.order_tmp = c->order_tmp; a.order = c->order; a.nlist = c->nlist; a.ncount = c->ncount;
@@ -328,7 +330,7 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     if (st != SC_OK) return st;
     const int lpa = choose_lpa(c);
     NlistArgs a{};
-    a.xs = c->xs; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.kmax = c->kmax;
+    a.xs = c->xs; a.xfr = c->xfr; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.kmax = c->kmax;
     const int warps = choose_nlist_warps(c);
     a.pairs_per_cta = choose_pairs_per_cta(c, lpa, warps);
     a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
@@ -538,7 +540,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     const double ndof = double(3 * c->N - 3);
     for (int64_t k = 1; k <= nsteps; ++k) {
         kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, c->cutoff ? c->xs_ref : nullptr,
-                                                        c->xf, N, hk, dt);
+                                                        c->xf, c->xfr, N, hk, dt);
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
         c->list_checked = false;
@@ -722,7 +724,7 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
 sc_status sc_set_state(sc_ctx *c, const double *d_pos, const double *d_vel) {
     if (!c || !d_pos) return fail(c, SC_ERR_INVALID, "sc_set_state: d_pos is NULL%s");
     const int N = int(c->N);
-    pack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(d_pos, c->xs, c->xf, N);
+    pack_positions_kernel<<<ceil_div(N, kBlock), kBlock, 0, c->stream>>>(d_pos, c->xs, c->xf, c->xfr, N);
     SC_CUDA_CHECK(c, cudaGetLastError());
     c->launches += 1;
     c->have_pos = true;
