@@ -34,7 +34,7 @@
  *
  * Stream: every call enqueues on the cudaStream_t given to sc_create and returns without
  * waiting, except the calls that return a host scalar or copy to host memory
- * (sc_energy, sc_kinetic, sc_stats, sc_eval_host, sc_step_host), which synchronise that stream.
+ * (sc_energy, sc_kinetic, sc_stats, sc_rdf, sc_eval_host, sc_step_host), which synchronise that stream.
  *
  * Errors: every call returns an sc_status; nothing is thrown across the ABI and nothing is
  * printed.  sc_last_error gives a human-readable message for the last failing call on a ctx.
@@ -100,10 +100,14 @@ typedef enum {
     SC_OPT_ROWS_PER_THREAD = 1,   /* i-atoms held in registers per thread: 1, 2 or 4           */
     SC_OPT_LANES_PER_ROW = 2,     /* lanes of a warp that share one row group: 1,2,4,8,16,32
                                      (list sweeps: lanes per neighbour row, 8, 16 or 32; smaller
-                                     values are raised to 8)                                     */
+                                     values are raised to 8; one-launch step loop: threads of a
+                                     row inside one warp)                                        */
     SC_OPT_WARPS_PER_CTA = 3,     /* consumer warps per CTA (they split the j range): 1..8      */
-    SC_OPT_PERSISTENT = 4,        /* 1: whole sc_step loop in one cooperative kernel (small N);
-                                     2: never; 0: choose by N                                    */
+    SC_OPT_PERSISTENT = 4,        /* all pairs, N <= 6144: the whole sc_step loop (all nsteps) in ONE
+                                     cooperative launch, records staged in shared memory, grid
+                                     barriers between the phases of a step.  0: library default
+                                     (on whenever it applies), 1: on, 2: never (one launch per
+                                     sweep and per integrator stage).  Off while sc_profile is on. */
     SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
     SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max entries per row of the Verlet list (cutoff path); rounded
                                      down to a multiple of 32 (at least 32)                      */
