@@ -346,6 +346,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
                 const double4 pi = sm[i];
                 double b[4] = {0.0, 0.0, 0.0, 0.0};               // second chain
                 int j = q;
+                for (; j + 3 * JL < N; j += 4 * JL) {              // 4 independent pair terms in flight
+                    small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
+                    small_force_term<NE, ME>(pi, sm[j + JL], j + JL == i, An, n_exp, m_exp, b);
+                    small_force_term<NE, ME>(pi, sm[j + 2 * JL], j + 2 * JL == i, An, n_exp, m_exp, acc);
+                    small_force_term<NE, ME>(pi, sm[j + 3 * JL], j + 3 * JL == i, An, n_exp, m_exp, b);
+                }
                 for (; j + JL < N; j += 2 * JL) {
                     small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
                     small_force_term<NE, ME>(pi, sm[j + JL], j + JL == i, An, n_exp, m_exp, b);
