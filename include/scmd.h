@@ -114,8 +114,12 @@ typedef enum {
     SC_OPT_LANGEVIN_STEP = 7,     /* generator step of the next Langevin update (>= 0)          */
     SC_OPT_CELLS_PER_RADIUS = 8,  /* cutoff path: cell edge = list radius / G, G = 1..4 (default 4);
                                      takes effect at the next list build                         */
-    SC_OPT_ATOMS_PER_CTA = 9      /* cutoff path: consecutive atoms one CTA of the list sweeps
+    SC_OPT_ATOMS_PER_CTA = 9,     /* cutoff path: consecutive atoms one CTA of the list sweeps
                                      works through (rounded to the warp layout)                  */
+    SC_OPT_NEWTON3 = 10           /* all pairs, FP64, 8192 <= N <= 131072: evaluate every unordered
+                                     pair once and add its term to both atoms (0: library default
+                                     = on where its partial sums fit the workspace, 1: on,
+                                     2: off = the one-sided sweeps)                              */
 } sc_option;
 
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */

@@ -1,0 +1,236 @@
+// sc_allpairs_n3.cuh -- the two all-pairs sweeps with Newton's third law: every UNORDERED pair is
+// evaluated once and its term is added to both atoms, 13 / 25 FP64 instructions per unordered pair instead of
+// 2 x 11 / 2 x 22 for the two ordered pairs (PAPER.md:127 has one particle per thread and full N^2).
+//
+// Decomposition.  A CTA (8 warps) owns a block of RB = 32 * IT rows i; lane t of EVERY warp holds rows
+// row0 + k * 32 + t (k < IT) in registers.  The j range is cut into chunks of 32 atoms; the block takes the chunks
+// from its own first chunk to the end (the upper triangle), warp w every 8th of them.  For a chunk, lane t loads
+// atom j = 32 c + t and the warp ROTATES the chunk through its lanes: 32 steps, in each of which a lane evaluates
+// its IT rows against the j record it currently holds and then passes the record -- together with the reaction
+// sums accumulated on it so far -- to the next lane by warp shuffles.  After 32 steps every record is back in its
+// home lane carrying the sum over the warp's 32 * IT rows, and is stored as this block's partial for j.  No atomics,
+// no shared memory in the loop; rows i accumulate in registers as in the one-sided sweeps.
+//
+// Diagonal: in the chunks that overlap the block's own rows a pair counts iff j > i (by index); pairs with i or j
+// beyond N are evaluated on dummy records 1e100 away, whose terms underflow to exact zeros.
+//
+// Sums.  part[b][j] (j >= first row of block b: triangular storage) holds block b's reaction sums, self[i] the
+// row sums of i's own block; a finalize kernel adds self[i] + part[0..block(i)][i] in that fixed order, so the
+// result is bit-reproducible.  Storage: ~N^2 / (2 RB) records of 32 bytes (0.54 GB at N = 65536), which is what
+// limits the variant to N <= 131072.
+#pragma once
+#include "sc_allpairs.cuh"
+#include "sc_device.cuh"
+
+namespace scmd {
+
+constexpr int kN3Warps = 8;
+constexpr double kN3Far = 1.0e100;
+
+struct N3Args {
+    const double4 *xs;      // [N] (x, y, z, s')
+    int n_atoms, n_pad;     // n_pad = round_up(N, 32)
+    double4 *part;          // triangular: block b at offset n3_part_offset(b), n_pad - b * RB records (FORCE) ...
+    double *part_rho;       // ... or doubles (density sweep); the same memory
+    double4 *self;          // [n_pad] row sums of the atom's own block (x, y, z) / (rho, -, -)
+    double *partial;        // [gridDim.x] per-CTA sum r^-n over ORDERED pairs (FORCE && ENERGY)
+    PairConsts c;
+};
+
+__host__ __device__ inline size_t n3_part_offset(int b, int n_pad, int rb) {
+    return size_t(b) * size_t(n_pad) - size_t(rb) * (size_t(b) * size_t(b > 0 ? b - 1 : 0) / 2);
+}
+inline size_t n3_part_records(int n_atoms, int rb) {
+    const int n_pad = (n_atoms + 31) / 32 * 32, nb = (n_atoms + rb - 1) / rb;
+    return n3_part_offset(nb, n_pad, rb);
+}
+
+__device__ __forceinline__ double rot1(double v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
+__device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
+
+template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
+__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3Args a) {
+    constexpr int RB = 32 * IT;
+    __shared__ double red[kN3Warps][IT][4][32];            // epilogue: per-warp row sums
+    __shared__ double red_e[kN3Warps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int N = a.n_atoms;
+    const int row0 = blockIdx.x * RB;
+    const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
+    const double An = a.c.An;
+
+    int irow[IT];
+    double xi[IT], yi[IT], zi[IT], si[IT];
+    double f0[IT], f1[IT], f2[IT];
+    double esum = 0.0;
+#pragma unroll
+    for (int k = 0; k < IT; ++k) {
+        irow[k] = row0 + k * 32 + lane;
+        if (irow[k] < N) {
+            const double4 p = a.xs[irow[k]];
+            xi[k] = p.x; yi[k] = p.y; zi[k] = p.z; si[k] = p.w;
+        } else {                                           // dummy row: far from everything, also from the dummy j
+            xi[k] = kN3Far * double(k + 2); yi[k] = -kN3Far * double(lane + 1); zi[k] = 0.0; si[k] = 0.0;
+        }
+        f0[k] = f1[k] = f2[k] = 0.0;
+    }
+
+    const int cb = row0 >> 5, nch = (N + 31) >> 5;
+    double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    for (int c = cb + warp; c < nch; c += kN3Warps) {
+        int jidx = (c << 5) + lane;
+        double xj, yj, zj, sj;
+        if (jidx < N) {
+            const double4 p = a.xs[jidx];
+            xj = p.x; yj = p.y; zj = p.z; sj = p.w;
+        } else {
+            xj = -kN3Far * double(lane + 1); yj = kN3Far; zj = kN3Far; sj = 0.0;
+        }
+        const int jhome = jidx;
+        double g0 = 0.0, g1 = 0.0, g2 = 0.0;               // reaction sums travelling with the record
+        const bool diag = c < cb + IT;                     // warp-uniform
+        auto step = [&](auto masked) {
+            // the record of the NEXT step is fetched first (positions do not change): its shuffle latency hides
+            // behind this step's arithmetic; only the reaction sums have to wait for it
+            const double xn = rot1(xj), yn = rot1(yj), zn = rot1(zj);
+            double sn = 0.0;
+            if constexpr (FORCE) sn = rot1(sj);
+            int jn = 0;
+            if constexpr (decltype(masked)::value) jn = rot1(jidx);
+#pragma unroll
+            for (int k = 0; k < IT; ++k) {
+                const double dx = xi[k] - xj, dy = yi[k] - yj, dz = zi[k] - zj;
+                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                if constexpr (!FORCE) {
+                    double term;
+                    if constexpr (ME > 0 && ME % 2 == 0) {
+                        double w = rcp_fast(r2);
+                        if constexpr (decltype(masked)::value) w = jidx > irow[k] ? w : 0.0;
+                        term = ipow_c<ME / 2>(w);
+                    } else {
+                        double y = rsqrt_fast(r2);
+                        if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.0;
+                        term = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+                    }
+                    f0[k] += term;
+                    g0 += term;
+                } else {
+                    double y = rsqrt_fast(r2);
+                    if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.0;
+                    const double w = y * y;
+                    const double ss = si[k] + sj;
+                    double coef, pn;
+                    if constexpr (NE == 9 && ME == 6) {
+                        const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
+                        coef = w4 * fma(An, y3, -ss);
+                        pn = w4 * y;
+                    } else {
+                        const double pm = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+                        pn = (NE > 0) ? ipow_c<(NE > 0 ? NE : 1)>(y) : ipow_rt(y, n_exp);
+                        coef = w * fma(An, pn, -ss * pm);
+                    }
+                    if constexpr (ENERGY) esum += pn;
+                    f0[k] = fma(coef, dx, f0[k]); f1[k] = fma(coef, dy, f1[k]); f2[k] = fma(coef, dz, f2[k]);
+                    g0 = fma(-coef, dx, g0); g1 = fma(-coef, dy, g1); g2 = fma(-coef, dz, g2);
+                }
+            }
+            // pass the sums on with the record
+            g0 = rot1(g0);
+            if constexpr (FORCE) { g1 = rot1(g1); g2 = rot1(g2); sj = sn; }
+            xj = xn; yj = yn; zj = zn;
+            if constexpr (decltype(masked)::value) jidx = jn;
+        };
+        if (diag) {
+            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
+        } else {
+#pragma unroll 2
+            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
+        }
+        // the record is home again (32 rotations by one lane)
+        if (jhome < N) {
+            if constexpr (FORCE) part[jhome - row0] = make_double4(g0, g1, g2, 0.0);
+            else part_rho[jhome - row0] = g0;
+        }
+    }
+
+    // ---- rows i: sum over the warps of the CTA in a fixed order ----
+#pragma unroll
+    for (int k = 0; k < IT; ++k) {
+        red[warp][k][0][lane] = f0[k];
+        if constexpr (FORCE) { red[warp][k][1][lane] = f1[k]; red[warp][k][2][lane] = f2[k]; }
+    }
+    if constexpr (FORCE && ENERGY) {
+        esum = warp_sum(esum);
+        if (lane == 0) red_e[warp] = esum;
+    }
+    __syncthreads();
+    for (int r = threadIdx.x; r < RB; r += kN3Warps * 32) {
+        const int k = r >> 5, l = r & 31, i = row0 + r;
+        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+        for (int w = 0; w < kN3Warps; ++w) {
+            v0 += red[w][k][0][l];
+            if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
+        }
+        if (i < N) a.self[i] = make_double4(v0, v1, v2, 0.0);
+    }
+    if constexpr (FORCE && ENERGY) {
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
+            a.partial[blockIdx.x] = 2.0 * tot;             // every unordered pair stands for two ordered ones
+        }
+    }
+}
+
+// ---- finalize: self[i] + part[0 .. block(i)][i] in that order ----
+struct N3FinalArgs {
+    double4 *xs;
+    const double4 *part;
+    const double *part_rho;
+    const double4 *self;
+    double *rho, *force, *partial;      // partial: [gridDim.x] sum sqrt(rho) (density)
+    int n_atoms, n_pad, rb;
+    PairConsts c;
+};
+
+#ifdef SCMD_MAIN_TU
+template <bool FORCE>
+__global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
+    __shared__ double scratch[32];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double contrib = 0.0;
+    if (i < a.n_atoms) {
+        const int bi = i / a.rb;
+        const double4 s = a.self[i];
+        double v0 = s.x, v1 = s.y, v2 = s.z;
+        for (int b = 0; b <= bi; ++b) {
+            const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(i - b * a.rb);
+            if constexpr (FORCE) {
+                const double4 p = a.part[at];
+                v0 += p.x; v1 += p.y; v2 += p.z;
+            } else {
+                v0 += a.part_rho[at];
+            }
+        }
+        if constexpr (FORCE) {
+            a.force[3 * size_t(i)] = v0; a.force[3 * size_t(i) + 1] = v1; a.force[3 * size_t(i) + 2] = v2;
+        } else {
+            const double rho = a.c.am * v0;
+            if (a.rho) a.rho[i] = rho;
+            const double root = rho > 0.0 ? sqrt(rho) : 0.0;           // reading Q9
+            a.xs[i].w = rho > 0.0 ? a.c.Bm / root : 0.0;
+            contrib = root;
+        }
+    }
+    if constexpr (!FORCE) {
+        const double t = block_sum(contrib, scratch);
+        if (threadIdx.x == 0) a.partial[blockIdx.x] = t;
+    }
+}
+#endif  // SCMD_MAIN_TU
+
+// instantiated in inst_allpairs_n3.cu; nullptr if this shape is not compiled
+const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy);
+
+}  // namespace scmd

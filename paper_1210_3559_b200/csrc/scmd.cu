@@ -16,6 +16,7 @@
 #include "sc_probe.cuh"
 #include "sc_small.cuh"
 #include "sc_analysis.cuh"
+#include "sc_allpairs_n3.cuh"
 
 using namespace scmd;
 
@@ -56,6 +57,8 @@ struct sc_ctx {
     unsigned long long *rdf_counts = nullptr;   // [kRdfMaxBins + 1] histogram; the last word is the reference-atom count
     int *rdf_refs = nullptr;      // [N] reference atoms of sc_rdf
     double *rdf_meta = nullptr;   // [4] centre
+    double4 *n3_part = nullptr;   // Newton's-third-law sweeps: triangular reaction partials, row sums (else NULL)
+    double4 *n3_self = nullptr;
     double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
     unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
     unsigned long long small_barrier_count = 0;
@@ -96,7 +99,7 @@ struct sc_ctx {
     std::vector<OccEntry> occ_cache;
 
     // options (0 = default)
-    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0;
+    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0;
 
     // profiling
     bool profile = false;
@@ -145,6 +148,11 @@ int cutoff_max_dim(int64_t N) {
     return d;
 }
 
+// Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
+constexpr int64_t kN3MinAtoms = 8192, kN3MaxAtoms = 131072;   // workspace carved in this range
+constexpr int64_t kN3DefaultMinAtoms = 24576;                  // measured: below ~24k the triangle leaves SMs idle
+constexpr int kN3RowsPerThread = 4;
+
 // one place that lays the workspace out; base == nullptr only measures
 size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin) {
     Carver w(base);
@@ -172,6 +180,11 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         double *spr = w.take<double>(n);
         unsigned long long *bar = w.take<unsigned long long>(2);
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
+    }
+    if (!(prm->r_cut > 0.0) && precision == SC_PREC_FP64 && N >= kN3MinAtoms && N <= kN3MaxAtoms) {
+        double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
+        double4 *ns = w.take<double4>(n + 32);
+        if (c && base) { c->n3_part = np; c->n3_self = ns; }
     }
     if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
         FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
@@ -364,8 +377,42 @@ sc_status check_flags(sc_ctx *c) {
     return SC_OK;
 }
 
+// all pairs, every unordered pair once (sc_allpairs_n3.cuh): sweep + finalize + scalar reduction
+sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
+    const bool fast = (c->p.n == 9 && c->p.m == 6);
+    const int it = kN3RowsPerThread, rb = 32 * it, N = int(c->N);
+    const void *fn = allpairs_n3_fn(it, fast, force, energy);
+    if (!fn) return fail(c, SC_ERR_INVALID, "Newton's-third-law sweep: no kernel for this shape%s");
+    const int nb = ceil_div(N, rb);
+    N3Args a{};
+    a.xs = c->xs; a.n_atoms = N; a.n_pad = round_up(N, 32);
+    a.part = c->n3_part; a.part_rho = reinterpret_cast<double *>(c->n3_part); a.self = c->n3_self;
+    a.partial = c->part_b; a.c = c->consts;
+    void *params[1] = {&a};
+    cudaError_t e = cudaLaunchKernel(fn, dim3(nb), dim3(kN3Warps * 32), params, 0, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
+    N3FinalArgs f{};
+    f.xs = c->xs; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
+    f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.c = c->consts;
+    const int fb = ceil_div(N, 256);
+    if (force) n3_finalize_kernel<true><<<fb, 256, 0, c->stream>>>(f);
+    else n3_finalize_kernel<false><<<fb, 256, 0, c->stream>>>(f);
+    c->launches += 2;
+    if (!force) {
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, fb, c->scal, kSlotEEmb, -c->consts.eps_c);
+        c->launches += 1;
+    } else if (energy) {
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, nb, c->scal, kSlotEPair, c->consts.En);
+        c->launches += 1;
+    }
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    return SC_OK;
+}
+
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (c->cutoff) return run_sweep_cutoff(c, force, energy);
+    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || c->N >= kN3DefaultMinAtoms) && !c->opt_it && !c->opt_tpr)
+        return run_sweep_n3(c, force, energy);
     TileChoice tc = choose_tile(c, force, energy);
     const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);
     if (!fn) return fail(c, SC_ERR_INVALID, "all-pairs sweep: no kernel for this tile shape%s");
@@ -710,6 +757,11 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
                 reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
                 c->density_valid = c->forces_valid = c->energy_valid = false;
             }
+            break;
+        case SC_OPT_NEWTON3:
+            if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "Newton's third law must be 0, 1 or 2%s");
+            c->opt_n3 = int(value);
+            c->density_valid = c->forces_valid = c->energy_valid = false;
             break;
         case SC_OPT_ATOMS_PER_CTA:
             if (value < 0 || value > 4096) return fail(c, SC_ERR_INVALID, "atoms per CTA must be 0..4096%s");

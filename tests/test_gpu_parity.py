@@ -85,6 +85,39 @@ def test_tile_shapes_ragged(scmd, oracle_ld, it, tpr, warps):
     check_eval(scmd, oracle_ld, w.pos, options=opts)
 
 
+@pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3)),
+                                        (12345, dict(n=7, m=3, eps=0.02, c=30.0, a=3.3))])
+def test_newton3_sweeps(scmd, oracle_ld, n_atoms, kw):
+    """Every unordered pair once, its term added to both atoms (csrc/sc_allpairs_n3.cuh): block-aligned and ragged
+    sizes (dummy rows and records, diagonal chunks), (9, 6) and generic exponents; same tolerances as the one-sided
+    sweeps, and the two agree with each other to rounding."""
+    w = W.fcc_cluster(n_atoms, 1500.0, seed=81)
+    on = {scmd.SC_OPT_NEWTON3: 1}
+    check_eval(scmd, oracle_ld, w.pos, options=on, **kw)
+    a = gpu_eval(scmd, w.pos, options=on, **kw)
+    b = gpu_eval(scmd, w.pos, options={scmd.SC_OPT_NEWTON3: 2}, **kw)
+    a2 = gpu_eval(scmd, w.pos, options=on, **kw)
+    for sc in (a[0], b[0], a2[0]):
+        sc.close()
+    assert rel_l2(a[2], b[2]) < 1e-12 and rel(a[3], b[3]) < 1e-13
+    assert np.array_equal(a[1], a2[1]) and np.array_equal(a[2], a2[2]) and a[3] == a2[3]      # bit-reproducible
+
+
+def test_newton3_trajectory(scmd, oracle_ld):
+    """100 velocity-Verlet steps at N = 8192 through the Newton's-third-law sweeps: positions within 1e-8 A."""
+    import torch
+    w = W.fcc_cluster(8192, 1200.0, seed=82)
+    ref = oracle_ld.run(w.pos, w.vel, oracle_ld.params(), dt=1.0, nsteps=100)
+    sc = scmd.SuttonChen(8192)
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3, 1)
+    sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"), torch.as_tensor(w.vel, device="cuda"))
+    sc.sc_step(1.0, 100)
+    pos, _ = sc.sc_get_state()
+    assert np.abs(pos.cpu().numpy() - ref["pos"]).max() < TRAJ_TOL
+    assert rel(sc.sc_energy(), ref["epot"][-1]) < 1e-10
+    sc.close()
+
+
 @pytest.mark.parametrize("n_atoms", [1, 2, 3, 31, 33, 511, 512, 513, 1025])
 def test_small_and_boundary_sizes(scmd, oracle_ld, n_atoms):
     """Degenerate and tile-boundary sizes.  N = 1: rho = 0, F = 0, U = 0 (reading Q9)."""
