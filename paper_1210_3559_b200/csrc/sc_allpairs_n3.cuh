@@ -2,9 +2,9 @@
 // evaluated once and its term is added to both atoms, 13 / 25 FP64 instructions per unordered pair instead of
 // 2 x 11 / 2 x 22 for the two ordered pairs (PAPER.md:127 has one particle per thread and full N^2).
 //
-// Decomposition.  A CTA (8 warps) owns a block of RB = 32 * IT rows i; lane t of EVERY warp holds rows
+// Decomposition.  A CTA (12 warps) owns a block of RB = 32 * IT rows i; lane t of EVERY warp holds rows
 // row0 + k * 32 + t (k < IT) in registers.  The j range is cut into chunks of 32 atoms; the block takes the chunks
-// from its own first chunk to the end (the upper triangle), warp w every 8th of them.  For a chunk, lane t loads
+// from its own first chunk to the end (the upper triangle), warp w every 12th of them.  For a chunk, lane t loads
 // atom j = 32 c + t and the warp ROTATES the chunk through its lanes: 32 steps, in each of which a lane evaluates
 // its IT rows against the j record it currently holds and then passes the record -- together with the reaction
 // sums accumulated on it so far -- to the next lane by warp shuffles.  After 32 steps every record is back in its
@@ -24,7 +24,7 @@
 
 namespace scmd {
 
-constexpr int kN3Warps = 8;
+constexpr int kN3Warps = 12;
 constexpr double kN3Far = 1.0e100;
 
 struct N3Args {
@@ -51,7 +51,7 @@ __device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3Args a) {
     constexpr int RB = 32 * IT;
-    __shared__ double red[kN3Warps][IT][4][32];            // epilogue: per-warp row sums
+    __shared__ double red[kN3Warps][IT][3][32];            // epilogue: per-warp row sums
     __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int N = a.n_atoms;

@@ -149,7 +149,7 @@ int cutoff_max_dim(int64_t N) {
 }
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
-constexpr int64_t kN3MinAtoms = 8192, kN3MaxAtoms = 131072;   // workspace carved in this range
+constexpr int64_t kN3MinAtoms = 8192, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
 constexpr int64_t kN3DefaultMinAtoms = 24576;                  // measured: below ~24k the triangle leaves SMs idle
 constexpr int kN3RowsPerThread = 4;
 
@@ -380,7 +380,7 @@ sc_status check_flags(sc_ctx *c) {
 // all pairs, every unordered pair once (sc_allpairs_n3.cuh): sweep + finalize + scalar reduction
 sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
-    const int it = kN3RowsPerThread, rb = 32 * it, N = int(c->N);
+    const int it = kN3RowsPerThread, rb = 32 * it, N = int(c->N);   // measured: 2 rows per thread lose 10 % at N = 65536
     const void *fn = allpairs_n3_fn(it, fast, force, energy);
     if (!fn) return fail(c, SC_ERR_INVALID, "Newton's-third-law sweep: no kernel for this shape%s");
     const int nb = ceil_div(N, rb);
@@ -411,7 +411,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
 
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (c->cutoff) return run_sweep_cutoff(c, force, energy);
-    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || c->N >= kN3DefaultMinAtoms) && !c->opt_it && !c->opt_tpr)
+    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || (c->N >= kN3DefaultMinAtoms && !c->opt_it && !c->opt_tpr)))
         return run_sweep_n3(c, force, energy);
     TileChoice tc = choose_tile(c, force, energy);
     const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);

@@ -33,7 +33,7 @@ def test_workspace_bytes_validation(lib):
     n1 = lib.sc_workspace_bytes(ctypes.byref(P), 1415, pkg.SC_PREC_FP64, 0.0)
     n2 = lib.sc_workspace_bytes(ctypes.byref(P), 65536, pkg.SC_PREC_FP64, 0.0)
     assert 0 < n1 < 64 * 1024 * 1024 and n1 < n2 < 1024 * 1024 * 1024    # N = 65536 carves 0.54 GB of Newton's-third-law partials
-    n3 = lib.sc_workspace_bytes(ctypes.byref(P), 262144, pkg.SC_PREC_FP64, 0.0)  # beyond their range: O(N) again
+    n3 = lib.sc_workspace_bytes(ctypes.byref(P), 300000, pkg.SC_PREC_FP64, 0.0)  # beyond their range: O(N) again
     assert n3 < 256 * 1024 * 1024
     assert lib.sc_workspace_bytes(ctypes.byref(P), 0, pkg.SC_PREC_FP64, 0.0) == 0          # N < 1
     assert lib.sc_workspace_bytes(ctypes.byref(P), 100, 7, 0.0) == 0                       # precision
