@@ -265,6 +265,8 @@ def run_ours(args):
     sc = scmd.SuttonChen(N, r_cut=spec.r_cut, skin=spec.skin, precision=prec)
     d_pos = torch.as_tensor(w.pos, device=dev)
     d_vel = torch.as_tensor(w.vel, device=dev)
+    if args.one_sided:
+        sc.sc_set_option(scmd.SC_OPT_NEWTON3, 2)
     sc.sc_set_state(d_pos, d_vel)
     sc.sc_energy()                                                     # first evaluation (builds the rows)
     stats0 = sc.sc_stats()
@@ -334,7 +336,7 @@ def run_ours(args):
     if rank != 0:
         return
     i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
-    newton3 = spec.r_cut <= 0 and spec.prec == "fp64" and 24576 <= N <= 262144
+    newton3 = spec.r_cut <= 0 and spec.prec == "fp64" and 24576 <= N <= 262144 and not args.one_sided
     if newton3:
         i_f, i_d = I_FORCE_ENERGY_N3, I_DENSITY_N3
     if one_launch:
@@ -421,6 +423,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--one-sided", action="store_true",
+                    help="all pairs: force the one-sided sweeps (SC_OPT_NEWTON3 = 2) where Newton's third law is the default")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
