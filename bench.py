@@ -39,9 +39,10 @@ UNIT = "ordered pairs/s (both sweeps)"
 # thread-level FP64-pipe instructions (FP64 path) / FMA-pipe lane operations (mixed path)
 I_DENSITY = {"fp64": 11, "mixed": 16}
 I_FORCE_ENERGY = {"fp64": 22, "mixed": 27}
-# Newton's-third-law sweeps (all pairs, FP64, 24576 <= N <= 262144: csrc/sc_allpairs_n3.cuh): 13 / 25 FP64 instructions
+# Newton's-third-law sweeps (all pairs, 24576 <= N <= 262144: csrc/sc_allpairs_n3.cuh): 13 / 25 FP64 instructions
 # per UNORDERED pair = 6.5 / 12.5 per ordered pair
-I_DENSITY_N3, I_FORCE_ENERGY_N3 = 6.5, 12.5
+I_DENSITY_N3 = {"fp64": 6.5, "mixed": 10.0}      # mixed: 20 / 30 FMA-pipe lane operations per unordered pair
+I_FORCE_ENERGY_N3 = {"fp64": 12.5, "mixed": 15.0}
 # nominal B200 ALU peaks: 148 SMs x lanes x 2 FLOP x 1.965 GHz
 SM_COUNT, SM_MAX_GHZ = 148, 1.965
 LANES = {"fp64": 64, "mixed": 128}
@@ -336,9 +337,9 @@ def run_ours(args):
     if rank != 0:
         return
     i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
-    newton3 = spec.r_cut <= 0 and spec.prec == "fp64" and 24576 <= N <= 262144 and not args.one_sided
+    newton3 = spec.r_cut <= 0 and 24576 <= N <= 262144 and not args.one_sided
     if newton3:
-        i_f, i_d = I_FORCE_ENERGY_N3, I_DENSITY_N3
+        i_f, i_d = I_FORCE_ENERGY_N3[spec.prec], I_DENSITY_N3[spec.prec]
     if one_launch:
         # one kernel holds both sweeps: split its time in proportion to the instruction counts
         t_both = local_ms * 1e-3 / (args.steps * md_per_call)
@@ -360,7 +361,8 @@ def run_ours(args):
     if one_launch:
         kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
     elif newton3:
-        kernel = "allpairs_n3_kernel<force+energy> (every unordered pair once) + n3_finalize_kernel"
+        kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3f_kernel") + \
+                 "<force+energy> (every unordered pair once) + n3_finalize_kernel"
     elif spec.r_cut > 0:
         kernel = f"nlist_kernel<force+energy, {spec.prec}>"
     else:
@@ -377,9 +379,9 @@ def run_ours(args):
     if newton3:
         # the same time measured against the ONE-SIDED instruction count (22 per ordered pair, the formulation
         # BASELINE.json's north_star names): > 1 means the algorithmic saving outruns a one-sided sweep at FP64 peak
-        roofline["frac_vs_one_sided_count"] = I_FORCE_ENERGY["fp64"] * 2.0 * pairs_per_step / t_force / 1e12 / peak
-        roofline["note"] = ("frac counts the instructions this kernel must execute: 25 per unordered pair = 12.5 per "
-                            "ordered pair (DESIGN.md 6.8)")
+        roofline["frac_vs_one_sided_count"] = I_FORCE_ENERGY[spec.prec] * 2.0 * pairs_per_step / t_force / 1e12 / peak
+        roofline["note"] = (f"frac counts the instructions this kernel must execute: {2 * i_f:g} per unordered pair = "
+                            f"{i_f:g} per ordered pair (DESIGN.md 6.8)")
     if spec.r_cut > 0:
         # the list path's memory side: the method's own bytes are records in + forces out;
         # the neighbour indices (4 B per entry per sweep) are the data structure's cost

@@ -11,6 +11,20 @@ const void *pick(bool force, bool energy) {
 }
 }  // namespace
 
+namespace {
+template <int IT, int NE, int ME>
+const void *pickf(bool force, bool energy) {
+    if (!force) return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, false, false>);
+    if (energy) return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, true, true>);
+    return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, true, false>);
+}
+}  // namespace
+
+const void *allpairs_n3f_fn(int it, bool fast, bool force, bool energy) {
+    if (it == 4) return fast ? pickf<4, 9, 6>(force, energy) : pickf<4, 0, 0>(force, energy);
+    return nullptr;
+}
+
 const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy) {
     if (it == 4) return fast ? pick<4, 9, 6>(force, energy) : pick<4, 0, 0>(force, energy);
     if (it == 2) return fast ? pick<2, 9, 6>(force, energy) : pick<2, 0, 0>(force, energy);

@@ -183,9 +183,167 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     }
 }
 
+// ---- mixed precision: the same rotation in binary32 on split records (x = xh + xl, RecF), binary64 accumulation ----
+// Rows accumulate in binary32 over one chunk (32 terms) and are then added into binary64 sums; the reaction sums
+// travel in binary32 (128 terms) and are stored as binary64 partials.  No binary64 instruction in the rotation.
+// Sweep 1 keeps TWO binary32 sums per accumulator, one for pairs closer than 20 A and one for the rest: a far term
+// (r^-6 ~ 1e-11) added to a sum that already holds a nearest-neighbour term (4e-3) would be absorbed entirely, a
+// one-sided loss that biased rho by ~1.5e-7 and the energy by 6-8e-8 of BASELINE.json's 1e-7 (measured before the
+// split); the energy and force terms of sweep 2 fall off as r^-9, r^-10 and need no such care.
+__device__ __forceinline__ float rot1(float v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
+
+struct N3FArgs {
+    const RecF *xfr;        // [N] split binary32 records
+    int n_atoms, n_pad;
+    double4 *part;
+    double *part_rho;
+    double4 *self;
+    double *partial;
+    PairConsts c;
+};
+
+template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
+__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3FArgs a) {
+    constexpr int RB = 32 * IT;
+    __shared__ double red[kN3Warps][IT][3][32];
+    __shared__ double red_e[kN3Warps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int N = a.n_atoms;
+    const int row0 = blockIdx.x * RB;
+    const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
+    const float Anf = float(a.c.An);
+    constexpr float kFarF = 1.0e15f;                       // r^2 ~ 1e30 stays finite, its reciprocal powers vanish
+
+    int irow[IT];
+    RecF pi[IT];
+    double F0[IT], F1[IT], F2[IT];
+    double esum = 0.0;
+#pragma unroll
+    for (int k = 0; k < IT; ++k) {
+        irow[k] = row0 + k * 32 + lane;
+        if (irow[k] < N) pi[k] = a.xfr[irow[k]];
+        else pi[k] = RecF{kFarF * float(k + 2), -kFarF * float(lane + 1), 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        F0[k] = F1[k] = F2[k] = 0.0;
+    }
+    const int cb = row0 >> 5, nch = (N + 31) >> 5;
+    double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    for (int c = cb + warp; c < nch; c += kN3Warps) {
+        int jidx = (c << 5) + lane;
+        RecF pj;
+        if (jidx < N) pj = a.xfr[jidx];
+        else pj = RecF{-kFarF * float(lane + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
+        const int jhome = jidx;
+        float g0 = 0.f, g1 = 0.f, g2 = 0.f, e32 = 0.f, gfar = 0.f;
+        float f0[IT], f1[IT], f2[IT], ffar[IT];
+#pragma unroll
+        for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2[k] = ffar[k] = 0.f;
+        const bool diag = c < cb + IT;
+        auto step = [&](auto masked) {
+            RecF pn;
+            pn.xh = rot1(pj.xh); pn.yh = rot1(pj.yh); pn.zh = rot1(pj.zh);
+            pn.xl = rot1(pj.xl); pn.yl = rot1(pj.yl); pn.zl = rot1(pj.zl);
+            pn.s = 0.f; pn.pad = 0.f;
+            if constexpr (FORCE) pn.s = rot1(pj.s);
+            int jn = 0;
+            if constexpr (decltype(masked)::value) jn = rot1(jidx);
+#pragma unroll
+            for (int k = 0; k < IT; ++k) {
+                const float dx = (pi[k].xh - pj.xh) + (pi[k].xl - pj.xl), dy = (pi[k].yh - pj.yh) + (pi[k].yl - pj.yl);
+                const float dz = (pi[k].zh - pj.zh) + (pi[k].zl - pj.zl);
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                if constexpr (!FORCE) {
+                    float term;
+                    if constexpr (ME > 0 && ME % 2 == 0) {
+                        float w = rcp_fast_f(r2);
+                        if constexpr (decltype(masked)::value) w = jidx > irow[k] ? w : 0.f;
+                        term = ipow_cf<ME / 2>(w);
+                    } else {
+                        float y = rsqrt_fast_f(r2);
+                        if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.f;
+                        term = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+                    }
+                    const bool far = r2 > 400.0f;                    // 20 A
+                    const float tn = far ? 0.f : term, tf = far ? term : 0.f;
+                    f0[k] += tn; ffar[k] += tf;
+                    g0 += tn; gfar += tf;
+                } else {
+                    float y = rsqrt_fast_f(r2);
+                    if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.f;
+                    const float w = y * y;
+                    const float ss = pi[k].s + pj.s;
+                    float coef, pnw;
+                    if constexpr (NE == 9 && ME == 6) {
+                        const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+                        coef = w4 * fmaf(Anf, y3, -ss);
+                        pnw = w4 * y;
+                    } else {
+                        const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+                        pnw = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+                        coef = w * fmaf(Anf, pnw, -ss * pm);
+                    }
+                    if constexpr (ENERGY) e32 += pnw;
+                    f0[k] = fmaf(coef, dx, f0[k]); f1[k] = fmaf(coef, dy, f1[k]); f2[k] = fmaf(coef, dz, f2[k]);
+                    g0 = fmaf(-coef, dx, g0); g1 = fmaf(-coef, dy, g1); g2 = fmaf(-coef, dz, g2);
+                }
+            }
+            g0 = rot1(g0);
+            if constexpr (FORCE) { g1 = rot1(g1); g2 = rot1(g2); }
+            else gfar = rot1(gfar);
+            pj = pn;
+            if constexpr (decltype(masked)::value) jidx = jn;
+        };
+        if (diag) {
+            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
+        } else {
+#pragma unroll 2
+            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
+        }
+        if (jhome < N) {
+            if constexpr (FORCE) part[jhome - row0] = make_double4(double(g0), double(g1), double(g2), 0.0);
+            else part_rho[jhome - row0] = double(g0) + double(gfar);
+        }
+#pragma unroll
+        for (int k = 0; k < IT; ++k) {                     // one chunk of binary32 row sums into binary64
+            F0[k] += double(f0[k]);
+            if constexpr (!FORCE) F0[k] += double(ffar[k]);
+            if constexpr (FORCE) { F1[k] += double(f1[k]); F2[k] += double(f2[k]); }
+        }
+        if constexpr (FORCE && ENERGY) esum += double(e32);
+    }
+#pragma unroll
+    for (int k = 0; k < IT; ++k) {
+        red[warp][k][0][lane] = F0[k];
+        if constexpr (FORCE) { red[warp][k][1][lane] = F1[k]; red[warp][k][2][lane] = F2[k]; }
+    }
+    if constexpr (FORCE && ENERGY) {
+        esum = warp_sum(esum);
+        if (lane == 0) red_e[warp] = esum;
+    }
+    __syncthreads();
+    for (int r = threadIdx.x; r < RB; r += kN3Warps * 32) {
+        const int k = r >> 5, l = r & 31, i = row0 + r;
+        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+        for (int w = 0; w < kN3Warps; ++w) {
+            v0 += red[w][k][0][l];
+            if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
+        }
+        if (i < N) a.self[i] = make_double4(v0, v1, v2, 0.0);
+    }
+    if constexpr (FORCE && ENERGY) {
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
+            a.partial[blockIdx.x] = 2.0 * tot;
+        }
+    }
+}
+
 // ---- finalize: self[i] + part[0 .. block(i)][i] in that order ----
 struct N3FinalArgs {
     double4 *xs;
+    RecF *xfr;                          // mixed: sweep 1 stores fl32(s') here as well (else NULL)
+    FPair *xf;                          // mixed: ... and into the packed records of the one-sided sweeps
     const double4 *part;
     const double *part_rho;
     const double4 *self;
@@ -219,7 +377,10 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
             const double rho = a.c.am * v0;
             if (a.rho) a.rho[i] = rho;
             const double root = rho > 0.0 ? sqrt(rho) : 0.0;           // reading Q9
-            a.xs[i].w = rho > 0.0 ? a.c.Bm / root : 0.0;
+            const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;
+            a.xs[i].w = sp;
+            if (a.xfr) a.xfr[i].s = float(sp);
+            if (a.xf) reinterpret_cast<float *>(a.xf + (i >> 1))[6 + (i & 1)] = -float(sp);
             contrib = root;
         }
     }
@@ -232,5 +393,6 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
 
 // instantiated in inst_allpairs_n3.cu; nullptr if this shape is not compiled
 const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy);
+const void *allpairs_n3f_fn(int it, bool fast, bool force, bool energy);      // mixed precision
 
 }  // namespace scmd

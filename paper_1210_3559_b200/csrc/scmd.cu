@@ -181,10 +181,11 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         unsigned long long *bar = w.take<unsigned long long>(2);
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
     }
-    if (!(prm->r_cut > 0.0) && precision == SC_PREC_FP64 && N >= kN3MinAtoms && N <= kN3MaxAtoms) {
+    if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms) {
         double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
         double4 *ns = w.take<double4>(n + 32);
-        if (c && base) { c->n3_part = np; c->n3_self = ns; }
+        RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
+        if (c && base) { c->n3_part = np; c->n3_self = ns; if (xr) c->xfr = xr; }
     }
     if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
         FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
@@ -382,17 +383,22 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
     const int it = kN3RowsPerThread, rb = 32 * it, N = int(c->N);   // measured: 2 rows per thread lose 10 % at N = 65536
     const void *fn = allpairs_n3_fn(it, fast, force, energy);
-    if (!fn) return fail(c, SC_ERR_INVALID, "Newton's-third-law sweep: no kernel for this shape%s");
     const int nb = ceil_div(N, rb);
+    const bool mixed = c->precision == SC_PREC_MIXED;
+    if (mixed) fn = allpairs_n3f_fn(it, fast, force, energy);
+    if (!fn) return fail(c, SC_ERR_INVALID, "Newton's-third-law sweep: no kernel for this shape%s");
     N3Args a{};
     a.xs = c->xs; a.n_atoms = N; a.n_pad = round_up(N, 32);
     a.part = c->n3_part; a.part_rho = reinterpret_cast<double *>(c->n3_part); a.self = c->n3_self;
     a.partial = c->part_b; a.c = c->consts;
-    void *params[1] = {&a};
+    N3FArgs af{};
+    af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
+    af.partial = a.partial; af.c = a.c;
+    void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
     cudaError_t e = cudaLaunchKernel(fn, dim3(nb), dim3(kN3Warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
     N3FinalArgs f{};
-    f.xs = c->xs; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
+    f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
     f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.c = c->consts;
     const int fb = ceil_div(N, 256);
     if (force) n3_finalize_kernel<true><<<fb, 256, 0, c->stream>>>(f);

@@ -94,6 +94,23 @@ def test_generic_exponents_mixed(scmd, oracle_ld, n, m):
     check_eval(scmd, oracle_ld, w.pos, n=n, m=m, eps=0.02, c=30.0, a=3.3, energy_tol=2e-7)
 
 
+@pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3))])
+def test_newton3_sweeps_mixed(scmd, oracle_ld, n_atoms, kw):
+    """The Newton's-third-law sweeps in mixed precision (binary32 rotation on split records, binary64 sums):
+    BASELINE.json's mixed tolerances, and agreement with the one-sided mixed sweeps."""
+    w = W.fcc_cluster(n_atoms, 1500.0, seed=83)
+    P = oracle_ld.params(**kw)
+    rho_o, f_o, (e_o, _, _) = oracle_ld.energy_forces(w.pos, P)
+    out = {}
+    for mode in (1, 2):
+        sc, rho, f, e = gpu_eval(scmd, w.pos, options={scmd.SC_OPT_NEWTON3: mode}, **kw)
+        sc.close()
+        assert float(np.max(np.abs(rho - rho_o) / rho_o)) < RHO_TOL
+        assert rel_l2(f, f_o) < FORCE_TOL and rel(e, e_o) < ENERGY_TOL
+        out[mode] = (f, e)
+    assert rel_l2(out[1][0], out[2][0]) < 5e-6
+
+
 def test_nve_drift_and_trajectory_mixed(scmd, oracle_ld):
     """Ni1415 at 2000 K, 100 NVE steps: total energy conserved to the velocity-Verlet level and the
     trajectory stays within 1e-5 A of the binary64 oracle (the 1e-8 A bound is the FP64 path's)."""
