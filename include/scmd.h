@@ -116,10 +116,10 @@ typedef enum {
                                      takes effect at the next list build                         */
     SC_OPT_ATOMS_PER_CTA = 9,     /* cutoff path: consecutive atoms one CTA of the list sweeps
                                      works through (rounded to the warp layout)                  */
-    SC_OPT_NEWTON3 = 10           /* all pairs, either precision, 8192 <= N <= 262144 (the range in which
+    SC_OPT_NEWTON3 = 10           /* all pairs, either precision, 7000 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
-                                     both atoms.  0: library default (on for N >= 24576), 1: on,
+                                     both atoms.  0: library default (on; mixed: for N >= 16384), 1: on,
                                      2: off = the one-sided sweeps                               */
 } sc_option;
 

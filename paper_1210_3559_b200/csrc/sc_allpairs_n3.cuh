@@ -15,7 +15,7 @@
 // beyond N are evaluated on dummy records 1e100 away, whose terms underflow to exact zeros.
 //
 // Sums.  part[b][j] (j >= first row of block b: triangular storage) holds block b's reaction sums, self[i] the
-// row sums of i's own block; a finalize kernel adds self[i] + part[0..block(i)][i] in that fixed order, so the
+// row sums of i's own block, one per j segment; a finalize kernel adds self[0..][i] + part[0..block(i)][i] in that fixed order, so the
 // result is bit-reproducible.  Storage: ~N^2 / (2 RB) records of 32 bytes (0.54 GB at N = 65536), which is what
 // limits the variant to N <= 131072.
 #pragma once
@@ -32,8 +32,11 @@ struct N3Args {
     int n_atoms, n_pad;     // n_pad = round_up(N, 32)
     double4 *part;          // triangular: block b at offset n3_part_offset(b), n_pad - b * RB records (FORCE) ...
     double *part_rho;       // ... or doubles (density sweep); the same memory
-    double4 *self;          // [n_pad] row sums of the atom's own block (x, y, z) / (rho, -, -)
-    double *partial;        // [gridDim.x] per-CTA sum r^-n over ORDERED pairs (FORCE && ENERGY)
+    double4 *self;          // [gridDim.y][n_pad] row sums per j segment (x, y, z) / (rho, -, -)
+    double *partial;        // [gridDim.y * gridDim.x] per-CTA sum r^-n over ORDERED pairs (FORCE && ENERGY)
+    int seg_chunks;         // chunks of 32 atoms per j segment: CTA (b, s) takes chunks cb(b) + s L .. + L of block b's
+                            //   triangle, so that all CTAs carry about the same work (a triangle cut by rows only leaves
+                            //   the SMs idle at the end: measured 6 % at N = 65536, 20 % at N = 32768)
     PairConsts c;
 };
 
@@ -56,6 +59,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int N = a.n_atoms;
     const int row0 = blockIdx.x * RB;
+    if ((row0 >> 5) + int(blockIdx.y) * a.seg_chunks >= ((a.n_atoms + 31) >> 5)) {   // no such segment in this block's triangle
+        if (FORCE && ENERGY && threadIdx.x == 0) a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 0.0;
+        return;
+    }
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
 
@@ -76,9 +83,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     }
 
     const int cb = row0 >> 5, nch = (N + 31) >> 5;
+    const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
-    for (int c = cb + warp; c < nch; c += kN3Warps) {
+    for (int c = c_begin + warp; c < c_end; c += kN3Warps) {
         int jidx = (c << 5) + lane;
         double xj, yj, zj, sj;
         if (jidx < N) {
@@ -172,13 +180,13 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
-        if (i < N) a.self[i] = make_double4(v0, v1, v2, 0.0);
+        if (i < N) a.self[size_t(blockIdx.y) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
     }
     if constexpr (FORCE && ENERGY) {
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
-            a.partial[blockIdx.x] = 2.0 * tot;             // every unordered pair stands for two ordered ones
+            a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;   // every unordered pair stands for two ordered ones
         }
     }
 }
@@ -199,6 +207,7 @@ struct N3FArgs {
     double *part_rho;
     double4 *self;
     double *partial;
+    int seg_chunks;
     PairConsts c;
 };
 
@@ -210,6 +219,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int N = a.n_atoms;
     const int row0 = blockIdx.x * RB;
+    if ((row0 >> 5) + int(blockIdx.y) * a.seg_chunks >= ((a.n_atoms + 31) >> 5)) {   // no such segment in this block's triangle
+        if (FORCE && ENERGY && threadIdx.x == 0) a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 0.0;
+        return;
+    }
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const float Anf = float(a.c.An);
     constexpr float kFarF = 1.0e15f;                       // r^2 ~ 1e30 stays finite, its reciprocal powers vanish
@@ -226,9 +239,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3
         F0[k] = F1[k] = F2[k] = 0.0;
     }
     const int cb = row0 >> 5, nch = (N + 31) >> 5;
+    const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
-    for (int c = cb + warp; c < nch; c += kN3Warps) {
+    for (int c = c_begin + warp; c < c_end; c += kN3Warps) {
         int jidx = (c << 5) + lane;
         RecF pj;
         if (jidx < N) pj = a.xfr[jidx];
@@ -328,13 +342,13 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
-        if (i < N) a.self[i] = make_double4(v0, v1, v2, 0.0);
+        if (i < N) a.self[size_t(blockIdx.y) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
     }
     if constexpr (FORCE && ENERGY) {
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
-            a.partial[blockIdx.x] = 2.0 * tot;
+            a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;
         }
     }
 }
@@ -348,7 +362,7 @@ struct N3FinalArgs {
     const double *part_rho;
     const double4 *self;
     double *rho, *force, *partial;      // partial: [gridDim.x] sum sqrt(rho) (density)
-    int n_atoms, n_pad, rb;
+    int n_atoms, n_pad, rb, seg_chunks;
     PairConsts c;
 };
 
@@ -360,8 +374,12 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
     double contrib = 0.0;
     if (i < a.n_atoms) {
         const int bi = i / a.rb;
-        const double4 s = a.self[i];
-        double v0 = s.x, v1 = s.y, v2 = s.z;
+        const int nseg = (((a.n_atoms + 31) >> 5) - ((bi * a.rb) >> 5) + a.seg_chunks - 1) / a.seg_chunks;
+        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+        for (int sg = 0; sg < nseg; ++sg) {                 // row sums of the segments of i's own block
+            const double4 s = a.self[size_t(sg) * a.n_pad + i];
+            v0 += s.x; v1 += s.y; v2 += s.z;
+        }
         for (int b = 0; b <= bi; ++b) {
             const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(i - b * a.rb);
             if constexpr (FORCE) {

@@ -149,9 +149,10 @@ int cutoff_max_dim(int64_t N) {
 }
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
-constexpr int64_t kN3MinAtoms = 8192, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
-constexpr int64_t kN3DefaultMinAtoms = 24576;                  // measured: below ~24k the triangle leaves SMs idle
+constexpr int64_t kN3MinAtoms = 7000, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
+constexpr int64_t kN3DefaultMinAtoms = 7000, kN3DefaultMinAtomsMixed = 16384;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
+constexpr int kN3MaxSegments = 17;                             // j segments of the longest row block
 
 // one place that lays the workspace out; base == nullptr only measures
 size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin) {
@@ -183,7 +184,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
     }
     if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms) {
         double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
-        double4 *ns = w.take<double4>(n + 32);
+        double4 *ns = w.take<double4>((n + 32) * kN3MaxSegments);
         RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
         if (c && base) { c->n3_part = np; c->n3_self = ns; if (xr) c->xfr = xr; }
     }
@@ -393,13 +394,17 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     a.partial = c->part_b; a.c = c->consts;
     N3FArgs af{};
     af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
-    af.partial = a.partial; af.c = a.c;
+    // j segments: 8 (N >= 49152) or 16 of them cut the first row block's triangle; a multiple of the 12 warps each
+    const int nch = ceil_div(N, 32), want = N >= 49152 ? 8 : 16;
+    const int seg = round_up(ceil_div(nch, want), kN3Warps), nseg = ceil_div(nch, seg);
+    a.seg_chunks = seg;
+    af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
     void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
-    cudaError_t e = cudaLaunchKernel(fn, dim3(nb), dim3(kN3Warps * 32), params, 0, c->stream);
+    cudaError_t e = cudaLaunchKernel(fn, dim3(nb, nseg), dim3(kN3Warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
     N3FinalArgs f{};
     f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
-    f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.c = c->consts;
+    f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.seg_chunks = seg; f.c = c->consts;
     const int fb = ceil_div(N, 256);
     if (force) n3_finalize_kernel<true><<<fb, 256, 0, c->stream>>>(f);
     else n3_finalize_kernel<false><<<fb, 256, 0, c->stream>>>(f);
@@ -408,7 +413,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
         reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, fb, c->scal, kSlotEEmb, -c->consts.eps_c);
         c->launches += 1;
     } else if (energy) {
-        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, nb, c->scal, kSlotEPair, c->consts.En);
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, nb * nseg, c->scal, kSlotEPair, c->consts.En);
         c->launches += 1;
     }
     SC_CUDA_CHECK(c, cudaGetLastError());
@@ -417,7 +422,8 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
 
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (c->cutoff) return run_sweep_cutoff(c, force, energy);
-    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || (c->N >= kN3DefaultMinAtoms && !c->opt_it && !c->opt_tpr)))
+    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || (c->N >= (c->precision == SC_PREC_MIXED ? kN3DefaultMinAtomsMixed : kN3DefaultMinAtoms) &&
+                            !c->opt_it && !c->opt_tpr)))
         return run_sweep_n3(c, force, energy);
     TileChoice tc = choose_tile(c, force, energy);
     const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);
