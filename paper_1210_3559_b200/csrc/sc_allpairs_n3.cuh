@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         if (diag) {
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
         } else {
-#pragma unroll 2
+#pragma unroll 4
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
         }
         // the record is home again (32 rotations by one lane)
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3
         if (diag) {
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
         } else {
-#pragma unroll 2
+#pragma unroll 4
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
         }
         if (jhome < N) {
