@@ -394,8 +394,8 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     a.partial = c->part_b; a.c = c->consts;
     N3FArgs af{};
     af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
-    // j segments: 8 (N >= 49152) or 16 of them cut the first row block's triangle; a multiple of the 12 warps each
-    const int nch = ceil_div(N, 32), want = N >= 49152 ? 8 : 16;
+    // j segments: 8 (N >= 24576) or 12 of them cut the first row block's triangle; a multiple of the 12 warps each
+    const int nch = ceil_div(N, 32), want = N >= 24576 ? 8 : 12;             // measured: flat between 8 and 16
     const int seg = round_up(ceil_div(nch, want), kN3Warps), nseg = ceil_div(nch, seg);
     a.seg_chunks = seg;
     af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
