@@ -131,7 +131,7 @@ class SuttonChen:
     """One libscmd context: owns a torch workspace tensor and the opaque sc_ctx."""
 
     def __init__(self, n_atoms: int, *, n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0,
-                 precision: int = SC_PREC_FP64, skin: float = 0.0, device=None, stream=None):
+                 precision: int = SC_PREC_FP64, skin: float = 0.0, device=None, stream=None, poison: bool = False):
         torch = _torch()
         self.lib = load_library()
         self.n_atoms = int(n_atoms)
@@ -144,6 +144,8 @@ class SuttonChen:
             if nbytes == 0:
                 raise ScError(SC_ERR_INVALID, "sc_workspace_bytes", "invalid parameters")
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            if poison:                       # every byte 0xFF (NaN as binary64 / binary32, -1 as int): the library must
+                self.workspace.fill_(255)    # never read workspace memory it has not written itself
             base = (self.workspace.data_ptr() + 255) // 256 * 256
             self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
             st = self.lib.sc_create(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin),
