@@ -361,7 +361,7 @@ def run_ours(args):
     if one_launch:
         kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
     elif newton3:
-        kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3f_kernel") + \
+        kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3p_kernel") + \
                  "<force+energy> (every unordered pair once) + n3_finalize_kernel"
     elif spec.r_cut > 0:
         kernel = f"nlist_kernel<force+energy, {spec.prec}>"

@@ -13,15 +13,15 @@ const void *pick(bool force, bool energy) {
 
 namespace {
 template <int IT, int NE, int ME>
-const void *pickf(bool force, bool energy) {
-    if (!force) return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, false, false>);
-    if (energy) return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, true, true>);
-    return reinterpret_cast<const void *>(allpairs_n3f_kernel<IT, NE, ME, true, false>);
+const void *pickp(bool force, bool energy) {
+    if (!force) return reinterpret_cast<const void *>(allpairs_n3p_kernel<IT, NE, ME, false, false>);
+    if (energy) return reinterpret_cast<const void *>(allpairs_n3p_kernel<IT, NE, ME, true, true>);
+    return reinterpret_cast<const void *>(allpairs_n3p_kernel<IT, NE, ME, true, false>);
 }
 }  // namespace
 
-const void *allpairs_n3f_fn(int it, bool fast, bool force, bool energy) {
-    if (it == 4) return fast ? pickf<4, 9, 6>(force, energy) : pickf<4, 0, 0>(force, energy);
+const void *allpairs_n3p_fn(int it, bool fast, bool force, bool energy) {
+    if (it == 4) return fast ? pickp<4, 9, 6>(force, energy) : pickp<4, 0, 0>(force, energy);
     return nullptr;
 }
 

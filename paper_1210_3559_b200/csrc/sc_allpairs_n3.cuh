@@ -211,119 +211,158 @@ struct N3FArgs {
     PairConsts c;
 };
 
+// Packed: a warp rotates a chunk of 64 atoms: lane t holds records j_a = 64 c + t and j_b = 64 c + 32 + t in the two
+// halves of Blackwell's binary32 pair registers (PTX add / mul / fma.f32x2, SASS FADD2 / FMUL2 / FFMA2), j-side values
+// NEGATED so that only additions are needed; the rows i are duplicated into both halves once per launch.  One
+// rotation step is then 4 rows x 2 records = 8 pairs per lane for the instruction count of 4.
+__device__ __forceinline__ f2 rot1_f2(f2 v) {
+    return f2_make(rot1(f2_lo(v)), rot1(f2_hi(v)));
+}
+
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
-__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3f_kernel(const N3FArgs a) {
+__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3FArgs a) {
     constexpr int RB = 32 * IT;
     __shared__ double red[kN3Warps][IT][3][32];
     __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int N = a.n_atoms;
     const int row0 = blockIdx.x * RB;
-    if ((row0 >> 5) + int(blockIdx.y) * a.seg_chunks >= ((a.n_atoms + 31) >> 5)) {   // no such segment in this block's triangle
+    // a.seg_chunks counts chunks of 32 atoms and is even here: segments of seg_chunks / 2 chunks of 64
+    const int seg64 = a.seg_chunks >> 1;
+    const int cb = row0 >> 6, nch = (N + 63) >> 6;
+    const int c_begin = cb + int(blockIdx.y) * seg64, c_end = min(nch, c_begin + seg64);
+    if (c_begin >= nch) {
         if (FORCE && ENERGY && threadIdx.x == 0) a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 0.0;
         return;
     }
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
-    const float Anf = float(a.c.An);
-    constexpr float kFarF = 1.0e15f;                       // r^2 ~ 1e30 stays finite, its reciprocal powers vanish
+    const f2 An2 = f2_dup(float(a.c.An));
+    const f2 zero2 = f2_dup(0.f), one2 = f2_dup(1.0f), mone2 = f2_dup(-1.0f), mhalf2 = f2_dup(-0.5f);
+    constexpr float kFarF = 1.0e15f;
 
     int irow[IT];
-    RecF pi[IT];
+    f2 xh[IT], yh[IT], zh[IT], xl[IT], yl[IT], zl[IT], si[IT];     // row values in both halves
     double F0[IT], F1[IT], F2[IT];
     double esum = 0.0;
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
         irow[k] = row0 + k * 32 + lane;
-        if (irow[k] < N) pi[k] = a.xfr[irow[k]];
-        else pi[k] = RecF{kFarF * float(k + 2), -kFarF * float(lane + 1), 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        RecF p;
+        if (irow[k] < N) p = a.xfr[irow[k]];
+        else p = RecF{kFarF * float(k + 2), -kFarF * float(lane + 1), 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        xh[k] = f2_dup(p.xh); yh[k] = f2_dup(p.yh); zh[k] = f2_dup(p.zh);
+        xl[k] = f2_dup(p.xl); yl[k] = f2_dup(p.yl); zl[k] = f2_dup(p.zl); si[k] = f2_dup(p.s);
         F0[k] = F1[k] = F2[k] = 0.0;
     }
-    const int cb = row0 >> 5, nch = (N + 31) >> 5;
-    const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    auto fetch = [&](int j) -> RecF {
+        if (j < N) return a.xfr[j];
+        return RecF{-kFarF * float((j & 63) + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
+    };
     for (int c = c_begin + warp; c < c_end; c += kN3Warps) {
-        int jidx = (c << 5) + lane;
-        RecF pj;
-        if (jidx < N) pj = a.xfr[jidx];
-        else pj = RecF{-kFarF * float(lane + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
-        const int jhome = jidx;
-        float g0 = 0.f, g1 = 0.f, g2 = 0.f, e32 = 0.f, gfar = 0.f;
-        float f0[IT], f1[IT], f2[IT], ffar[IT];
+        const int ja = (c << 6) + lane, jb = ja + 32;
+        int jidx_a = ja, jidx_b = jb;
+        const RecF pa = fetch(ja), pb = fetch(jb);
+        // negated j records, (a, b) in the (low, high) halves
+        f2 nxh = f2_make(-pa.xh, -pb.xh), nyh = f2_make(-pa.yh, -pb.yh), nzh = f2_make(-pa.zh, -pb.zh);
+        f2 nxl = f2_make(-pa.xl, -pb.xl), nyl = f2_make(-pa.yl, -pb.yl), nzl = f2_make(-pa.zl, -pb.zl);
+        f2 sj = f2_make(pa.s, pb.s);
+        f2 g0 = zero2, g1 = zero2, g2 = zero2, gfar = zero2, e2 = zero2;
+        f2 f0[IT], f1[IT], f2v[IT], ffar[IT];
 #pragma unroll
-        for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2[k] = ffar[k] = 0.f;
-        const bool diag = c < cb + IT;
+        for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2v[k] = ffar[k] = zero2;
+        const bool diag = c < cb + IT / 2;                 // the block's own rows span IT / 2 chunks of 64
         auto step = [&](auto masked) {
-            RecF pn;
-            pn.xh = rot1(pj.xh); pn.yh = rot1(pj.yh); pn.zh = rot1(pj.zh);
-            pn.xl = rot1(pj.xl); pn.yl = rot1(pj.yl); pn.zl = rot1(pj.zl);
-            pn.s = 0.f; pn.pad = 0.f;
-            if constexpr (FORCE) pn.s = rot1(pj.s);
-            int jn = 0;
-            if constexpr (decltype(masked)::value) jn = rot1(jidx);
+            const f2 xhn = rot1_f2(nxh), yhn = rot1_f2(nyh), zhn = rot1_f2(nzh);
+            const f2 xln = rot1_f2(nxl), yln = rot1_f2(nyl), zln = rot1_f2(nzl);
+            f2 sjn = zero2;
+            if constexpr (FORCE) sjn = rot1_f2(sj);
+            int jan = 0, jbn = 0;
+            if constexpr (decltype(masked)::value) { jan = rot1(jidx_a); jbn = rot1(jidx_b); }
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
-                const float dx = (pi[k].xh - pj.xh) + (pi[k].xl - pj.xl), dy = (pi[k].yh - pj.yh) + (pi[k].yl - pj.yl);
-                const float dz = (pi[k].zh - pj.zh) + (pi[k].zl - pj.zl);
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                const f2 dx = f2_add(f2_add(xh[k], nxh), f2_add(xl[k], nxl));
+                const f2 dy = f2_add(f2_add(yh[k], nyh), f2_add(yl[k], nyl));
+                const f2 dz = f2_add(f2_add(zh[k], nzh), f2_add(zl[k], nzl));
+                const f2 r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+                bool ka = true, kb = true;                 // pair counts (diagonal chunks: iff j > i)
+                if constexpr (decltype(masked)::value) { ka = jidx_a > irow[k]; kb = jidx_b > irow[k]; }
                 if constexpr (!FORCE) {
-                    float term;
+                    f2 term;
                     if constexpr (ME > 0 && ME % 2 == 0) {
-                        float w = rcp_fast_f(r2);
-                        if constexpr (decltype(masked)::value) w = jidx > irow[k] ? w : 0.f;
-                        term = ipow_cf<ME / 2>(w);
+                        const f2 y0 = f2_make(mufu_rcp(f2_lo(r2)), mufu_rcp(f2_hi(r2)));
+                        const f2 e = f2_fma(r2, f2_mul(y0, mone2), one2);              // 1 - x y0, one rounding
+                        f2 w = f2_fma(y0, e, y0);
+                        if constexpr (decltype(masked)::value) w = f2_make(ka ? f2_lo(w) : 0.f, kb ? f2_hi(w) : 0.f);
+                        term = f2_ipow_c<ME / 2>(w);
                     } else {
-                        float y = rsqrt_fast_f(r2);
-                        if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.f;
-                        term = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+                        const f2 y0 = f2_make(mufu_rsq(f2_lo(r2)), mufu_rsq(f2_hi(r2)));
+                        const f2 ep = f2_fma(f2_mul(r2, y0), y0, mone2);
+                        f2 y = f2_fma(f2_mul(y0, ep), mhalf2, y0);
+                        if constexpr (decltype(masked)::value) y = f2_make(ka ? f2_lo(y) : 0.f, kb ? f2_hi(y) : 0.f);
+                        term = (ME > 0) ? f2_ipow_c<(ME > 0 ? ME : 1)>(y) : f2_ipow_rt(y, m_exp);
                     }
-                    const bool far = r2 > 400.0f;                    // 20 A
-                    const float tn = far ? 0.f : term, tf = far ? term : 0.f;
-                    f0[k] += tn; ffar[k] += tf;
-                    g0 += tn; gfar += tf;
+                    // two sums per accumulator (pairs closer than 20 A / the rest): see the header of this section
+                    const bool fa = f2_lo(r2) > 400.0f, fb = f2_hi(r2) > 400.0f;
+                    const f2 tn = f2_make(fa ? 0.f : f2_lo(term), fb ? 0.f : f2_hi(term));
+                    const f2 tf = f2_make(fa ? f2_lo(term) : 0.f, fb ? f2_hi(term) : 0.f);
+                    f0[k] = f2_add(f0[k], tn); ffar[k] = f2_add(ffar[k], tf);
+                    g0 = f2_add(g0, tn); gfar = f2_add(gfar, tf);
                 } else {
-                    float y = rsqrt_fast_f(r2);
-                    if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.f;
-                    const float w = y * y;
-                    const float ss = pi[k].s + pj.s;
-                    float coef, pnw;
+                    const f2 y0 = f2_make(mufu_rsq(f2_lo(r2)), mufu_rsq(f2_hi(r2)));
+                    const f2 ep = f2_fma(f2_mul(r2, y0), y0, mone2);                     // t y0 - 1
+                    f2 y = f2_fma(f2_mul(y0, ep), mhalf2, y0);                           // y0 - y0 e' / 2
+                    if constexpr (decltype(masked)::value) y = f2_make(ka ? f2_lo(y) : 0.f, kb ? f2_hi(y) : 0.f);
+                    const f2 w = f2_mul(y, y);
+                    const f2 nss = f2_fma(f2_add(si[k], sj), mone2, zero2);              // -(s'_i + s'_j)
+                    f2 coef, pnw;
                     if constexpr (NE == 9 && ME == 6) {
-                        const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
-                        coef = w4 * fmaf(Anf, y3, -ss);
-                        pnw = w4 * y;
+                        const f2 w2 = f2_mul(w, w), w4 = f2_mul(w2, w2), y3 = f2_mul(w, y);
+                        coef = f2_mul(w4, f2_fma(An2, y3, nss));
+                        pnw = f2_mul(w4, y);
                     } else {
-                        const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
-                        pnw = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
-                        coef = w * fmaf(Anf, pnw, -ss * pm);
+                        const f2 pm = (ME > 0) ? f2_ipow_c<(ME > 0 ? ME : 1)>(y) : f2_ipow_rt(y, m_exp);
+                        pnw = (NE > 0) ? f2_ipow_c<(NE > 0 ? NE : 1)>(y) : f2_ipow_rt(y, n_exp);
+                        coef = f2_mul(w, f2_fma(An2, pnw, f2_mul(nss, pm)));
                     }
-                    if constexpr (ENERGY) e32 += pnw;
-                    f0[k] = fmaf(coef, dx, f0[k]); f1[k] = fmaf(coef, dy, f1[k]); f2[k] = fmaf(coef, dz, f2[k]);
-                    g0 = fmaf(-coef, dx, g0); g1 = fmaf(-coef, dy, g1); g2 = fmaf(-coef, dz, g2);
+                    if constexpr (ENERGY) e2 = f2_add(e2, pnw);
+                    f0[k] = f2_fma(coef, dx, f0[k]); f1[k] = f2_fma(coef, dy, f1[k]); f2v[k] = f2_fma(coef, dz, f2v[k]);
+                    const f2 ncoef = f2_mul(coef, mone2);
+                    g0 = f2_fma(ncoef, dx, g0); g1 = f2_fma(ncoef, dy, g1); g2 = f2_fma(ncoef, dz, g2);
                 }
             }
-            g0 = rot1(g0);
-            if constexpr (FORCE) { g1 = rot1(g1); g2 = rot1(g2); }
-            else gfar = rot1(gfar);
-            pj = pn;
-            if constexpr (decltype(masked)::value) jidx = jn;
+            g0 = rot1_f2(g0);
+            if constexpr (FORCE) { g1 = rot1_f2(g1); g2 = rot1_f2(g2); sj = sjn; }
+            else gfar = rot1_f2(gfar);
+            nxh = xhn; nyh = yhn; nzh = zhn; nxl = xln; nyl = yln; nzl = zln;
+            if constexpr (decltype(masked)::value) { jidx_a = jan; jidx_b = jbn; }
         };
         if (diag) {
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
         } else {
-#pragma unroll 4
+#pragma unroll 2
             for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
         }
-        if (jhome < N) {
-            if constexpr (FORCE) part[jhome - row0] = make_double4(double(g0), double(g1), double(g2), 0.0);
-            else part_rho[jhome - row0] = double(g0) + double(gfar);
+        // both records are home again
+        if constexpr (FORCE) {
+            if (ja < N) part[ja - row0] = make_double4(double(f2_lo(g0)), double(f2_lo(g1)), double(f2_lo(g2)), 0.0);
+            if (jb < N) part[jb - row0] = make_double4(double(f2_hi(g0)), double(f2_hi(g1)), double(f2_hi(g2)), 0.0);
+        } else {
+            if (ja < N) part_rho[ja - row0] = double(f2_lo(g0)) + double(f2_lo(gfar));
+            if (jb < N) part_rho[jb - row0] = double(f2_hi(g0)) + double(f2_hi(gfar));
         }
 #pragma unroll
         for (int k = 0; k < IT; ++k) {                     // one chunk of binary32 row sums into binary64
-            F0[k] += double(f0[k]);
-            if constexpr (!FORCE) F0[k] += double(ffar[k]);
-            if constexpr (FORCE) { F1[k] += double(f1[k]); F2[k] += double(f2[k]); }
+            F0[k] += double(f2_lo(f0[k]) + f2_hi(f0[k]));
+            if constexpr (FORCE) {
+                F1[k] += double(f2_lo(f1[k]) + f2_hi(f1[k]));
+                F2[k] += double(f2_lo(f2v[k]) + f2_hi(f2v[k]));
+            } else {
+                F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
+            }
         }
-        if constexpr (FORCE && ENERGY) esum += double(e32);
+        if constexpr (FORCE && ENERGY) esum += double(f2_lo(e2) + f2_hi(e2));
     }
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
@@ -411,6 +450,6 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
 
 // instantiated in inst_allpairs_n3.cu; nullptr if this shape is not compiled
 const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy);
-const void *allpairs_n3f_fn(int it, bool fast, bool force, bool energy);      // mixed precision
+const void *allpairs_n3p_fn(int it, bool fast, bool force, bool energy);      // mixed precision, packed pairs
 
 }  // namespace scmd

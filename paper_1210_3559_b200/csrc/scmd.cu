@@ -386,7 +386,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const void *fn = allpairs_n3_fn(it, fast, force, energy);
     const int nb = ceil_div(N, rb);
     const bool mixed = c->precision == SC_PREC_MIXED;
-    if (mixed) fn = allpairs_n3f_fn(it, fast, force, energy);
+    if (mixed) fn = allpairs_n3p_fn(it, fast, force, energy);
     if (!fn) return fail(c, SC_ERR_INVALID, "Newton's-third-law sweep: no kernel for this shape%s");
     N3Args a{};
     a.xs = c->xs; a.n_atoms = N; a.n_pad = round_up(N, 32);
