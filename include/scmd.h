@@ -119,7 +119,7 @@ typedef enum {
     SC_OPT_NEWTON3 = 10           /* all pairs, either precision, 7000 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
-                                     both atoms.  0: library default (on; mixed: for N >= 16384), 1: on,
+                                     both atoms.  0: library default (on), 1: on,
                                      2: off = the one-sided sweeps                               */
 } sc_option;
 

@@ -197,7 +197,9 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
 // Sweep 1 keeps TWO binary32 sums per accumulator, one for pairs closer than 20 A and one for the rest: a far term
 // (r^-6 ~ 1e-11) added to a sum that already holds a nearest-neighbour term (4e-3) would be absorbed entirely, a
 // one-sided loss that biased rho by ~1.5e-7 and the energy by 6-8e-8 of BASELINE.json's 1e-7 (measured before the
-// split); the energy and force terms of sweep 2 fall off as r^-9, r^-10 and need no such care.
+// split).  The pair-energy sum of sweep 2 (r^-9) needs the same split, at 10 A: unsplit it lost 1e-7 of the energy of
+// the N = 8000 liquid droplet (a lane's sum holds a nearest-neighbour term with probability ~1500 / N); the force
+// terms have the same loss, far inside their 1e-5 tolerance.
 __device__ __forceinline__ float rot1(float v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
 
 struct N3FArgs {
@@ -268,7 +270,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         f2 nxh = f2_make(-pa.xh, -pb.xh), nyh = f2_make(-pa.yh, -pb.yh), nzh = f2_make(-pa.zh, -pb.zh);
         f2 nxl = f2_make(-pa.xl, -pb.xl), nyl = f2_make(-pa.yl, -pb.yl), nzl = f2_make(-pa.zl, -pb.zl);
         f2 sj = f2_make(pa.s, pb.s);
-        f2 g0 = zero2, g1 = zero2, g2 = zero2, gfar = zero2, e2 = zero2;
+        f2 g0 = zero2, g1 = zero2, g2 = zero2, gfar = zero2, e2 = zero2, e2far = zero2;
         f2 f0[IT], f1[IT], f2v[IT], ffar[IT];
 #pragma unroll
         for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2v[k] = ffar[k] = zero2;
@@ -326,7 +328,11 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
                         pnw = (NE > 0) ? f2_ipow_c<(NE > 0 ? NE : 1)>(y) : f2_ipow_rt(y, n_exp);
                         coef = f2_mul(w, f2_fma(An2, pnw, f2_mul(nss, pm)));
                     }
-                    if constexpr (ENERGY) e2 = f2_add(e2, pnw);
+                    if constexpr (ENERGY) {                 // two sums again: r^-9 of a pair beyond 10 A must not meet a
+                        const bool ea = f2_lo(r2) > 100.0f, eb = f2_hi(r2) > 100.0f;   // nearest-neighbour term
+                        e2 = f2_add(e2, f2_make(ea ? 0.f : f2_lo(pnw), eb ? 0.f : f2_hi(pnw)));
+                        e2far = f2_add(e2far, f2_make(ea ? f2_lo(pnw) : 0.f, eb ? f2_hi(pnw) : 0.f));
+                    }
                     f0[k] = f2_fma(coef, dx, f0[k]); f1[k] = f2_fma(coef, dy, f1[k]); f2v[k] = f2_fma(coef, dz, f2v[k]);
                     const f2 ncoef = f2_mul(coef, mone2);
                     g0 = f2_fma(ncoef, dx, g0); g1 = f2_fma(ncoef, dy, g1); g2 = f2_fma(ncoef, dz, g2);
@@ -362,7 +368,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
                 F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
             }
         }
-        if constexpr (FORCE && ENERGY) esum += double(f2_lo(e2) + f2_hi(e2));
+        if constexpr (FORCE && ENERGY) esum += double(f2_lo(e2) + f2_hi(e2)) + double(f2_lo(e2far) + f2_hi(e2far));
     }
 #pragma unroll
     for (int k = 0; k < IT; ++k) {

@@ -150,7 +150,7 @@ int cutoff_max_dim(int64_t N) {
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
 constexpr int64_t kN3MinAtoms = 7000, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
-constexpr int64_t kN3DefaultMinAtoms = 7000, kN3DefaultMinAtomsMixed = 16384;   // measured crossovers
+constexpr int64_t kN3DefaultMinAtoms = 7000, kN3DefaultMinAtomsMixed = 7000;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
 constexpr int kN3MaxSegments = 17;                             // j segments of the longest row block
 

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 @pytest.mark.parametrize("n_atoms,kw,opts", [
     (149, {}, {}), (1415, dict(precision=1), {}),                          # one-launch loop
     (7003, {}, {}), (7003, {}, {"SC_OPT_NEWTON3": 2}),                     # Newton's third law / one-sided, FP64
-    (16391, dict(precision=1), {}), (7003, dict(precision=1), {}),         # mixed: Newton's third law / one-sided
+    (16391, dict(precision=1), {}), (7003, dict(precision=1), {"SC_OPT_NEWTON3": 2}),   # mixed: Newton's third law / one-sided
     (3001, dict(r_cut=8.0, skin=1.0), {}), (3001, dict(r_cut=8.0, skin=1.0, precision=1), {}),
 ])
 def test_poisoned_workspace(scmd, oracle_ld, n_atoms, kw, opts):
