@@ -150,6 +150,37 @@ class Oracle:
                                            int(n_bins), counts.ctypes.data_as(_IP), _dptr(out))
         return counts, int(n_ref), out
 
+    @staticmethod
+    def msd_aligned(pos, ref, r_centre: float = 0.0, align: int = 2):
+        """Mean-square displacement of Eq. (12)'s numerator after the rigid-body fit of
+        PAPER.md:209: "cluster was translated and rotated as a whole in order to minimize the root-mean-square
+        displacement of atoms from a reference structure ... the diffusion coefficient was calculated for all
+        atoms located within 10 A of the cluster center of mass".  Plain numpy in binary64, written out as the
+        definition: centroids (equal masses), the proper rotation that minimises sum_i |R x_i' - y_i'|^2 over
+        ALL atoms (Kabsch: SVD of the 3x3 covariance, det fixed to +1), then the mean of |R x_i' - y_i'|^2 over
+        the atoms whose REFERENCE position lies strictly within r_centre of the reference centroid (DESIGN.md
+        Q20; r_centre <= 0: every atom).  align: 0 none, 1 translation only, 2 translation + rotation.
+        -> (msd in A^2, number of selected atoms, R[3,3]); msd = 0.0 when nothing is selected."""
+        x = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+        y = np.ascontiguousarray(ref, dtype=np.float64).reshape(-1, 3)
+        assert x.shape == y.shape
+        cy = y.mean(axis=0)
+        yc = y - cy
+        if align == 0:
+            xc = x - cy                       # no fit: plain displacement y_i - x_i, selection about the reference centroid
+        else:
+            xc = x - x.mean(axis=0)
+        R = np.eye(3)
+        if align == 2:
+            H = xc.T @ yc                     # H_ab = sum_i x'_ia y'_ib
+            U, _, Vt = np.linalg.svd(H)
+            d = 1.0 if np.linalg.det(Vt.T @ U.T) >= 0.0 else -1.0
+            R = Vt.T @ np.diag([1.0, 1.0, d]) @ U.T
+        disp2 = ((xc @ R.T - yc) ** 2).sum(axis=1)
+        sel = np.ones(len(y), dtype=bool) if not (r_centre > 0.0) else (yc ** 2).sum(axis=1) < r_centre ** 2
+        n_sel = int(sel.sum())
+        return (float(disp2[sel].mean()) if n_sel else 0.0), n_sel, R
+
     def philox4x32_10(self, ctr, key) -> np.ndarray:
         c = np.ascontiguousarray(ctr, dtype=np.uint32); k = np.ascontiguousarray(key, dtype=np.uint32)
         out = np.zeros(4, dtype=np.uint32)
