@@ -34,7 +34,7 @@
  *
  * Stream: every call enqueues on the cudaStream_t given to sc_create and returns without
  * waiting, except the calls that return a host scalar or copy to host memory
- * (sc_energy, sc_kinetic, sc_stats, sc_rdf, sc_eval_host, sc_step_host), which synchronise that stream.
+ * (sc_energy, sc_kinetic, sc_stats, sc_rdf, sc_msd, sc_eval_host, sc_step_host), which synchronise that stream.
  *
  * Errors: every call returns an sc_status; nothing is thrown across the ABI and nothing is
  * printed.  sc_last_error gives a human-readable message for the last failing call on a ctx.
@@ -179,6 +179,33 @@ sc_status sc_stats(sc_ctx *ctx, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, in
  */
 sc_status sc_rdf(sc_ctx *ctx, const double *h_centre, double r_select, double bin_width, int32_t n_bins,
                  int64_t *h_counts, int64_t *h_n_ref, double *h_centre_used);
+
+/*
+ * Mean-square displacement for the diffusion coefficient D = <dr^2> / (2 z dt), Eq. (12)
+ * (PAPER.md:195-199), with the rigid-body fit of PAPER.md:209: "cluster was translated and
+ * rotated as a whole in order to minimize the root-mean-square displacement of atoms from a
+ * reference structure ... the diffusion coefficient was calculated for all atoms located
+ * within 10 A of the cluster center of mass".
+ *   d_ref_pos  DEVICE, [N*3] doubles, the reference structure y_i in the caller's atom order
+ *              (e.g. an earlier sc_get_state); read only, stays the caller's.
+ *   align      0: no fit, displacement x_i - y_i;  1: centroids (equal masses) superposed;
+ *              2: centroids superposed and the proper rotation R (det = +1) that minimises
+ *              sum_i |R x_i' - y_i'|^2 over ALL atoms (x' = x - centroid of x, likewise y').
+ *   r_centre   Angstrom; the average runs over the atoms whose REFERENCE position lies strictly
+ *              within r_centre of the reference centroid (Q20); <= 0: every atom.
+ *   *h_msd     HOST; mean of |R x_i' - y_i'|^2 over the selected atoms in Angstrom^2 (0 if none
+ *              is selected).  D in cm^2/s = 0.1 * msd / (6 * dt_fs) is the caller's arithmetic.
+ *   *h_n_sel   HOST, may be NULL; number of selected atoms.
+ *   h_rot      HOST, may be NULL; R row-major, 9 doubles (identity for align < 2).  Where the
+ *              minimiser is not unique (N = 1, collinear atoms) any minimiser is returned; the
+ *              residual is unique.
+ * All arithmetic in binary64 in either precision mode; works with and without a cutoff;
+ * five small launches, sums in a fixed order (same input -> same bits); synchronises the stream.
+ * SC_ERR_STATE without positions, SC_ERR_INVALID for NULL d_ref_pos / h_msd, align outside
+ * 0..2 or NaN r_centre, SC_ERR_NONFINITE if the reference holds non-finite values.
+ */
+sc_status sc_msd(sc_ctx *ctx, const double *d_ref_pos, double r_centre, int32_t align, double *h_msd,
+                 int64_t *h_n_sel, double *h_rot);
 
 /*
  * Host-buffer entry points (the end-to-end path): copies are part of the call.

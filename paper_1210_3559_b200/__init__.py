@@ -6,7 +6,8 @@ kernels under csrc/.  PyTorch is used for device memory and streams.  There is n
 fallback: if libscmd.so is missing or no CUDA device is present, calls raise.
 """
 from .binding import (  # noqa: F401
-    SC_OK, SC_PREC_FP64, SC_PREC_MIXED, SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN,
+    SC_OK, SC_ERR_INVALID, SC_ERR_CUDA, SC_ERR_NOMEM, SC_ERR_STATE, SC_ERR_NONFINITE, SC_ERR_CAPACITY,
+    SC_PREC_FP64, SC_PREC_MIXED, SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN,
     SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
     SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY, SC_OPT_LANGEVIN_STEP, SC_OPT_CELLS_PER_RADIUS,
     SC_OPT_ATOMS_PER_CTA, SC_OPT_NEWTON3,

@@ -82,6 +82,7 @@ def load_library() -> ctypes.CDLL:
         "sc_eval_host": (i32, [vp, vp, vp, vp, DP]),
         "sc_step_host": (i32, [vp, vp, vp, dbl, TP, i64, DP]),
         "sc_rdf": (i32, [vp, DP, dbl, dbl, i32, IP, IP, DP]),
+        "sc_msd": (i32, [vp, vp, dbl, i32, DP, IP, DP]),
         "sc_launch_count": (i32, [vp, IP]),
         "sc_profile": (i32, [vp, i32]),
         "sc_profile_read": (i32, [vp, DP, DP]),
@@ -252,6 +253,15 @@ class SuttonChen:
                                     counts.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), ctypes.byref(n_ref), used),
                     "sc_rdf")
         return counts, n_ref.value, np.array(list(used))
+
+    def sc_msd(self, ref_pos, r_centre: float = 0.0, align: int = 2):
+        """-> (msd in A^2, n_sel, R[3,3] numpy); ref_pos: device tensor [N,3] float64; see sc_msd in include/scmd.h."""
+        import numpy as np
+        msd, n_sel = ctypes.c_double(), ctypes.c_int64()
+        rot = (ctypes.c_double * 9)()
+        self._check(self.lib.sc_msd(self._ctx, _dev_ptr(ref_pos, 3 * self.n_atoms, "d_ref_pos"), float(r_centre), int(align),
+                                    ctypes.byref(msd), ctypes.byref(n_sel), rot), "sc_msd")
+        return msd.value, n_sel.value, np.array(list(rot)).reshape(3, 3)
 
     def sc_launch_count(self) -> int:
         v = ctypes.c_int64()

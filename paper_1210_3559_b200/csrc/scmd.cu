@@ -57,6 +57,8 @@ struct sc_ctx {
     unsigned long long *rdf_counts = nullptr;   // [kRdfMaxBins + 1] histogram; the last word is the reference-atom count
     int *rdf_refs = nullptr;      // [N] reference atoms of sc_rdf
     double *rdf_meta = nullptr;   // [4] centre
+    double *msd_part = nullptr;   // [3 * kMsdMaxBlocks * kMsdPartStride] per-CTA partials of sc_msd
+    double *msd_meta = nullptr;   // [kMsdMeta] centroids, rotation, totals
     double4 *n3_part = nullptr;   // Newton's-third-law sweeps: triangular reaction partials, row sums (else NULL)
     double4 *n3_self = nullptr;
     double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
@@ -171,10 +173,12 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
     unsigned long long *rc = w.take<unsigned long long>(kRdfMaxBins + 2);
     int *rr = w.take<int>(n);
     double *rm = w.take<double>(4);
+    double *mp = w.take<double>(size_t(3) * kMsdMaxBlocks * kMsdPartStride);
+    double *mm = w.take<double>(kMsdMeta);
     if (c && base) {
         c->xs = xs; c->vel = vel; c->force = force; c->rho = rho; c->part_a = pa; c->part_b = pb;
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
-        c->rdf_counts = rc; c->rdf_refs = rr; c->rdf_meta = rm;
+        c->rdf_counts = rc; c->rdf_refs = rr; c->rdf_meta = rm; c->msd_part = mp; c->msd_meta = mm;
     }
     if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms) {
         double4 *xb = w.take<double4>(n);
@@ -944,6 +948,35 @@ sc_status sc_rdf(sc_ctx *c, const double *h_centre, double r_select, double bin_
     for (int b = 0; b < n_bins; ++b) h_counts[b] = int64_t(host[size_t(b)]);
     if (h_n_ref) *h_n_ref = int64_t(nref_word & 0xffffffffull);
     if (h_centre_used) { h_centre_used[0] = centre[0]; h_centre_used[1] = centre[1]; h_centre_used[2] = centre[2]; }
+    return SC_OK;
+}
+
+sc_status sc_msd(sc_ctx *c, const double *d_ref_pos, double r_centre, int32_t align, double *h_msd, int64_t *h_n_sel,
+                 double *h_rot) {
+    if (!c) return SC_ERR_INVALID;
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_msd: no positions set%s");
+    if (!d_ref_pos || !h_msd || align < 0 || align > 2 || std::isnan(r_centre))
+        return fail(c, SC_ERR_INVALID, "sc_msd: need d_ref_pos, h_msd, align in 0..2, r_centre not NaN%s");
+    const int N = int(c->N);
+    const int nb = int(std::min<int64_t>(ceil_div(c->N, kMsdBlock), kMsdMaxBlocks));
+    const int *perm = c->cutoff ? c->perm : nullptr;
+    double *p0 = c->msd_part, *p1 = p0 + size_t(kMsdMaxBlocks) * kMsdPartStride, *p2 = p1 + size_t(kMsdMaxBlocks) * kMsdPartStride;
+    const double rc2 = r_centre > 0.0 ? r_centre * r_centre : 0.0;
+    msd_centroid_kernel<<<nb, kMsdBlock, 0, c->stream>>>(c->xs, d_ref_pos, perm, N, p0);
+    msd_covariance_kernel<<<nb, kMsdBlock, 0, c->stream>>>(c->xs, d_ref_pos, perm, N, int(align), p0, p1, c->msd_meta);
+    msd_rotation_kernel<<<1, 32, 0, c->stream>>>(p1, nb, int(align), c->msd_meta);
+    msd_accumulate_kernel<<<nb, kMsdBlock, 0, c->stream>>>(c->xs, d_ref_pos, perm, N, rc2, c->msd_meta, p2);
+    msd_total_kernel<<<1, 32, 0, c->stream>>>(p2, nb, c->msd_meta);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 5;
+    double meta[17];
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(meta, c->msd_meta, sizeof(meta), cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    const double cnt = meta[16];
+    *h_msd = cnt > 0.0 ? meta[15] / cnt : 0.0;
+    if (h_n_sel) *h_n_sel = int64_t(cnt);
+    if (h_rot) for (int q = 0; q < 9; ++q) h_rot[q] = meta[6 + q];
+    if (!std::isfinite(meta[15])) return fail(c, SC_ERR_NONFINITE, "sc_msd: the displacement sum is not finite%s");
     return SC_OK;
 }
 

@@ -18,7 +18,7 @@ def test_header_symbols_are_all_exported(lib):
     names = pkg.exported_symbols()
     must = {"sc_create", "sc_destroy", "sc_density", "sc_forces", "sc_energy", "sc_step", "sc_kinetic",
             "sc_set_state", "sc_get_state", "sc_workspace_bytes", "sc_stats", "sc_eval_host", "sc_step_host",
-            "sc_last_error", "sc_set_option", "sc_launch_count", "sc_probe_throughput", "sc_rdf"}
+            "sc_last_error", "sc_set_option", "sc_launch_count", "sc_probe_throughput", "sc_rdf", "sc_msd"}
     assert must <= set(names)
     for name in names:
         assert hasattr(lib, name), f"{name} declared in include/scmd.h but not exported by libscmd.so"
