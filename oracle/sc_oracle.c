@@ -35,6 +35,7 @@
  *            value is r2 = fma(dz, dz, fma(dy, dy, dx*dx)) in binary64 with
  *            dx = x_i - x_j etc. in binary64 -- the one place where the precision of an
  *            intermediate is fixed, because floating point decides a set membership.
+ *   energy-shifted cutoff (cut_shift = 1, reading Q21): see cut_shift_term below.
  *   rho_i == 0 (atom with no neighbour in range, or N = 1): rho^-1/2 := 0, sqrt(rho) := 0
  *            (reading Q9).  Self term excluded by index (Q11).
  *
@@ -82,6 +83,7 @@ typedef struct {
     int32_t n, m;            /* exponents, n > m > 0 */
     double eps, c, a, mass;  /* eV, -, Angstrom, u */
     double r_cut;            /* Angstrom; <= 0 means all pairs (the paper's case) */
+    int32_t cut_shift;       /* with r_cut > 0: 0 plain truncation, 1 energy-shifted terms (reading Q21) */
 } oracle_params;
 
 static real ipow(real u, int k) {
@@ -98,6 +100,15 @@ static int pair_in_range(const double *pi, const double *pj, double r_cut) {
     return r2 < r_cut * r_cut;
 }
 
+/* Energy-shifted cutoff (reading Q21; not in the paper): inside the cutoff each pair term loses
+ * its value at the cutoff, (a/r)^k -> (a/r)^k - (a/r_cut)^k for k = n in Eq. (1) and k = m in Eq. (2), so that
+ * U is continuous when a pair crosses r_cut.  Constants drop out of the gradient: the force keeps its form, with
+ * rho_i the shifted density.  Returns the constant to subtract (0 without a cutoff or with cut_shift = 0). */
+static real cut_shift_term(const oracle_params *p, int k) {
+    if (!(p->r_cut > 0.0) || !p->cut_shift) return (real)0;
+    return ipow((real)p->a / (real)p->r_cut, k);
+}
+
 static real pair_distance(const double *pi, const double *pj, real *d) {
     d[0] = (real)pi[0] - (real)pj[0];
     d[1] = (real)pi[1] - (real)pj[1];
@@ -110,13 +121,14 @@ static void density_real(int64_t N, const double *pos, const oracle_params *p, r
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t i = 0; i < N; ++i) {
         real acc = 0;
+        const real shift = cut_shift_term(p, p->m);
         for (int64_t j = 0; j < N; ++j) {
             if (j == i) continue;
             if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
             real d[3];
             real r = pair_distance(pos + 3 * i, pos + 3 * j, d);
             real u = (real)p->a / r;
-            acc += ipow(u, p->m);
+            acc += ipow(u, p->m) - shift;
         }
         rho[i] = acc;
     }
@@ -129,6 +141,7 @@ static void force_row(int64_t N, const double *pos, const oracle_params *p, cons
                       int64_t i, real f[3], real *pair_sum) {
     real fx = 0, fy = 0, fz = 0, ps = 0;
     const real half_cm = (real)p->c * (real)p->m / 2;
+    const real shift = cut_shift_term(p, p->n);
     for (int64_t j = 0; j < N; ++j) {
         if (j == i) continue;
         if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
@@ -142,7 +155,7 @@ static void force_row(int64_t N, const double *pos, const oracle_params *p, cons
         fx += g * d[0];
         fy += g * d[1];
         fz += g * d[2];
-        ps += un;
+        ps += un - shift;
     }
     f[0] = fx; f[1] = fy; f[2] = fz;
     *pair_sum = ps;
@@ -278,7 +291,7 @@ int oracle_density_rows(int64_t N, const double *pos, const oracle_params *p,
             if (!pair_in_range(pos + 3 * i, pos + 3 * j, p->r_cut)) continue;
             real d[3];
             real r = pair_distance(pos + 3 * i, pos + 3 * j, d);
-            acc += ipow((real)p->a / r, p->m);
+            acc += ipow((real)p->a / r, p->m) - cut_shift_term(p, p->m);
         }
         rho_out[k] = (double)acc;
     }

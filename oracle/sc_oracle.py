@@ -28,7 +28,7 @@ _VARIANTS = {
 class OracleParams(ctypes.Structure):
     _fields_ = [("n", ctypes.c_int32), ("m", ctypes.c_int32),
                 ("eps", ctypes.c_double), ("c", ctypes.c_double), ("a", ctypes.c_double),
-                ("mass", ctypes.c_double), ("r_cut", ctypes.c_double)]
+                ("mass", ctypes.c_double), ("r_cut", ctypes.c_double), ("cut_shift", ctypes.c_int32)]
 
 
 def build(force: bool = False) -> None:
@@ -79,8 +79,8 @@ class Oracle:
         L.oracle_langevin_normals.restype = None
 
     @staticmethod
-    def params(n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0) -> OracleParams:
-        return OracleParams(int(n), int(m), float(eps), float(c), float(a), float(mass), float(r_cut))
+    def params(n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0, cut_shift=0) -> OracleParams:
+        return OracleParams(int(n), int(m), float(eps), float(c), float(a), float(mass), float(r_cut), int(cut_shift))
 
     @staticmethod
     def _pos(pos) -> np.ndarray:
