@@ -116,11 +116,18 @@ typedef enum {
                                      takes effect at the next list build                         */
     SC_OPT_ATOMS_PER_CTA = 9,     /* cutoff path: consecutive atoms one CTA of the list sweeps
                                      works through (rounded to the warp layout)                  */
-    SC_OPT_NEWTON3 = 10           /* all pairs, either precision, 7000 <= N <= 262144 (the range in which
+    SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 7000 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
                                      both atoms.  0: library default (on), 1: on,
                                      2: off = the one-sided sweeps                               */
+    SC_OPT_CUTOFF_SHIFT = 11      /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
+                                     configs; 1 energy-shifted terms: inside r_cut every pair term
+                                     loses its value at the cutoff, (a/r)^k -> (a/r)^k - (a/r_cut)^k
+                                     for k = n in Eq. (1) and k = m in Eq. (2), so U is continuous
+                                     when a pair crosses r_cut and NVE runs keep their energy; the
+                                     force keeps its form, with rho_i the shifted density (DESIGN.md
+                                     Q21).  Ignored without a cutoff.                            */
 } sc_option;
 
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */

@@ -429,6 +429,7 @@ struct NlistArgs {
     double *partial;          // [gridDim.x]
     unsigned long long *pairs_in_cut;   // sweep 1: += ordered pairs with r^2 < r_c^2 (zeroed by the host)
     double rc2;
+    double shift_m;           // energy-shifted cutoff (SC_OPT_CUTOFF_SHIFT): r_c^-m, taken off every in-range term of sweep 1; else 0
     PairConsts c;
 };
 
@@ -581,7 +582,7 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
         const int *row = a.nlist + size_t(live ? gp : 0) * stride + q;
         double acc0[4] = {0.0, 0.0, 0.0, 0.0}, acc1[4] = {0.0, 0.0, 0.0, 0.0};
         float f0[4] = {0.f, 0.f, 0.f, 0.f}, f1[4] = {0.f, 0.f, 0.f, 0.f};
-        int np_row = 0;
+        int np0 = 0, np1 = 0;                            // sweep 1: in-range entries of each atom of the pair
         bool unsure = false;
 
         auto entry = [&](int j, const double4 &p) {
@@ -591,11 +592,11 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 const RecF &fp = reinterpret_cast<const RecF &>(p);
                 const PairGeomF ga = nlist_geom_f(fa, fp), gb = nlist_geom_f(fb, fp);
                 unsure = unsure || fabsf(ga.q2 - rc2f) <= band || fabsf(gb.q2 - rc2f) <= band;
-                nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, ga, ga.q2 < rc2f && j != i0, Anf, n_exp, m_exp, f0, np_row);
-                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, np_row);
+                nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, ga, ga.q2 < rc2f && j != i0, Anf, n_exp, m_exp, f0, np0);
+                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, np1);
             } else {
-                nlist_term<NE, ME, FORCE, ENERGY>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, np_row);
-                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, np_row);
+                nlist_term<NE, ME, FORCE, ENERGY>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, np0);
+                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, np1);
             }
         };
         auto flush = [&]() {
@@ -643,7 +644,7 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 // as the FP64 path takes it (reading Q7: set membership is the oracle's).
 #pragma unroll
                 for (int c = 0; c < 4; ++c) { acc0[c] = 0.0; acc1[c] = 0.0; f0[c] = 0.f; f1[c] = 0.f; }
-                np_row = 0;
+                np0 = 0; np1 = 0;
                 const RecF &fa = reinterpret_cast<const RecF &>(pa), &fb = reinterpret_cast<const RecF &>(pb);
                 for (int it = 0; it < niter; ++it) {
                     const int j = row[it * LPA];
@@ -651,14 +652,22 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                     const RecF &fp = reinterpret_cast<const RecF &>(p);
                     const bool in0 = j != i0 && nlist_exact_in_range(a.xs, i0, j, rc2);
                     const bool in1 = j != i1 && nlist_exact_in_range(a.xs, i1, j, rc2);
-                    nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, nlist_geom_f(fa, fp), in0, Anf, n_exp, m_exp, f0, np_row);
-                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, np_row);
+                    nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, nlist_geom_f(fa, fp), in0, Anf, n_exp, m_exp, f0, np0);
+                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, np1);
                     if ((it & 3) == 3) flush();                  // same flush points as the fast loop
                 }
                 flush();
             }
         }
-        npairs += np_row;
+        npairs += np0 + np1;
+        if constexpr (!FORCE) {
+            // per-atom neighbour counts over the LPA lanes (integers: exact), for the shifted density
+#pragma unroll
+            for (int off = LPA / 2; off > 0; off >>= 1) {
+                np0 += __shfl_xor_sync(0xffffffffu, np0, off);
+                np1 += __shfl_xor_sync(0xffffffffu, np1, off);
+            }
+        }
 
         // ---- reduce over the LPA lanes of the pair (fixed order) ----
         constexpr int NV = FORCE ? (ENERGY ? 4 : 3) : 1;
@@ -671,7 +680,8 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 const double *acc = h ? acc1 : acc0;
                 if (i >= N) continue;
                 if constexpr (!FORCE) {
-                    const double rho = a.c.am * acc[0];
+                    // shifted cutoff: every in-range term loses r_c^-m (shift_m = 0 otherwise: exact no-op)
+                    const double rho = a.c.am * fma(-double(h ? np1 : np0), a.shift_m, acc[0]);
                     a.rho[i] = rho;
                     const double root = rho > 0.0 ? sqrt(rho) : 0.0;       // reading Q9
                     const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;

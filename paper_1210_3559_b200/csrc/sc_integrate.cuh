@@ -176,6 +176,17 @@ __global__ void reduce_partials_kernel(const double *__restrict__ part, int n, d
     if (threadIdx.x == 0) scal[slot] = scale * t;
 }
 
+// the same with a count-proportional constant taken off the sum first (energy-shifted cutoff: every in-range ordered
+// pair loses r_c^-n; the count is the one sweep 1 left for the same positions): scal[slot] = scale * (sum - shift * count)
+__global__ void reduce_partials_shift_kernel(const double *__restrict__ part, int n, double *__restrict__ scal, int slot,
+                                             double scale, const unsigned long long *__restrict__ count, double shift) {
+    __shared__ double scratch[32];
+    double v = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) v += part[k];
+    const double t = block_sum(v, scratch);
+    if (threadIdx.x == 0) scal[slot] = scale * fma(-double(*count), shift, t);
+}
+
 // one block: KE and T from the per-block |v|^2 sums; optionally the rescale factor for T_target
 //   KE = 1/2 m sum|v|^2 / ACC ;  T = 2 KE / (kB ndof) ;  lambda = sqrt(T_target / T)
 // After a rescale the stored KE and T are those of the rescaled velocities.

@@ -101,7 +101,7 @@ struct sc_ctx {
     std::vector<OccEntry> occ_cache;
 
     // options (0 = default)
-    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0;
+    int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0, opt_shift = 0;
 
     // profiling
     bool profile = false;
@@ -355,6 +355,7 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
     a.pairs_in_cut = c->counters + kCntPairsInCut;
     a.rc2 = c->p.r_cut * c->p.r_cut;
+    a.shift_m = c->opt_shift ? ipow_host(1.0 / c->p.r_cut, c->p.m) : 0.0;
     a.c = c->consts;
     if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
@@ -364,8 +365,13 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     c->launches += 1;
     if (!force || energy) {
         const int grid = ceil_div((c->N + 1) / 2, a.pairs_per_cta);
-        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
-                                                         force ? c->consts.En : -c->consts.eps_c);
+        if (force && c->opt_shift)
+            reduce_partials_shift_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, kSlotEPair, c->consts.En,
+                                                                   c->counters + kCntPairsInCut,
+                                                                   ipow_host(1.0 / c->p.r_cut, c->p.n));
+        else
+            reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
+                                                             force ? c->consts.En : -c->consts.eps_c);
         SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
     }
@@ -777,6 +783,11 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
         case SC_OPT_NEWTON3:
             if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "Newton's third law must be 0, 1 or 2%s");
             c->opt_n3 = int(value);
+            c->density_valid = c->forces_valid = c->energy_valid = false;
+            break;
+        case SC_OPT_CUTOFF_SHIFT:
+            if (value < 0 || value > 1) return fail(c, SC_ERR_INVALID, "cutoff shift must be 0 or 1%s");
+            c->opt_shift = int(value);
             c->density_valid = c->forces_valid = c->energy_valid = false;
             break;
         case SC_OPT_ATOMS_PER_CTA:
