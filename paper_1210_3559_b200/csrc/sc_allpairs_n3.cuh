@@ -406,26 +406,33 @@ struct N3FinalArgs {
     const double4 *part;
     const double *part_rho;
     const double4 *self;
-    double *rho, *force, *partial;      // partial: [gridDim.x] sum sqrt(rho) (density)
+    double *rho, *force, *partial;      // partial: [gridDim.x = ceil(N / 32)] sum sqrt(rho) (density)
     int n_atoms, n_pad, rb, seg_chunks;
     PairConsts c;
 };
 
+constexpr int kN3FinAtoms = 32;         // atoms per CTA of the finalize kernel: one per lane
+constexpr int kN3FinWarps = 8;          // its warps share the segments and the row blocks of those atoms
+
 #ifdef SCMD_MAIN_TU
+// A CTA takes 32 consecutive atoms (one per lane: every load is a contiguous 256 B or 1 KB line run); warp w sums the
+// segments sg = w, w + 8, ... and the row blocks b = w, w + 8, ... <= block(i), then the 8 sums are added in warp order.
+// (One thread per atom walking all blocks left 32 CTAs on 148 SMs at N = 8000: 21 us for the force variant.)
 template <bool FORCE>
-__global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
-    __shared__ double scratch[32];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double contrib = 0.0;
+__global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3FinalArgs a) {
+    __shared__ double red[kN3FinWarps][3][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int i = blockIdx.x * kN3FinAtoms + lane;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
     if (i < a.n_atoms) {
         const int bi = i / a.rb;
         const int nseg = (((a.n_atoms + 31) >> 5) - ((bi * a.rb) >> 5) + a.seg_chunks - 1) / a.seg_chunks;
-        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        for (int sg = 0; sg < nseg; ++sg) {                 // row sums of the segments of i's own block
+        for (int sg = w; sg < nseg; sg += kN3FinWarps) {    // row sums of the segments of i's own block
             const double4 s = a.self[size_t(sg) * a.n_pad + i];
             v0 += s.x; v1 += s.y; v2 += s.z;
         }
-        for (int b = 0; b <= bi; ++b) {
+#pragma unroll 4
+        for (int b = w; b <= bi; b += kN3FinWarps) {
             const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(i - b * a.rb);
             if constexpr (FORCE) {
                 const double4 p = a.part[at];
@@ -434,6 +441,19 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
                 v0 += a.part_rho[at];
             }
         }
+    }
+    red[w][0][lane] = v0;
+    if constexpr (FORCE) { red[w][1][lane] = v1; red[w][2][lane] = v2; }
+    __syncthreads();
+    if (w != 0) return;
+    v0 = 0.0; v1 = 0.0; v2 = 0.0;
+#pragma unroll
+    for (int k = 0; k < kN3FinWarps; ++k) {
+        v0 += red[k][0][lane];
+        if constexpr (FORCE) { v1 += red[k][1][lane]; v2 += red[k][2][lane]; }
+    }
+    double contrib = 0.0;
+    if (i < a.n_atoms) {
         if constexpr (FORCE) {
             a.force[3 * size_t(i)] = v0; a.force[3 * size_t(i) + 1] = v1; a.force[3 * size_t(i) + 2] = v2;
         } else {
@@ -448,8 +468,8 @@ __global__ void __launch_bounds__(256) n3_finalize_kernel(const N3FinalArgs a) {
         }
     }
     if constexpr (!FORCE) {
-        const double t = block_sum(contrib, scratch);
-        if (threadIdx.x == 0) a.partial[blockIdx.x] = t;
+        const double t = warp_sum(contrib);
+        if (lane == 0) a.partial[blockIdx.x] = t;
     }
 }
 #endif  // SCMD_MAIN_TU

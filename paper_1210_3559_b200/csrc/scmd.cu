@@ -415,9 +415,9 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     N3FinalArgs f{};
     f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
     f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.seg_chunks = seg; f.c = c->consts;
-    const int fb = ceil_div(N, 256);
-    if (force) n3_finalize_kernel<true><<<fb, 256, 0, c->stream>>>(f);
-    else n3_finalize_kernel<false><<<fb, 256, 0, c->stream>>>(f);
+    const int fb = ceil_div(N, kN3FinAtoms);
+    if (force) n3_finalize_kernel<true><<<fb, kN3FinWarps * 32, 0, c->stream>>>(f);
+    else n3_finalize_kernel<false><<<fb, kN3FinWarps * 32, 0, c->stream>>>(f);
     c->launches += 2;
     if (!force) {
         reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, fb, c->scal, kSlotEEmb, -c->consts.eps_c);
