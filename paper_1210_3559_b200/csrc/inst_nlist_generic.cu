@@ -12,11 +12,13 @@ cudaError_t launch(int block, const NlistArgs &a, bool force, bool energy, bool 
         return cudaGetLastError();
     };
     if (!mixed) {
-        if (!force) return go(nlist_kernel<LPA, 0, 0, false, false, false>);
+        if (!force) return a.shift_m != 0.0 ? go(nlist_kernel<LPA, 0, 0, false, false, false, true>)
+                                          : go(nlist_kernel<LPA, 0, 0, false, false, false>);
         if (energy) return go(nlist_kernel<LPA, 0, 0, true, true, false>);
         return go(nlist_kernel<LPA, 0, 0, true, false, false>);
     }
-    if (!force) return go(nlist_kernel<LPA, 0, 0, false, false, true>);
+    if (!force) return a.shift_m != 0.0 ? go(nlist_kernel<LPA, 0, 0, false, false, true, true>)
+                                          : go(nlist_kernel<LPA, 0, 0, false, false, true>);
     if (energy) return go(nlist_kernel<LPA, 0, 0, true, true, true>);
     return go(nlist_kernel<LPA, 0, 0, true, false, true>);
 }

@@ -553,7 +553,9 @@ __device__ __forceinline__ void nlist_term_f(const RecF &pi, const RecF &p, Pair
 // LPA lanes per atom PAIR (32 / LPA pairs per warp at a time).  A CTA works through pairs_per_cta
 // consecutive pairs of the internal (cell) order, its warps interleaved, so that the records its
 // gathers touch stay in L1.  Every fetched record serves both atoms of the pair.
-template <int LPA, int NE, int ME, bool FORCE, bool ENERGY, bool MIXED>
+// SHIFT (sweep 1 only): energy-shifted cutoff -- the in-range entries are counted per atom and the epilogue takes
+// count * r_c^-m off the sum (a separate instantiation: the per-atom counters cost the plain sweep 5 %).
+template <int LPA, int NE, int ME, bool FORCE, bool ENERGY, bool MIXED, bool SHIFT = false>
 __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a) {
     constexpr int AW = 32 / LPA;                         // pairs per warp
     __shared__ double scratch[32];
@@ -582,7 +584,7 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
         const int *row = a.nlist + size_t(live ? gp : 0) * stride + q;
         double acc0[4] = {0.0, 0.0, 0.0, 0.0}, acc1[4] = {0.0, 0.0, 0.0, 0.0};
         float f0[4] = {0.f, 0.f, 0.f, 0.f}, f1[4] = {0.f, 0.f, 0.f, 0.f};
-        int np0 = 0, np1 = 0;                            // sweep 1: in-range entries of each atom of the pair
+        int np0 = 0, np1 = 0;                            // sweep 1: in-range entries (SHIFT: of each atom of the pair)
         bool unsure = false;
 
         auto entry = [&](int j, const double4 &p) {
@@ -593,10 +595,10 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 const PairGeomF ga = nlist_geom_f(fa, fp), gb = nlist_geom_f(fb, fp);
                 unsure = unsure || fabsf(ga.q2 - rc2f) <= band || fabsf(gb.q2 - rc2f) <= band;
                 nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, ga, ga.q2 < rc2f && j != i0, Anf, n_exp, m_exp, f0, np0);
-                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, np1);
+                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
             } else {
                 nlist_term<NE, ME, FORCE, ENERGY>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, np0);
-                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, np1);
+                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, SHIFT ? np1 : np0);
             }
         };
         auto flush = [&]() {
@@ -653,14 +655,14 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                     const bool in0 = j != i0 && nlist_exact_in_range(a.xs, i0, j, rc2);
                     const bool in1 = j != i1 && nlist_exact_in_range(a.xs, i1, j, rc2);
                     nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, nlist_geom_f(fa, fp), in0, Anf, n_exp, m_exp, f0, np0);
-                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, np1);
+                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
                     if ((it & 3) == 3) flush();                  // same flush points as the fast loop
                 }
                 flush();
             }
         }
         npairs += np0 + np1;
-        if constexpr (!FORCE) {
+        if constexpr (!FORCE && SHIFT) {
             // per-atom neighbour counts over the LPA lanes (integers: exact), for the shifted density
 #pragma unroll
             for (int off = LPA / 2; off > 0; off >>= 1) {
@@ -680,8 +682,8 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 const double *acc = h ? acc1 : acc0;
                 if (i >= N) continue;
                 if constexpr (!FORCE) {
-                    // shifted cutoff: every in-range term loses r_c^-m (shift_m = 0 otherwise: exact no-op)
-                    const double rho = a.c.am * fma(-double(h ? np1 : np0), a.shift_m, acc[0]);
+                    // shifted cutoff: every in-range term loses r_c^-m
+                    const double rho = SHIFT ? a.c.am * fma(-double(h ? np1 : np0), a.shift_m, acc[0]) : a.c.am * acc[0];
                     a.rho[i] = rho;
                     const double root = rho > 0.0 ? sqrt(rho) : 0.0;       // reading Q9
                     const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;
