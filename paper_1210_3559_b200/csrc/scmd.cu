@@ -6,7 +6,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
+#include <functional>
 #include <new>
+#include <queue>
 #include <vector>
 
 #define SCMD_MAIN_TU 1   // this translation unit compiles the non-template kernels
@@ -102,6 +105,7 @@ struct sc_ctx {
 
     // options (0 = default)
     int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0, opt_shift = 0;
+    int n3_seg = 0;               // j-segment length of the Newton's-third-law sweeps (chunks of 32), chosen at first use
 
     // profiling
     bool profile = false;
@@ -154,7 +158,7 @@ int cutoff_max_dim(int64_t N) {
 constexpr int64_t kN3MinAtoms = 7000, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
 constexpr int64_t kN3DefaultMinAtoms = 7000, kN3DefaultMinAtomsMixed = 7000;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
-constexpr int kN3MaxSegments = 17;                             // j segments of the longest row block
+constexpr int kN3MaxSegments = 25;                             // j segments of the longest row block
 
 // one place that lays the workspace out; base == nullptr only measures
 size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin) {
@@ -389,6 +393,40 @@ sc_status check_flags(sc_ctx *c) {
     return SC_OK;
 }
 
+// Segment length of the Newton's-third-law sweeps, in chunks of 32 atoms.  Their CTAs (row block x j segment; one CTA
+// per SM at 168 registers x 384 threads) are handed to the SMs in launch order as SMs fall free, so the sweep lasts as
+// long as the busiest SM of that greedy schedule: with a few hundred CTAs on 148 SMs a badly filled last wave costs
+// 10 % (measured at N = 8000 ... 24576, where the best of 8 / 12 / 16 / 24 segments changes with N in no simple way).
+// The schedule is simulated for each candidate -- a CTA costs one unit of prologue / epilogue plus one per round of its
+// 12 warps over the segment's chunks (mixed: chunks of 64) -- and the shortest makespan wins.  Against measurement the
+// simulation picked the fastest candidate at 6 of 8 sizes between 7000 and 32768 and was within 1 % / 6 % at the others.
+int choose_n3_segment(const sc_ctx *c) {
+    const int N = int(c->N), nch = ceil_div(N, 32), nb = ceil_div(N, 32 * kN3RowsPerThread);
+    const int unit = c->precision == SC_PREC_MIXED ? 2 : 1;
+    int best_seg = 0, last_seg = 0;
+    double best_t = 0.0;
+    for (int want : {8, 12, 16, 20, 24}) {
+        const int seg = round_up(ceil_div(nch, want), kN3Warps * unit), nseg = ceil_div(nch, seg);
+        if (nseg > kN3MaxSegments || seg == last_seg) continue;
+        last_seg = seg;
+        std::priority_queue<double, std::vector<double>, std::greater<double>> sm;
+        for (int k = 0; k < c->sm_count; ++k) sm.push(0.0);
+        double makespan = 0.0;
+        for (int y = 0; y < nseg; ++y)
+            for (int b = 0; b < nb; ++b) {
+                const int c_begin = b * kN3RowsPerThread + y * seg;
+                if (c_begin >= nch) continue;
+                const int chunks = ceil_div(std::min(nch, c_begin + seg) - c_begin, unit);
+                const double t = sm.top() + 1.0 + double(ceil_div(chunks, kN3Warps));
+                sm.pop();
+                sm.push(t);
+                makespan = std::max(makespan, t);
+            }
+        if (!best_seg || makespan < best_t) { best_seg = seg; best_t = makespan; }
+    }
+    return best_seg;
+}
+
 // all pairs, every unordered pair once (sc_allpairs_n3.cuh): sweep + finalize + scalar reduction
 sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
@@ -404,9 +442,9 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     a.partial = c->part_b; a.c = c->consts;
     N3FArgs af{};
     af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
-    // j segments: 8 (N >= 24576) or 12 of them cut the first row block's triangle; a multiple of the 12 warps each
-    const int nch = ceil_div(N, 32), want = N >= 24576 ? 8 : 12;             // measured: flat between 8 and 16
-    const int seg = round_up(ceil_div(nch, want), kN3Warps), nseg = ceil_div(nch, seg);
+    // j segments cut the first row block's triangle; each a multiple of the 12 warps (choose_n3_segment)
+    if (!c->n3_seg) c->n3_seg = choose_n3_segment(c);
+    const int nch = ceil_div(N, 32), seg = c->n3_seg, nseg = ceil_div(nch, seg);
     a.seg_chunks = seg;
     af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
     void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
