@@ -398,11 +398,13 @@ sc_status check_flags(sc_ctx *c) {
 // long as the busiest SM of that greedy schedule: with a few hundred CTAs on 148 SMs a badly filled last wave costs
 // 10 % (measured at N = 8000 ... 24576, where the best of 8 / 12 / 16 / 24 segments changes with N in no simple way).
 // The schedule is simulated for each candidate -- a CTA costs one unit of prologue / epilogue plus one per round of its
-// 12 warps over the segment's chunks (mixed: chunks of 64) -- and the shortest makespan wins.  Against measurement the
-// simulation picked the fastest candidate at 6 of 8 sizes between 7000 and 32768 and was within 1 % / 6 % at the others.
+// 12 warps over the segment's chunks (mixed: chunks of 64, and a quarter unit of fixed cost: calibrated) -- and the
+// shortest makespan wins.  Against measurement the simulation picked the fastest candidate at 6 (FP64) and 5 (mixed)
+// of 8 sizes between 7000 and 32768 and was within 1 - 6 % at the others; above 49152 the choice is flat within 1 %.
 int choose_n3_segment(const sc_ctx *c) {
     const int N = int(c->N), nch = ceil_div(N, 32), nb = ceil_div(N, 32 * kN3RowsPerThread);
     const int unit = c->precision == SC_PREC_MIXED ? 2 : 1;
+    const double fixed = c->precision == SC_PREC_MIXED ? 0.25 : 1.0;
     int best_seg = 0, last_seg = 0;
     double best_t = 0.0;
     for (int want : {8, 12, 16, 20, 24}) {
@@ -417,7 +419,7 @@ int choose_n3_segment(const sc_ctx *c) {
                 const int c_begin = b * kN3RowsPerThread + y * seg;
                 if (c_begin >= nch) continue;
                 const int chunks = ceil_div(std::min(nch, c_begin + seg) - c_begin, unit);
-                const double t = sm.top() + 1.0 + double(ceil_div(chunks, kN3Warps));
+                const double t = sm.top() + fixed + double(ceil_div(chunks, kN3Warps));
                 sm.pop();
                 sm.push(t);
                 makespan = std::max(makespan, t);
