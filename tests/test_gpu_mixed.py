@@ -94,7 +94,8 @@ def test_generic_exponents_mixed(scmd, oracle_ld, n, m):
     check_eval(scmd, oracle_ld, w.pos, n=n, m=m, eps=0.02, c=30.0, a=3.3, energy_tol=2e-7)
 
 
-@pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3))])
+@pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3)),
+                                        (13400, {})])            # 13400: the segment chooser takes 18 j segments
 def test_newton3_sweeps_mixed(scmd, oracle_ld, n_atoms, kw):
     """The Newton's-third-law sweeps in mixed precision (binary32 rotation on split records, binary64 sums):
     BASELINE.json's mixed tolerances, and agreement with the one-sided mixed sweeps."""
