@@ -82,27 +82,50 @@ def test_degenerate_inputs(scmd, oracle_ld):
 
 
 @pytest.mark.parametrize("mixed", [False, True])
-def test_after_md_steps_on_both_paths(scmd, oracle_ld, mixed):
-    """The reference is an earlier sc_get_state; after MD steps the device msd equals the oracle's on the
-    device's own positions -- all pairs (internal order = caller's) and the list path (atoms are re-sorted
-    by cell at every rebuild: the reference is matched through the permutation)."""
+def test_list_path_matches_the_reference_through_the_cell_sort(scmd, oracle_ld, mixed):
+    """On the list path the resident records are re-sorted by cell at every build; the reference stays in the
+    caller's order and is matched through the permutation.  Two builds with different sorts (state A, then a
+    displaced and rotated state B), msd of B against A -- both synthetic, the oracle sees the same arrays."""
     import torch
-    w = W.fcc_cluster(4000, 1500.0, seed=77)
+    rng = np.random.default_rng(55)
     prec = dict(precision=scmd.SC_PREC_MIXED) if mixed else {}
+    a = W.fcc_cluster(4000, 300.0, seed=77).pos
+    b = (a + rng.normal(scale=0.4, size=a.shape)) @ rotation(rng).T + np.array([3.0, 1.0, -2.0])
     for kw in (dict(), dict(r_cut=7.0, skin=0.6)):
-        sc = scmd.SuttonChen(w.n_atoms, **kw, **prec)
-        sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"), torch.as_tensor(w.vel, device="cuda"))
-        ref, _ = sc.sc_get_state(want_vel=False)
-        assert sc.sc_msd(ref, 0.0, 0)[0] == 0.0
-        sc.sc_step(2.0, 150)
+        sc = scmd.SuttonChen(len(a), **kw, **prec)
+        d_a = torch.as_tensor(a, device="cuda")
+        sc.sc_set_state(d_a, None)
+        sc.sc_forces()                                            # first build: sorted by the cells of A
+        assert sc.sc_msd(d_a, 0.0, 0)[0] == 0.0
+        sc.sc_set_state(torch.as_tensor(b, device="cuda"), None)
+        sc.sc_forces()                                            # second build: the cells of B
         if kw:
-            assert sc.sc_stats()["n_rebuilds"] >= 2                        # at least one re-sort since the reference
-        cur, _ = sc.sc_get_state(want_vel=False)
+            assert sc.sc_stats()["n_rebuilds"] == 2
         for align, rc in ((0, 0.0), (1, 10.0), (2, 10.0), (2, 0.0)):
-            m, cnt, R = sc.sc_msd(ref, rc, align)
-            mo, cnto, Ro = oracle_ld.msd_aligned(cur.cpu().numpy(), ref.cpu().numpy(), rc, align)
+            m, cnt, R = sc.sc_msd(d_a, rc, align)
+            mo, cnto, Ro = oracle_ld.msd_aligned(b, a, rc, align)
             assert cnt == cnto and abs(m - mo) <= 1e-11 * mo and np.abs(R - Ro).max() < 1e-12
-            assert 0.01 < m < 1.0                                 # 300 fs of thermal motion at 1500 K
+        sc.close()
+
+
+def test_after_md_steps(scmd, oracle_ld):
+    """The reference is the initial structure; after 100 NVE steps the device msd of the device trajectory equals
+    the oracle's msd of the ORACLE's trajectory (the two agree to 1e-8 A, i.e. to ~1e-7 of an msd of 0.05 A^2),
+    through the multi-launch path, the list path (with re-sorts) and the one-launch loop."""
+    import torch
+    w = W.fcc_cluster(900, 1500.0, seed=78)
+    for kw, persistent in ((dict(), 1), (dict(), 2), (dict(r_cut=6.5, skin=0.4), 0)):
+        ref = oracle_ld.run(w.pos, w.vel, oracle_ld.params(r_cut=kw.get("r_cut", 0.0)), dt=1.0, nsteps=100)
+        sc = scmd.SuttonChen(w.n_atoms, **kw)
+        sc.sc_set_option(scmd.SC_OPT_PERSISTENT, persistent)
+        d0 = torch.as_tensor(w.pos, device="cuda")
+        sc.sc_set_state(d0, torch.as_tensor(w.vel, device="cuda"))
+        sc.sc_step(1.0, 100)
+        for align, rc in ((0, 0.0), (2, 10.0), (2, 0.0)):
+            m, cnt, _ = sc.sc_msd(d0, rc, align)
+            mo, cnto, _ = oracle_ld.msd_aligned(ref["pos"], w.pos, rc, align)
+            assert cnt == cnto and abs(m - mo) <= 1e-6 * mo
+            assert 0.005 < m < 1.0                                # 100 fs of thermal motion
         sc.close()
 
 

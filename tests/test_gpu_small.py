@@ -98,7 +98,7 @@ def test_rescale_ramp_across_paths(scmd, oracle_ld):
 @pytest.mark.parametrize("n_atoms", [2, 147, 1415, 4100])
 def test_mixed_precision_in_one_launch(scmd, oracle_ld, n_atoms):
     """Mixed path (binary32 pair arithmetic on split coordinates): forces / energy left by the loop within
-    BASELINE.json's mixed tolerances of the oracle at the oracle's positions after a few steps, trajectory
+    BASELINE.json's mixed tolerances of the oracle at the oracle's own positions after a few steps, trajectory
     within 1e-5 A over 100 steps at N = 1415 (as the multi-launch mixed path), and the packed records of the
     multi-launch sweeps are refreshed (a forced re-evaluation agrees)."""
     w = W.config_c2() if n_atoms == 1415 else W.fcc_cluster(n_atoms, 1200.0, seed=900 + n_atoms)
@@ -112,17 +112,19 @@ def test_mixed_precision_in_one_launch(scmd, oracle_ld, n_atoms):
     assert sc.sc_launch_count() - before == 1
     pos, vel = state(sc)
     assert np.abs(pos - ref["pos"]).max() < 1e-5
-    rho_o, f_o, (e_o, _, _) = oracle_ld.energy_forces(pos, P)               # at the GPU's own final positions
+    # forces / energy left by the loop against the oracle at the ORACLE's final positions (the two trajectories are
+    # within 1e-5 A, which moves a force by < 1e-6 of its size: inside the mixed tolerance)
+    rho_o, f_o, (e_o, _, _) = oracle_ld.energy_forces(ref["pos"], P)
     f = sc.sc_forces().cpu().numpy()
     assert np.linalg.norm(f - f_o) <= 1e-5 * np.linalg.norm(f_o)
     assert abs(sc.sc_energy() - e_o) <= 1e-7 * abs(e_o)
-    # multi-launch sweeps from the refreshed records: same state, forced re-evaluation
-    import torch
+    # multi-launch sweeps from the refreshed records: one more step there = one more oracle step (stale records
+    # would be off by the ~0.05 A the atoms moved inside the loop)
     sc.sc_set_option(scmd.SC_OPT_PERSISTENT, 2)
     sc.sc_step(1.0, 1)
-    ref2 = oracle_ld.run(pos, vel, P, dt=1.0, nsteps=1)
+    ref2 = oracle_ld.run(ref["pos"], ref["vel"], P, dt=1.0, nsteps=1)
     pos2, _ = state(sc)
-    assert np.abs(pos2 - ref2["pos"]).max() < 1e-7
+    assert np.abs(pos2 - ref2["pos"]).max() < 1e-5
     sc.close()
 
 
