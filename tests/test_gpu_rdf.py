@@ -45,19 +45,23 @@ def test_explicit_centre_bit_exact(scmd, oracle_ld, n_atoms, r_select, width, n_
         assert n_ref == 2607
 
 
-def test_after_steps_with_cutoff_and_mixed(scmd, oracle_ld):
-    """The histogram works on the current positions whatever the internal atom order (cutoff path) and
-    precision mode: compare at the positions the library returns."""
-    w = W.fcc_cluster(3000, 1500.0, seed=9)
-    for kw in (dict(r_cut=8.0, skin=1.0), dict(precision=1), dict()):
-        sc = ctx(scmd, w.pos, w.vel, **kw)
-        sc.sc_step(1.0, 25)
-        pos, _ = sc.sc_get_state()
-        pos = pos.cpu().numpy()
-        centre = pos.mean(axis=0)
+def test_cell_sorted_order_and_mixed(scmd, oracle_ld):
+    """The histogram works on the resident records whatever their internal order (the list path re-sorts them
+    by cell at every build) and whatever the precision mode: two builds with different sorts, then the counts of
+    the second (synthetic) state against the oracle on the same array."""
+    rng = np.random.default_rng(19)
+    a = W.fcc_cluster(3000, 1500.0, seed=9).pos
+    b = a + rng.normal(scale=0.35, size=a.shape)                  # a hot, disordered state
+    centre = b.mean(axis=0)
+    ref, n_o, _ = oracle_ld.rdf_counts(b, 5.0, 0.4, 80, centre=centre)
+    for kw in (dict(r_cut=8.0, skin=1.0), dict(r_cut=8.0, skin=1.0, precision=1), dict(precision=1), dict()):
+        import torch
+        sc = ctx(scmd, a, None, **kw)
+        sc.sc_forces()                                            # build 1: cells of A
+        sc.sc_set_state(torch.as_tensor(b, device="cuda"), None)
+        sc.sc_forces()                                            # build 2: cells of B
         counts, n_ref, _ = sc.sc_rdf(5.0, 0.4, 80, centre=centre)
         sc.close()
-        ref, n_o, _ = oracle_ld.rdf_counts(pos, 5.0, 0.4, 80, centre=centre)
         assert n_ref == n_o and np.array_equal(counts, ref)
 
 
