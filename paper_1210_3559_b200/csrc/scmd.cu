@@ -105,6 +105,7 @@ struct sc_ctx {
 
     // options (0 = default)
     int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0, opt_shift = 0;
+    int emb_pending = 0;          // sweep 1 left this many per-CTA sums of sqrt(rho) in part_a, not yet totalled into U_emb
     int n3_seg = 0;               // j-segment length of the Newton's-third-law sweeps (chunks of 32), chosen at first use
 
     // profiling
@@ -369,15 +370,18 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     c->launches += 1;
     if (!force || energy) {
         const int grid = ceil_div((c->N + 1) / 2, a.pairs_per_cta);
-        if (force && c->opt_shift)
-            reduce_partials_shift_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, kSlotEPair, c->consts.En,
-                                                                   c->counters + kCntPairsInCut,
-                                                                   ipow_host(1.0 / c->p.r_cut, c->p.n));
-        else
-            reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
-                                                             force ? c->consts.En : -c->consts.eps_c);
-        SC_CUDA_CHECK(c, cudaGetLastError());
-        c->launches += 1;
+        if (!force) {
+            c->emb_pending = grid;                                // totalled when an energy is asked for (ensure_forces)
+        } else {
+            if (c->opt_shift)
+                reduce_partials_shift_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, kSlotEPair, c->consts.En,
+                                                                       c->counters + kCntPairsInCut,
+                                                                       ipow_host(1.0 / c->p.r_cut, c->p.n));
+            else
+                reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, kSlotEPair, c->consts.En);
+            SC_CUDA_CHECK(c, cudaGetLastError());
+            c->launches += 1;
+        }
     }
     return SC_OK;
 }
@@ -460,8 +464,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     else n3_finalize_kernel<false><<<fb, kN3FinWarps * 32, 0, c->stream>>>(f);
     c->launches += 2;
     if (!force) {
-        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, fb, c->scal, kSlotEEmb, -c->consts.eps_c);
-        c->launches += 1;
+        c->emb_pending = fb;
     } else if (energy) {
         reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, nb * nseg, c->scal, kSlotEPair, c->consts.En);
         c->launches += 1;
@@ -493,9 +496,10 @@ sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (e == cudaSuccess) e = cudaLaunchKernel(fn, dim3(grid), dim3((tc.warps + 1) * 32), params, smem, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "all-pairs sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
-    if (!force || energy) {
-        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, force ? kSlotEPair : kSlotEEmb,
-                                                         force ? c->consts.En : -c->consts.eps_c);
+    if (!force) {
+        c->emb_pending = grid;
+    } else if (energy) {
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(a.partial, grid, c->scal, kSlotEPair, c->consts.En);
         SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
     }
@@ -514,6 +518,13 @@ sc_status ensure_forces(sc_ctx *c, bool energy) {
     if (c->profile) cudaEventRecord(c->ev[0], c->stream);
     sc_status st = ensure_density(c);
     if (st != SC_OK) return st;
+    if (energy && c->emb_pending) {
+        // U_emb = -eps c sum sqrt(rho_i) from the per-CTA sums sweep 1 left behind: only energy steps pay for this launch
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, c->emb_pending, c->scal, kSlotEEmb, -c->consts.eps_c);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+        c->emb_pending = 0;
+    }
     if (c->profile) cudaEventRecord(c->ev[1], c->stream);
     st = run_sweep(c, true, energy);
     if (st != SC_OK) return st;
@@ -622,6 +633,7 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
     c->small_barrier_count += nbar * uint64_t(grid);
     if (thermo == SC_THERMO_LANGEVIN) c->langevin_step += uint64_t(nsteps);
     c->lambda_pending = false;                           // consumed (and the last scale applied) by the kernel
+    c->emb_pending = 0;                                  // the loop wrote both energy scalars itself
     c->density_valid = c->forces_valid = c->energy_valid = true;
     return SC_OK;
 }
