@@ -209,7 +209,8 @@ sc_status sc_rdf(sc_ctx *ctx, const double *h_centre, double r_select, double bi
  * All arithmetic in binary64 in either precision mode; works with and without a cutoff;
  * five small launches, sums in a fixed order (same input -> same bits); synchronises the stream.
  * SC_ERR_STATE without positions, SC_ERR_INVALID for NULL d_ref_pos / h_msd, align outside
- * 0..2 or NaN r_centre, SC_ERR_NONFINITE if the reference holds non-finite values.
+ * 0..2 or NaN r_centre, SC_ERR_NONFINITE if the displacement sum is not finite (non-finite
+ * reference or positions).
  */
 sc_status sc_msd(sc_ctx *ctx, const double *d_ref_pos, double r_centre, int32_t align, double *h_msd,
                  int64_t *h_n_sel, double *h_rot);
