@@ -355,9 +355,13 @@ def run_ours(args):
     except Exception:
         peak_measured = None
     traffic = None
-    tfile = ROOT / "profiles" / "roofline_traffic.json"
+    tfile = ROOT / "profiles" / "roofline_traffic.csv"      # dram bytes per launch of the dominant kernel, from ncu --set full
     if tfile.exists():
-        traffic = json.loads(tfile.read_text()).get(args.workload, {}).get("force_sweep_dram_bytes_per_launch")
+        import csv
+        with open(tfile, newline="") as fh:
+            for row in csv.DictReader(fh):
+                if row["workload"] == args.workload:
+                    traffic = float(row["force_sweep_dram_bytes_per_launch"])
     if one_launch:
         kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
     elif newton3:
