@@ -88,6 +88,7 @@ struct RebuildArgs {
     double *scal;
     unsigned long long *counters;
     int n_atoms, kmax, max_dim, have_vel, fine_max;
+    int zero_pairs;                 // != 0: a density sweep follows; zero counters[kCntPairsInCut] for it
     double r_list, half_skin2;
 };
 
@@ -103,6 +104,8 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
     const int N = a.n_atoms;
     // ---- decision: uniform over the grid (plain loads of values nobody writes before the last phase) ----
     const bool need = (a.counters[kCntListValid] == 0ull) || (a.scal[kSlotMaxDisp2] > a.half_skin2);
+    // this kernel precedes every density sweep of new positions: it also zeroes that sweep's pair counter
+    if (a.zero_pairs && blockIdx.x == 0 && threadIdx.x == 0) a.counters[kCntPairsInCut] = 0ull;
     if (!need) return;
 
     __shared__ double sh[9][8];

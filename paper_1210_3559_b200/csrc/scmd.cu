@@ -85,6 +85,7 @@ struct sc_ctx {
     double r_list = 0.0;
     int kmax = 0, kmax_cap = 0, max_dim = 1, coop_grid = 0, small_ctas = 0;
     bool list_checked = false;    // rebuild_kernel already launched for the current positions
+    bool pairs_zeroed = false;    // ... and it zeroed the in-range pair counter for the density sweep that follows
     double4 *xs_alt = nullptr, *xs_ref = nullptr;
     double *vel_alt = nullptr, *blockpart = nullptr;
     int *perm = nullptr, *perm_alt = nullptr, *cell_of = nullptr, *slot_of = nullptr, *cell_sorted = nullptr;
@@ -324,6 +325,7 @@ sc_status ensure_list(sc_ctx *c) {
     a.n_atoms = int(c->N); a.kmax = c->kmax; a.max_dim = c->max_dim;
     a.fine_max = c->opt_fine ? c->opt_fine : kFineMax;
     a.have_vel = c->have_vel ? 1 : 0;
+    a.zero_pairs = c->density_valid ? 0 : 1;            // the density sweep that follows counts from zero
     a.r_list = c->r_list; a.half_skin2 = 0.25 * c->skin * c->skin;
     void *params[] = {&a};
     cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void *>(rebuild_kernel), dim3(c->coop_grid), dim3(256),
@@ -331,6 +333,7 @@ sc_status ensure_list(sc_ctx *c) {
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "rebuild_kernel launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     c->list_checked = true;
+    c->pairs_zeroed = a.zero_pairs != 0;
     return SC_OK;
 }
 
@@ -362,7 +365,11 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     a.rc2 = c->p.r_cut * c->p.r_cut;
     a.shift_m = c->opt_shift ? ipow_host(1.0 / c->p.r_cut, c->p.m) : 0.0;
     a.c = c->consts;
-    if (!force) SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
+    if (!force) {
+        if (!c->pairs_zeroed)
+            SC_CUDA_CHECK(c, cudaMemsetAsync(c->counters + kCntPairsInCut, 0, sizeof(unsigned long long), c->stream));
+        c->pairs_zeroed = false;
+    }
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
     cudaError_t e = fast ? launch_nlist_96(lpa, warps * 32, a, force, energy, mixed, c->stream)
                          : launch_nlist_generic(lpa, warps * 32, a, force, energy, mixed, c->stream);
