@@ -274,7 +274,8 @@ def run_ours(args):
     pairs_per_step = float(stats0["n_pairs_in_cut"])                   # N(N-1) for all pairs
     # small all-pairs clusters run the whole sc_step loop in one cooperative launch (csrc/sc_small.cuh):
     # there a bench step is one sc_step call of MD_PER_CALL MD steps and the roofline kernel is the loop itself
-    one_launch = spec.r_cut <= 0 and N <= 6144
+    # the library's own default choices (scmd.cu: kSmallDefaultMaxAtoms*, kN3DefaultMinAtoms*)
+    one_launch = spec.r_cut <= 0 and N <= (4096 if spec.prec == "fp64" else 2304)
     md_per_call = 100 if one_launch else 1
     if not one_launch:
         sc.sc_profile(True)
@@ -337,7 +338,8 @@ def run_ours(args):
     if rank != 0:
         return
     i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
-    newton3 = spec.r_cut <= 0 and 7000 <= N <= 262144 and not args.one_sided
+    newton3 = (spec.r_cut <= 0 and (4097 if spec.prec == "fp64" else 4609) <= N <= 262144 and not one_launch
+               and not args.one_sided)
     if newton3:
         i_f, i_d = I_FORCE_ENERGY_N3[spec.prec], I_DENSITY_N3[spec.prec]
     if one_launch:

@@ -157,8 +157,8 @@ int cutoff_max_dim(int64_t N) {
 }
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
-constexpr int64_t kN3MinAtoms = 7000, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
-constexpr int64_t kN3DefaultMinAtoms = 7000, kN3DefaultMinAtomsMixed = 7000;   // measured crossovers
+constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
+constexpr int64_t kN3DefaultMinAtoms = 4097, kN3DefaultMinAtomsMixed = 4609;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
 constexpr int kN3MaxSegments = 25;                             // j segments of the longest row block
 
@@ -574,12 +574,15 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
 // ---------------------------------------------------------------------------------------------
 // one-launch step loop (sc_small.cuh): small all-pairs FP64 clusters
 // ---------------------------------------------------------------------------------------------
-constexpr int64_t kSmallDefaultMaxAtoms = kSmallMaxAtoms;   // measured: the loop beats the multi-launch path up to its capacity
+// measured crossovers with the multi-launch path (Newton's-third-law sweeps, FP64; one-sided packed sweeps, mixed):
+// FP64: N = 3000 43 us per step either way, N = 4096 62.5 (loop) against 61.5 us, N = 5000 129 against 68 us;
+// mixed: N = 2057 23 (loop) against 28 us, N = 2500 44 against 37 us
+constexpr int64_t kSmallDefaultMaxAtoms = 4096, kSmallDefaultMaxAtomsMixed = 2304;
 
 bool small_path_wanted(const sc_ctx *c) {
     if (c->cutoff || !c->xs_b || c->opt_persistent == 2 || c->profile) return false;
     if (c->N > kSmallMaxAtoms) return false;
-    return c->opt_persistent == 1 || c->N <= kSmallDefaultMaxAtoms;
+    return c->opt_persistent == 1 || c->N <= (c->precision == SC_PREC_MIXED ? kSmallDefaultMaxAtomsMixed : kSmallDefaultMaxAtoms);
 }
 
 sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int thermo, int64_t nsteps) {
