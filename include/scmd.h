@@ -106,7 +106,8 @@ typedef enum {
     SC_OPT_PERSISTENT = 4,        /* all pairs, N <= 6144: the whole sc_step loop (all nsteps) in ONE
                                      cooperative launch, records staged in shared memory, grid
                                      barriers between the phases of a step.  0: library default
-                                     (on whenever it applies), 1: on, 2: never (one launch per
+                                     (on for N <= 4096, mixed precision N <= 2304: the measured
+                                     crossovers), 1: on, 2: never (one launch per
                                      sweep and per integrator stage).  Off while sc_profile is on. */
     SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
     SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max entries per row of the Verlet list (cutoff path); rounded
@@ -116,10 +117,11 @@ typedef enum {
                                      takes effect at the next list build                         */
     SC_OPT_ATOMS_PER_CTA = 9,     /* cutoff path: consecutive atoms one CTA of the list sweeps
                                      works through (rounded to the warp layout)                  */
-    SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 7000 <= N <= 262144 (the range in which
+    SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 2048 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
-                                     both atoms.  0: library default (on), 1: on,
+                                     both atoms.  0: library default (on from N = 4097, mixed
+                                     precision 4609), 1: on,
                                      2: off = the one-sided sweeps                               */
     SC_OPT_CUTOFF_SHIFT = 11      /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
                                      configs; 1 energy-shifted terms: inside r_cut every pair term
