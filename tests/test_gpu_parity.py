@@ -86,7 +86,8 @@ def test_tile_shapes_ragged(scmd, oracle_ld, it, tpr, warps):
 
 
 @pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3)),
-                                        (12345, dict(n=7, m=3, eps=0.02, c=30.0, a=3.3))])
+                                        (12345, dict(n=7, m=3, eps=0.02, c=30.0, a=3.3)),
+                                        (2048, {}), (4097, {}), (5003, {})])   # smallest carved size, the default's lower end
 def test_newton3_sweeps(scmd, oracle_ld, n_atoms, kw):
     """Every unordered pair once, its term added to both atoms (csrc/sc_allpairs_n3.cuh): block-aligned and ragged
     sizes (dummy rows and records, diagonal chunks), (9, 6) and generic exponents; same tolerances as the one-sided
