@@ -11,7 +11,10 @@ roofline target (N >= 65,536) is quoted on.  Other workloads (same JSON line):
     Ni<N>-<fcc|liquid|mackay>-<allpairs|cutoff10>-<fp64|mixed>
 Prints ONE JSON line.  N > 1 GPUs = N independent replicas
 (the paper's own use: up to 15 independent trajectories per temperature); the
-only collective is the timing reduction.
+only collective is the timing reduction.  `--gpus N` with N > 1 and no torchrun environment
+starts the N ranks itself (re-executes under `python -m torch.distributed.run`); under torchrun
+(the driver's launch) it is one of the ranks.  The default run also times, 20 steps each, the
+mixed all-pairs and the cutoff-list variants of the same cluster and reports them in `also`.
 """
 from __future__ import annotations
 
@@ -201,25 +204,57 @@ def in_range_fraction(w: W.Workload, r_cut: float) -> float:
     return hits / (rows.size * (w.n_atoms - 1.0))
 
 
-def cpu_baseline(w: W.Workload, r_cut: float = 0.0, pair_fraction: float = 1.0, budget_s: float = 12.0) -> dict:
-    """The oracle as it stands on the host cores: whole evaluations of the workload (or, when one
-    evaluation would exceed the budget, an evenly spaced row sample of it), repeated for ~budget_s."""
+ORACLE_BUILD = "binary64 oracle build (gcc -O3 -march=native -fopenmp, no fast-math, no FMA contraction)"
+
+
+def cpu_baseline(w: W.Workload, r_cut: float = 0.0, pair_fraction: float = 1.0, budget_s: float = 10.0) -> dict:
+    """The oracle as it stands on the host cores: (i) on all cores (OpenMP over rows) -- whole
+    evaluations of the workload or, when one would exceed the budget, an evenly spaced row sample of it,
+    repeated for ~budget_s; (ii) on ONE thread (the paper compared its GPU with a single CPU core,
+    PAPER.md:129), a smaller row sample of the same workload."""
+    from oracle import sc_oracle
+    cores = os.cpu_count() or 1
+    filt = ", filtered at r_c" if r_cut > 0 else ""
+    sc_oracle.set_threads(cores)
     rows = oracle_sample_rows(w.n_atoms, target_pair_passes=2.0e10)
     total_s, total_pairs, reps = 0.0, 0.0, 0
     while reps < 8 and (reps == 0 or total_s < budget_s):
         dt, pairs = oracle_time_sample(w, rows, r_cut, pair_fraction)
         total_s += dt; total_pairs += pairs; reps += 1
     what = "all rows" if rows.size == w.n_atoms else f"{rows.size} evenly spaced rows i"
-    return {"value": total_pairs / total_s, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+    # single thread: ~1/cores of the pair visits, so that it takes about as long
+    sc_oracle.set_threads(1)
+    rows1 = oracle_sample_rows(w.n_atoms, target_pair_passes=2.0e10 / cores)
+    s1, p1, reps1 = 0.0, 0.0, 0
+    while reps1 < 4 and (reps1 == 0 or s1 < 0.6 * budget_s):
+        dt, pairs = oracle_time_sample(w, rows1, r_cut, pair_fraction)
+        s1 += dt; p1 += pairs; reps1 += 1
+    sc_oracle.set_threads(cores)
+    what1 = "all rows" if rows1.size == w.n_atoms else f"{rows1.size} evenly spaced rows i"
+    return {"value": total_pairs / total_s, "unit": UNIT, "cores": cores, "kind": "oracle",
             "seconds": total_s,
-            "sample": f"{reps} x ({what} of {w.name}, all j, both sweeps{', filtered at r_c' if r_cut > 0 else ''}), "
-                      "binary64 oracle build, OpenMP on all host cores"}
+            "sample": f"{reps} x ({what} of {w.name}, all j, both sweeps{filt}), {ORACLE_BUILD}, OpenMP on all {cores} host cores",
+            "single_thread": {"value": p1 / s1, "unit": UNIT, "cores": 1, "seconds": s1,
+                              "sample": f"{reps1} x ({what1} of {w.name}, all j, both sweeps{filt}), same build, 1 thread"}}
+
+
+def config_dict(spec: Spec, n_atoms: int, pairs_per_step: float, world: int, md_per_call: int) -> dict:
+    """The `config` object of the JSON line: the same keys from both arms."""
+    return {"workload": spec.name, "n_atoms": n_atoms, "pairs_per_step": pairs_per_step,
+            "r_cut": spec.r_cut, "skin": spec.skin,
+            "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2": "flushed between timed steps (256 MiB memset outside the per-step events)",
+            "md_steps_per_bench_step": md_per_call,
+            "step": f"sc_step(dt=1 fs, nsteps={md_per_call}): kick+drift, [skin check / rebuild,] density sweep, "
+                    "force+energy sweep, kick+KE"}
 
 
 def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return
+    from oracle import sc_oracle
+    sc_oracle.set_threads(os.cpu_count() or 1)
     spec = Spec(args.workload)
     w = spec.generate()
     frac = in_range_fraction(w, spec.r_cut)
@@ -232,11 +267,14 @@ def run_reference(args):
         total_s += dt; total_pairs += pairs
     value = total_pairs / total_s
     sample = (f"each step = {rows.size} evenly spaced rows i of {w.name} (all j, both sweeps), "
-              f"binary64 oracle build, OpenMP on {os.cpu_count()} host cores")
+              f"{ORACLE_BUILD}, OpenMP on {os.cpu_count()} host cores")
+    n = w.n_atoms
+    pairs_per_step = float(n) * (n - 1) * frac       # in-range ordered pairs of one whole evaluation (estimate for a cutoff)
+    md_per_call = 1
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_atoms": w.n_atoms},
+            "config": config_dict(spec, n, pairs_per_step, 1, md_per_call),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -246,6 +284,176 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------- #
 # our arm
 # ------------------------------------------------------------------------------------------- #
+PATH_NAMES = {0: "one-sided", 1: "newton3", 2: "one-launch", 3: "lists"}
+
+
+def measure(scmd, spec: Spec, steps: int, warmup: int, rank: int, world: int, dev, one_sided: bool,
+            with_e2e: bool, sampler: "ClockSampler | None"):
+    """Time `steps` bench steps of one workload on this rank.  -> dict of local results (no collectives)."""
+    import torch
+    w = spec.generate(rank)
+    N = w.n_atoms
+    prec = scmd.SC_PREC_MIXED if spec.prec == "mixed" else scmd.SC_PREC_FP64
+    sc = scmd.SuttonChen(N, r_cut=spec.r_cut, skin=spec.skin, precision=prec)
+    d_pos = torch.as_tensor(w.pos, device=dev)
+    d_vel = torch.as_tensor(w.vel, device=dev)
+    if one_sided:
+        sc.sc_set_option(scmd.SC_OPT_NEWTON3, 2)
+    sc.sc_set_state(d_pos, d_vel)
+    sc.sc_energy()                                                     # first evaluation (builds the rows)
+    stats0 = sc.sc_stats()
+    pairs_per_step = float(stats0["n_pairs_in_cut"])                   # N(N-1) for all pairs
+    # which kernels the library runs for this context is the library's choice: ask it (SC_INFO_STEP_PATH).
+    # In the one-launch loop (small all-pairs clusters, csrc/sc_small.cuh) a bench step is one sc_step call of
+    # MD_PER_CALL MD steps and the roofline kernel is the loop itself.
+    step_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)
+    one_launch = step_path == 2
+    md_per_call = 100 if one_launch else 1
+    if not one_launch:
+        sc.sc_profile(True)
+        sweep_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)          # profiling forbids the loop: the path that is timed
+    else:
+        sweep_path = 2
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def one_step():
+        sc.sc_step(1.0, md_per_call)
+
+    for _ in range(max(warmup, 3)):
+        one_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    if sampler is not None:
+        sampler.mark()                                                 # samples before this are dropped (warm-up)
+    launches0 = sc.sc_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    ms_force, ms_density = [], []
+    torch.cuda.synchronize()
+    for k in range(steps):
+        flush.zero_()                                                  # L2 flush, outside the timed events
+        ev[k][0].record(stream)
+        one_step()
+        ev[k][1].record(stream)
+        if one_launch:
+            continue
+        prof = sc.sc_profile_read()                                    # synchronises
+        ms_force.append(prof["ms_force"]); ms_density.append(prof["ms_density"])
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = sc.sc_launch_count() - launches0
+    if one_launch:
+        assert launches == steps, f"one-launch loop expected, {launches} launches in {steps} calls"
+    stats1 = sc.sc_stats()
+    local_ms = sum(a.elapsed_time(b) for a, b in ev)
+    out = dict(w=w, N=N, pairs_per_step=pairs_per_step, md_per_call=md_per_call, one_launch=one_launch,
+               sweep_path=sweep_path, local_ms=local_ms, launches=launches, stats0=stats0, stats1=stats1,
+               ms_force=ms_force, ms_density=ms_density)
+
+    if with_e2e:
+        # end to end through the host-buffer entry point: upload positions, both sweeps (cutoff: plus the
+        # cell sort and row build, since new positions invalidate the rows), download forces + energy
+        # (pinned host memory), every step
+        h_pos = torch.as_tensor(w.pos).pin_memory()
+        h_force = torch.empty(N, 3, dtype=torch.float64).pin_memory()
+        for _ in range(2):
+            sc.sc_eval_host(h_pos, h_force)
+        torch.cuda.synchronize()
+        e2e_steps = max(3, min(steps, 10))
+        t_e2e = 0.0
+        for _ in range(e2e_steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            sc.sc_eval_host(h_pos, h_force)                            # returns after the D2H copy
+            t_e2e += time.perf_counter() - t0
+        out.update(e2e_ms=t_e2e * 1e3, e2e_steps=e2e_steps)
+    sc.close()
+    del flush
+    return out
+
+
+def roofline_block(scmd, spec: Spec, m: dict, steps: int) -> dict:
+    N, pairs_per_step, path = m["N"], m["pairs_per_step"], m["sweep_path"]
+    i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
+    newton3 = path == 1
+    if newton3:
+        i_f, i_d = I_FORCE_ENERGY_N3[spec.prec], I_DENSITY_N3[spec.prec]
+    if m["one_launch"]:
+        # one kernel holds both sweeps: split its time in proportion to the instruction counts
+        t_both = m["local_ms"] * 1e-3 / (steps * m["md_per_call"])
+        t_force, t_density = t_both * i_f / (i_f + i_d), t_both * i_d / (i_f + i_d)
+    else:
+        t_force = statistics.mean(m["ms_force"]) * 1e-3
+        t_density = statistics.mean(m["ms_density"]) * 1e-3
+    achieved = i_f * 2.0 * pairs_per_step / t_force / 1e12
+    probe_kind = 0 if spec.prec == "fp64" else 2
+    try:
+        rate, _ = scmd.probe_throughput(probe_kind)
+        peak_measured = rate * 2.0 / 1e12
+    except Exception:
+        peak_measured = None
+    traffic, traffic_source = None, None
+    tfile = ROOT / "profiles" / "roofline_traffic.csv"      # dram bytes per launch of the dominant kernel, from ncu --set full
+    if tfile.exists():
+        import csv
+        with open(tfile, newline="") as fh:
+            for row in csv.DictReader(fh):
+                if row["workload"] == spec.name:
+                    traffic = float(row["force_sweep_dram_bytes_per_launch"])
+                    traffic_source = "committed ncu reading, not measured in this run: " + row["source"]
+    if m["one_launch"]:
+        kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
+    elif newton3:
+        kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3p_kernel") + \
+                 "<force+energy> (every unordered pair once) + n3_finalize_kernel"
+    elif spec.r_cut > 0:
+        kernel = f"nlist_kernel<force+energy, {spec.prec}>"
+    else:
+        kernel = ("allpairs64_kernel" if spec.prec == "fp64" else "allpairs32_kernel") + "<force+energy>"
+    pipe = "FP64" if spec.prec == "fp64" else "FP32"
+    roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                "traffic_source": traffic_source,
+                "peak_source": f"nominal: 148 SM x {LANES[spec.prec]} {pipe} lanes x 2 x 1.965 GHz (DESIGN.md section 6); "
+                               "MEASURED_PEAKS.json has no CUDA-core figure",
+                "peak_measured_fma_probe": peak_measured,
+                "frac_vs_probe": achieved / peak_measured if peak_measured else None,
+                "alu_inst_per_pair": i_f, "ms_force_sweep": t_force * 1e3, "ms_density_sweep": t_density * 1e3,
+                "density_sweep_frac": i_d * 2.0 * pairs_per_step / t_density / 1e12 / peak,
+                "both_sweeps_frac": (i_d + i_f) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / peak}
+    if newton3:
+        # the same time measured against the ONE-SIDED instruction count (22 per ordered pair, the formulation
+        # BASELINE.json's north_star names): a speed-up figure (> 1 = faster than a one-sided sweep at FP64 peak),
+        # never a fraction of peak
+        roofline["speedup_vs_one_sided_at_peak"] = I_FORCE_ENERGY[spec.prec] * 2.0 * pairs_per_step / t_force / 1e12 / peak
+        roofline["note"] = (f"frac counts the instructions this kernel must execute: {2 * i_f:g} per unordered pair = "
+                            f"{i_f:g} per ordered pair (DESIGN.md 6.8)")
+    if spec.r_cut > 0:
+        # the list path's memory side (SURVEY 8d): the method's own bytes are records in + forces out;
+        # the neighbour rows are the data structure's cost
+        hbm_peak, hbm_src = 6469.9, "fallback literal (MEASURED_PEAKS.json absent)"
+        try:
+            hbm_peak = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]
+            hbm_src = "MEASURED_PEAKS.json hbm_gbs (measured copy)"
+        except Exception:
+            pass
+        alg_bytes = N * (32 + 8 + 24 + 32)                              # both sweeps: records, rho, forces
+        t_sweeps = t_force + t_density
+        hbm = {"algorithmic_bytes_per_step": alg_bytes, "peak_gbs": hbm_peak, "peak_source": hbm_src,
+               "algorithmic_gbs": alg_bytes / t_sweeps / 1e9, "frac": alg_bytes / t_sweeps / 1e9 / hbm_peak,
+               "rebuilds_in_timed_region": m["stats1"]["n_rebuilds"] - m["stats0"]["n_rebuilds"],
+               "max_neighbours": m["stats1"]["max_neighbours"]}
+        if traffic is not None:
+            hbm["moved_gbs_force_sweep"] = traffic / t_force / 1e9
+            hbm["moved_frac_force_sweep"] = traffic / t_force / 1e9 / hbm_peak
+        roofline["hbm"] = hbm
+    return roofline
+
+
 def run_ours(args):
     import torch
     import paper_1210_3559_b200 as scmd
@@ -260,171 +468,67 @@ def run_ours(args):
     scmd.load_library()
 
     spec = Spec(args.workload)
-    w = spec.generate(rank)
-    N = w.n_atoms
-    prec = scmd.SC_PREC_MIXED if spec.prec == "mixed" else scmd.SC_PREC_FP64
-    sc = scmd.SuttonChen(N, r_cut=spec.r_cut, skin=spec.skin, precision=prec)
-    d_pos = torch.as_tensor(w.pos, device=dev)
-    d_vel = torch.as_tensor(w.vel, device=dev)
-    if args.one_sided:
-        sc.sc_set_option(scmd.SC_OPT_NEWTON3, 2)
-    sc.sc_set_state(d_pos, d_vel)
-    sc.sc_energy()                                                     # first evaluation (builds the rows)
-    stats0 = sc.sc_stats()
-    pairs_per_step = float(stats0["n_pairs_in_cut"])                   # N(N-1) for all pairs
-    # small all-pairs clusters run the whole sc_step loop in one cooperative launch (csrc/sc_small.cuh):
-    # there a bench step is one sc_step call of MD_PER_CALL MD steps and the roofline kernel is the loop itself
-    # the library's own default choices (scmd.cu: kSmallDefaultMaxAtoms*, kN3DefaultMinAtoms*)
-    one_launch = spec.r_cut <= 0 and N <= (4096 if spec.prec == "fp64" else 2304)
-    md_per_call = 100 if one_launch else 1
-    if not one_launch:
-        sc.sc_profile(True)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
-    stream = torch.cuda.current_stream()
-
-    def one_step():
-        sc.sc_step(1.0, md_per_call)
-
-    sampler = ClockSampler(dev.index or 0)
-    if rank == 0:
-        sampler.start()                                                # samples before mark() are dropped
-    for _ in range(max(args.warmup, 3)):
-        one_step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    sampler.mark()
-    launches0 = sc.sc_launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    ms_force, ms_density = [], []
-    torch.cuda.synchronize()
-    for k in range(args.steps):
-        flush.zero_()                                                  # L2 flush, outside the timed events
-        ev[k][0].record(stream)
-        one_step()
-        ev[k][1].record(stream)
-        if one_launch:
-            continue
-        prof = sc.sc_profile_read()                                    # synchronises
-        ms_force.append(prof["ms_force"]); ms_density.append(prof["ms_density"])
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    launches = sc.sc_launch_count() - launches0
-    clocks = sampler.stop() if rank == 0 else None
-    stats1 = sc.sc_stats()
-    local_ms = sum(a.elapsed_time(b) for a, b in ev)
-    total_ms, total_pairs = aggregate(local_ms, pairs_per_step * args.steps * md_per_call, world)
+    sampler = ClockSampler(dev.index or 0) if rank == 0 else None
+    if sampler is not None:
+        sampler.start()
+    m = measure(scmd, spec, args.steps, args.warmup, rank, world, dev, args.one_sided, True, sampler)
+    clocks = sampler.stop() if sampler is not None else None
+    N, pairs_per_step, md_per_call = m["N"], m["pairs_per_step"], m["md_per_call"]
+    total_ms, total_pairs = aggregate(m["local_ms"], pairs_per_step * args.steps * md_per_call, world)
     value = total_pairs / (total_ms * 1e-3)
+    e2e_ms, e2e_pairs = aggregate(m["e2e_ms"], pairs_per_step * m["e2e_steps"], world)
+    launches = m["launches"]
 
-    # end to end through the host-buffer entry point: upload positions, both sweeps (cutoff: plus the
-    # cell sort and row build, since new positions invalidate the rows), download forces + energy
-    # (pinned host memory), every step
-    h_pos = torch.as_tensor(w.pos).pin_memory()
-    h_force = torch.empty(N, 3, dtype=torch.float64).pin_memory()
-    for _ in range(2):
-        sc.sc_eval_host(h_pos, h_force)
-    torch.cuda.synchronize()
-    e2e_steps = max(3, min(args.steps, 10))
-    t_e2e = 0.0
-    for _ in range(e2e_steps):
-        flush.zero_()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        sc.sc_eval_host(h_pos, h_force)                                # returns after the D2H copy
-        t_e2e += time.perf_counter() - t0
-    e2e_ms, e2e_pairs = aggregate(t_e2e * 1e3, pairs_per_step * e2e_steps, world)
-
+    # the other two variants of the same cluster (mixed all pairs, cutoff lists): 20 steps each, so that the
+    # mixed >= 60 % and the neighbour-list figures are timed by whoever runs this file, not claimed
+    also = []
+    if args.also and world == 1 and args.workload == DEFAULT_WORKLOAD and not args.one_sided:
+        for name in ALSO_WORKLOADS:
+            s2 = Spec(name)
+            m2 = measure(scmd, s2, 20, 3, rank, world, dev, False, False, None)
+            ms2 = m2["local_ms"] / 20
+            launches += m2["launches"]
+            also.append({"workload": name, "steps": 20, "warmup": 3, "ms_per_step": ms2,
+                         "value": m2["pairs_per_step"] * m2["md_per_call"] / (ms2 * 1e-3), "unit": UNIT,
+                         "md_steps_per_s": m2["md_per_call"] / (ms2 * 1e-3),
+                         "dtype": "f64" if s2.prec == "fp64" else "f32 pair math, f64 accumulation",
+                         "path": PATH_NAMES[m2["sweep_path"]], "pairs_per_step": m2["pairs_per_step"],
+                         "gpu_launches": m2["launches"], "roofline": roofline_block(scmd, s2, m2, 20)})
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
     if rank != 0:
         return
-    i_f, i_d, peak = I_FORCE_ENERGY[spec.prec], I_DENSITY[spec.prec], PEAK_TFLOPS[spec.prec]
-    newton3 = (spec.r_cut <= 0 and (4097 if spec.prec == "fp64" else 4609) <= N <= 262144 and not one_launch
-               and not args.one_sided)
-    if newton3:
-        i_f, i_d = I_FORCE_ENERGY_N3[spec.prec], I_DENSITY_N3[spec.prec]
-    if one_launch:
-        # one kernel holds both sweeps: split its time in proportion to the instruction counts
-        t_both = local_ms * 1e-3 / (args.steps * md_per_call)
-        t_force, t_density = t_both * i_f / (i_f + i_d), t_both * i_d / (i_f + i_d)
-    else:
-        t_force = statistics.mean(ms_force) * 1e-3
-        t_density = statistics.mean(ms_density) * 1e-3
-    achieved = i_f * 2.0 * pairs_per_step / t_force / 1e12
-    probe_kind = 0 if spec.prec == "fp64" else 2
-    try:
-        rate, _ = scmd.probe_throughput(probe_kind)
-        peak_measured = rate * 2.0 / 1e12
-    except Exception:
-        peak_measured = None
-    traffic = None
-    tfile = ROOT / "profiles" / "roofline_traffic.csv"      # dram bytes per launch of the dominant kernel, from ncu --set full
-    if tfile.exists():
-        import csv
-        with open(tfile, newline="") as fh:
-            for row in csv.DictReader(fh):
-                if row["workload"] == args.workload:
-                    traffic = float(row["force_sweep_dram_bytes_per_launch"])
-    if one_launch:
-        kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
-    elif newton3:
-        kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3p_kernel") + \
-                 "<force+energy> (every unordered pair once) + n3_finalize_kernel"
-    elif spec.r_cut > 0:
-        kernel = f"nlist_kernel<force+energy, {spec.prec}>"
-    else:
-        kernel = ("allpairs64_kernel" if spec.prec == "fp64" else "allpairs32_kernel") + "<force+energy>"
-    pipe = "FP64" if spec.prec == "fp64" else "FP32"
-    roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
-                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
-                "peak_source": f"nominal: 148 SM x {LANES[spec.prec]} {pipe} lanes x 2 x 1.965 GHz (DESIGN.md section 6); "
-                               "MEASURED_PEAKS.json has no CUDA-core figure",
-                "peak_measured_fma_probe": peak_measured,
-                "alu_inst_per_pair": i_f, "ms_force_sweep": t_force * 1e3, "ms_density_sweep": t_density * 1e3,
-                "density_sweep_frac": i_d * 2.0 * pairs_per_step / t_density / 1e12 / peak,
-                "both_sweeps_frac": (i_d + i_f) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / peak}
-    if newton3:
-        # the same time measured against the ONE-SIDED instruction count (22 per ordered pair, the formulation
-        # BASELINE.json's north_star names): > 1 means the algorithmic saving outruns a one-sided sweep at FP64 peak
-        roofline["frac_vs_one_sided_count"] = I_FORCE_ENERGY[spec.prec] * 2.0 * pairs_per_step / t_force / 1e12 / peak
-        roofline["note"] = (f"frac counts the instructions this kernel must execute: {2 * i_f:g} per unordered pair = "
-                            f"{i_f:g} per ordered pair (DESIGN.md 6.8)")
-    if spec.r_cut > 0:
-        # the list path's memory side: the method's own bytes are records in + forces out;
-        # the neighbour indices (4 B per entry per sweep) are the data structure's cost
-        hbm_peak = 6445.6
-        try:
-            hbm_peak = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]
-        except Exception:
-            pass
-        alg_bytes = N * (32 + 8 + 24 + 32)                              # both sweeps: records, rho, forces
-        roofline["hbm"] = {"algorithmic_bytes_per_step": alg_bytes, "peak_gbs": hbm_peak,
-                           "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy)",
-                           "algorithmic_gbs": alg_bytes / (t_force + t_density) / 1e9,
-                           "frac": alg_bytes / (t_force + t_density) / 1e9 / hbm_peak,
-                           "rebuilds_in_timed_region": stats1["n_rebuilds"] - stats0["n_rebuilds"],
-                           "max_neighbours": stats1["max_neighbours"]}
+    roofline = roofline_block(scmd, spec, m, args.steps)
     frac_pairs = pairs_per_step / (float(N) * (N - 1)) if N > 1 else 1.0
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64" if spec.prec == "fp64" else "f32 pair math, f64 accumulation",
             "data": "synthetic",
             "md_steps_per_s": world * args.steps * md_per_call / (total_ms * 1e-3),
-            "config": {"workload": args.workload, "n_atoms": N, "pairs_per_step": pairs_per_step,
-                       "r_cut": spec.r_cut, "skin": spec.skin,
-                       "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "flushed between timed steps (256 MiB memset outside the per-step events)",
-                       "md_steps_per_bench_step": md_per_call,
-                       "step": f"sc_step(dt=1 fs, nsteps={md_per_call}): kick+drift, [skin check / rebuild,] density sweep, "
-                               "force+energy sweep, kick+KE"},
+            "config": config_dict(spec, N, pairs_per_step, world, md_per_call),
+            "path": PATH_NAMES[m["sweep_path"]],
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * N,
                     "d2h_bytes_per_step": 24 * N + 16, "call": "sc_eval_host (pinned host buffers)",
-                    "ms_per_call": e2e_ms / e2e_steps},
-            "roofline": roofline, "cpu_baseline": cpu_baseline(w, spec.r_cut, frac_pairs)}
+                    "ms_per_call": e2e_ms / m["e2e_steps"]},
+            "roofline": roofline, "cpu_baseline": cpu_baseline(m["w"], spec.r_cut, frac_pairs)}
+    if also:
+        line["also"] = also
     print(json.dumps(line), flush=True)
 
 
-def main():
+ALSO_WORKLOADS = ["Ni65536-fcc-allpairs-mixed", "Ni65536-fcc-cutoff10-fp64"]
+
+
+def launcher_command(args, argv: list[str], port: int) -> list[str]:
+    """`--gpus N` without a torchrun environment: the command that starts the N ranks (one per GPU, NCCL)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve()), *argv]
+
+
+def main(argv=None):
+    argv = list(sys.argv[1:] if argv is None else argv)
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
@@ -433,7 +537,23 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--one-sided", action="store_true",
                     help="all pairs: force the one-sided sweeps (SC_OPT_NEWTON3 = 2) where Newton's third law is the default")
-    args = ap.parse_args()
+    ap.add_argument("--no-also", dest="also", action="store_false",
+                    help="default workload only: skip the mixed and cutoff-list variants reported in `also`")
+    args = ap.parse_args(argv)
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        # not under torchrun: start the ranks ourselves and hand over (rank 0 prints the line)
+        import socket
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "WARN")
+        raise SystemExit(subprocess.run(launcher_command(args, argv, port), env=env).returncode)
+    _, _, world = dist_env()
+    if args.impl == "ours" and world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE = {world}: launch with --nproc-per-node {args.gpus}")
     if args.impl == "reference":
         run_reference(args)
     else:

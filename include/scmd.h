@@ -132,8 +132,32 @@ typedef enum {
                                      Q21).  Ignored without a cutoff.                            */
 } sc_option;
 
+/* Read-only queries (sc_get_option), beside the sc_option values themselves. */
+typedef enum {
+    SC_INFO_STEP_PATH = 100,          /* which kernels sc_step / sc_forces run for this context as it is configured now:
+                                         0 one-sided all-pairs sweeps, 1 Newton's-third-law all-pairs sweeps,
+                                         2 the one-launch step loop (sc_step only; its sc_forces is 0 or 1), 3 cutoff lists */
+    SC_INFO_NEIGHBOUR_CAPACITY = 101, /* cutoff path: K_max entries per atom the rows hold now (0 for all pairs)       */
+    SC_INFO_NEIGHBOUR_CAPACITY_MAX = 102 /* ... and the largest value the workspace was sized for                        */
+} sc_info;
+
+/* Optional create-time sizing (sc_workspace_bytes_ex / sc_create_ex).  Zero-initialise, then set what is needed;
+ * a NULL pointer means all defaults (= sc_workspace_bytes / sc_create). */
+typedef struct {
+    int32_t neighbour_capacity;   /* cutoff path: K_max entries per atom the neighbour rows are sized for.  0 = default:
+                                     1.3 x the fcc number density 4 / a^3 inside the list sphere, which a system denser
+                                     than that overflows (SC_ERR_CAPACITY) -- then create the context again with the
+                                     max_neighbours sc_stats reported, plus headroom                                    */
+    int32_t newton3_storage;      /* all pairs: 0 = carve the ~N^2 / 8 bytes of partial sums of the Newton's-third-law
+                                     sweeps where they apply (2048 <= N <= 262144), 2 = never (SC_OPT_NEWTON3 is then
+                                     fixed at 2: one-sided sweeps, O(N) workspace)                                      */
+    int32_t reserved[6];          /* must be 0                                                                          */
+} sc_create_options;
+
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */
 size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t precision, double skin);
+size_t sc_workspace_bytes_ex(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
+                             const sc_create_options *options);
 
 /*
  * Create a context for n_atoms atoms.
@@ -147,8 +171,15 @@ size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t prec
  */
 sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
                     void *d_workspace, size_t workspace_bytes, void *cuda_stream, sc_ctx **out);
+sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
+                       const sc_create_options *options, void *d_workspace, size_t workspace_bytes,
+                       void *cuda_stream, sc_ctx **out);
 sc_status sc_destroy(sc_ctx *ctx);
 sc_status sc_set_option(sc_ctx *ctx, int32_t option, int64_t value);
+/* Current value of an sc_option (as set, 0 = library default; SC_OPT_LANGEVIN_STEP: the generator step of the
+ * next Langevin update, so that a run can be resumed exactly without the caller counting steps) or of an
+ * sc_info query.  No device work, no synchronisation. */
+sc_status sc_get_option(sc_ctx *ctx, int32_t option, int64_t *value);
 
 /* Copy positions (required) and velocities (d_vel may be NULL: velocities unset) in. */
 sc_status sc_set_state(sc_ctx *ctx, const double *d_pos, const double *d_vel);
@@ -236,25 +267,6 @@ sc_status sc_launch_count(sc_ctx *ctx, int64_t *n_launches);
  * (SC_ERR_STATE if none was recorded). */
 sc_status sc_profile(sc_ctx *ctx, int32_t enable);
 sc_status sc_profile_read(sc_ctx *ctx, double *h_ms_density, double *h_ms_force);
-
-/*
- * Diagnostics that need no context.  d_scratch: caller-owned device memory, >= 64 KiB.
- *
- * sc_probe_throughput: register-only dependent-FMA-chain kernel on every SM; reports
- *   thread-level instructions per second and the SM clock (MHz) held during the run.
- *   kind 0: FP64 DFMA   1: FP32 FFMA   2: packed FP32x2 FMA (counted as 2 per lane)
- *        3: MUFU.RSQ (binary32)        4: FP64 reciprocal seed (MUFU.RCP64H)
- *        5: FP32 FADD   6: FP32 FMUL   7: packed FADD2   8: packed FMUL2 (packed: 2 per lane)
- *   bench.py prints the measured figure beside the nominal ALU peak.
- * sc_probe_reciprocal: maximum relative error, over n_samples log-uniform x in [lo, hi], of
- *   h_err4 = { rcp seed, refined 1/x, rsqrt seed, refined x^-1/2 } as used by the FP64 sweeps,
- *   against IEEE division / sqrt on the device.
- * Both synchronise the stream.
- */
-sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, size_t scratch_bytes,
-                              double *h_inst_per_s, double *h_sm_clock_mhz);
-sc_status sc_probe_reciprocal(double lo, double hi, int32_t n_samples, void *cuda_stream, void *d_scratch,
-                              size_t scratch_bytes, double *h_err4);
 
 const char *sc_last_error(const sc_ctx *ctx);
 const char *sc_version(void);

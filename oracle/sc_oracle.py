@@ -5,13 +5,18 @@ legs may import this.  It never imports the CUDA package.  See sc_oracle.c's hea
 for what is computed and which passage of PAPER.md each function follows.
 
 Two shared objects are built from the one C file:
-  liboracle_ld.so     long-double pair arithmetic + accumulators  (parity reference)
-  liboracle_plain.so  binary64 throughout                          (the timed baseline)
+  liboracle_ld.so              long-double pair arithmetic + accumulators  (parity reference; gcc -O2)
+  liboracle_plain_<host>.so    binary64 throughout (the timed baseline; gcc -O3 -march=native -fopenmp as SURVEY.md
+                               section 8(d) prescribes, still no fast-math and no FMA contraction).  -march=native code
+                               must not travel between machines, so the file name carries a hash of this host's CPU
+                               flags and compiler version: the GPU box builds its own copy on first use.
 """
 from __future__ import annotations
 
 import ctypes
+import hashlib
 import os
+import platform
 import subprocess
 from pathlib import Path
 
@@ -19,9 +24,28 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "sc_oracle.c"
+
+
+def _host_tag() -> str:
+    """Short hash of what -march=native depends on: the CPU feature flags and the compiler version."""
+    flags = platform.machine()
+    try:
+        for line in Path("/proc/cpuinfo").read_text().splitlines():
+            if line.startswith(("flags", "Features")):
+                flags += line
+                break
+    except OSError:
+        pass
+    try:
+        flags += subprocess.run(["gcc", "-dumpfullversion"], capture_output=True, text=True).stdout
+    except OSError:
+        pass
+    return hashlib.sha1(flags.encode()).hexdigest()[:10]
+
+
 _VARIANTS = {
-    "ld": (_HERE / "liboracle_ld.so", ["-DSC_ORACLE_LONG_DOUBLE"]),
-    "plain": (_HERE / "liboracle_plain.so", []),
+    "ld": (_HERE / "liboracle_ld.so", ["-O2", "-DSC_ORACLE_LONG_DOUBLE"]),
+    "plain": (_HERE / f"liboracle_plain_{_host_tag()}.so", ["-O3", "-march=native"]),
 }
 
 
@@ -36,7 +60,7 @@ def build(force: bool = False) -> None:
     for name, (so, defs) in _VARIANTS.items():
         if not force and so.exists() and so.stat().st_mtime >= _SRC.stat().st_mtime:
             continue
-        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+        cmd = ["gcc", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
                "-fno-fast-math", *defs, str(_SRC), "-o", str(so), "-lm"]
         subprocess.run(cmd, check=True)
 

@@ -7,7 +7,9 @@ from pathlib import Path
 
 PKG = Path(__file__).resolve().parent
 _LIB_PATH = PKG / "libscmd.so"
+_PROBE_LIB_PATH = PKG / "libscmd_probe.so"
 _HEADER = PKG.parent / "include" / "scmd.h"
+_PROBE_HEADER = PKG.parent / "include" / "scmd_probe.h"
 
 SC_OK, SC_ERR_INVALID, SC_ERR_CUDA, SC_ERR_NOMEM, SC_ERR_STATE, SC_ERR_NONFINITE, SC_ERR_CAPACITY = range(7)
 SC_PREC_FP64, SC_PREC_MIXED = 0, 1
@@ -15,6 +17,7 @@ SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN = 0, 1, 2
 (SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
  SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY, SC_OPT_LANGEVIN_STEP, SC_OPT_CELLS_PER_RADIUS,
  SC_OPT_ATOMS_PER_CTA, SC_OPT_NEWTON3, SC_OPT_CUTOFF_SHIFT) = range(1, 12)
+SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX = 100, 101, 102
 _STATUS_NAMES = ["SC_OK", "SC_ERR_INVALID", "SC_ERR_CUDA", "SC_ERR_NOMEM", "SC_ERR_STATE",
                  "SC_ERR_NONFINITE", "SC_ERR_CAPACITY"]
 
@@ -26,6 +29,11 @@ class ScParams(ctypes.Structure):
     _fields_ = [("n", ctypes.c_int32), ("m", ctypes.c_int32), ("eps", ctypes.c_double),
                 ("c", ctypes.c_double), ("a", ctypes.c_double), ("mass", ctypes.c_double),
                 ("r_cut", ctypes.c_double)]
+
+
+class ScCreateOptions(ctypes.Structure):
+    _fields_ = [("neighbour_capacity", ctypes.c_int32), ("newton3_storage", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 6)]
 
 
 class ScThermostat(ctypes.Structure):
@@ -47,9 +55,9 @@ def library_path() -> Path:
     return _LIB_PATH
 
 
-def exported_symbols() -> list[str]:
-    """Function names include/scmd.h declares (parsed from the header)."""
-    text = _HEADER.read_text()
+def exported_symbols(header: Path | None = None) -> list[str]:
+    """Function names include/scmd.h (or the given header) declares (parsed from the header)."""
+    text = (header or _HEADER).read_text()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(sc_[a-z_0-9]+)\s*\(", text)))
 
@@ -68,9 +76,12 @@ def load_library() -> ctypes.CDLL:
     DP, IP = ctypes.POINTER(dbl), ctypes.POINTER(i64)
     sig = {
         "sc_workspace_bytes": (sz, [PP, i64, i32, dbl]),
+        "sc_workspace_bytes_ex": (sz, [PP, i64, i32, dbl, ctypes.POINTER(ScCreateOptions)]),
         "sc_create": (i32, [PP, i64, i32, dbl, vp, sz, vp, ctypes.POINTER(vp)]),
+        "sc_create_ex": (i32, [PP, i64, i32, dbl, ctypes.POINTER(ScCreateOptions), vp, sz, vp, ctypes.POINTER(vp)]),
         "sc_destroy": (i32, [vp]),
         "sc_set_option": (i32, [vp, i32, i64]),
+        "sc_get_option": (i32, [vp, i32, IP]),
         "sc_set_state": (i32, [vp, vp, vp]),
         "sc_get_state": (i32, [vp, vp, vp]),
         "sc_density": (i32, [vp, vp]),
@@ -86,8 +97,6 @@ def load_library() -> ctypes.CDLL:
         "sc_launch_count": (i32, [vp, IP]),
         "sc_profile": (i32, [vp, i32]),
         "sc_profile_read": (i32, [vp, DP, DP]),
-        "sc_probe_throughput": (i32, [i32, vp, vp, sz, DP, DP]),
-        "sc_probe_reciprocal": (i32, [dbl, dbl, i32, vp, vp, sz, DP]),
         "sc_last_error": (ctypes.c_char_p, [vp]),
         "sc_version": (ctypes.c_char_p, []),
     }
@@ -95,6 +104,25 @@ def load_library() -> ctypes.CDLL:
         fn = getattr(L, name)
         fn.restype, fn.argtypes = res, args
     _lib = L
+    return L
+
+
+_probe_lib = None
+
+
+def load_probe_library() -> ctypes.CDLL:
+    """dlopen libscmd_probe.so (include/scmd_probe.h): diagnostics for bench.py and the tests, not the product."""
+    global _probe_lib
+    if _probe_lib is not None:
+        return _probe_lib
+    if not _PROBE_LIB_PATH.exists():
+        raise ScError(SC_ERR_CUDA, "load_probe_library", f"{_PROBE_LIB_PATH} not found: run __graft_entry__.build()")
+    L = ctypes.CDLL(str(_PROBE_LIB_PATH))
+    vp, i32, dbl, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_double, ctypes.c_size_t
+    DP = ctypes.POINTER(dbl)
+    L.sc_probe_throughput.restype, L.sc_probe_throughput.argtypes = i32, [i32, vp, vp, sz, DP, DP]
+    L.sc_probe_reciprocal.restype, L.sc_probe_reciprocal.argtypes = i32, [dbl, dbl, i32, vp, vp, sz, DP]
+    _probe_lib = L
     return L
 
 
@@ -132,7 +160,8 @@ class SuttonChen:
     """One libscmd context: owns a torch workspace tensor and the opaque sc_ctx."""
 
     def __init__(self, n_atoms: int, *, n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0,
-                 precision: int = SC_PREC_FP64, skin: float = 0.0, device=None, stream=None, poison: bool = False):
+                 precision: int = SC_PREC_FP64, skin: float = 0.0, device=None, stream=None, poison: bool = False,
+                 neighbour_capacity: int = 0, newton3_storage: int = 0):
         torch = _torch()
         self.lib = load_library()
         self.n_atoms = int(n_atoms)
@@ -140,8 +169,10 @@ class SuttonChen:
         self.params = ScParams(int(n), int(m), float(eps), float(c), float(a), float(mass), float(r_cut))
         self.precision = int(precision)
         self._ctx = ctypes.c_void_p()
+        opts = ScCreateOptions(int(neighbour_capacity), int(newton3_storage))
         with torch.cuda.device(self.device):
-            nbytes = self.lib.sc_workspace_bytes(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin))
+            nbytes = self.lib.sc_workspace_bytes_ex(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin),
+                                                    ctypes.byref(opts))
             if nbytes == 0:
                 raise ScError(SC_ERR_INVALID, "sc_workspace_bytes", "invalid parameters")
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
@@ -149,8 +180,8 @@ class SuttonChen:
                 self.workspace.fill_(255)    # never read workspace memory it has not written itself
             base = (self.workspace.data_ptr() + 255) // 256 * 256
             self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
-            st = self.lib.sc_create(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin),
-                                    base, nbytes, self.stream.cuda_stream, ctypes.byref(self._ctx))
+            st = self.lib.sc_create_ex(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin),
+                                       ctypes.byref(opts), base, nbytes, self.stream.cuda_stream, ctypes.byref(self._ctx))
         if st != SC_OK:
             self._ctx = ctypes.c_void_p()
             raise ScError(st, "sc_create")
@@ -184,6 +215,11 @@ class SuttonChen:
     # -- the C ABI, name for name ------------------------------------------------------------
     def sc_set_option(self, option: int, value: int):
         self._check(self.lib.sc_set_option(self._ctx, int(option), int(value)), "sc_set_option")
+
+    def sc_get_option(self, option: int) -> int:
+        v = ctypes.c_int64()
+        self._check(self.lib.sc_get_option(self._ctx, int(option), ctypes.byref(v)), "sc_get_option")
+        return v.value
 
     def sc_set_state(self, d_pos, d_vel=None):
         n3 = 3 * self.n_atoms
@@ -288,7 +324,7 @@ def langevin_thermostat(T_start: float, T_end: float, gamma_per_fs: float, seed:
 def probe_throughput(kind: int):
     """-> (thread-level instructions per second, SM clock MHz); see sc_probe_throughput."""
     torch = _torch()
-    L = load_library()
+    L = load_probe_library()
     scratch = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
     v, mhz = ctypes.c_double(), ctypes.c_double()
     st = L.sc_probe_throughput(int(kind), torch.cuda.current_stream().cuda_stream, scratch.data_ptr(), scratch.numel(),
@@ -301,7 +337,7 @@ def probe_throughput(kind: int):
 def probe_reciprocal(lo: float, hi: float, n_samples: int = 1 << 22):
     """-> dict of maximum relative errors of the FP64 reciprocal building blocks."""
     torch = _torch()
-    L = load_library()
+    L = load_probe_library()
     scratch = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
     out = (ctypes.c_double * 4)()
     st = L.sc_probe_reciprocal(float(lo), float(hi), int(n_samples), torch.cuda.current_stream().cuda_stream,

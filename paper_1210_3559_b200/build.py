@@ -10,6 +10,8 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libscmd.so"
+PROBE_SRC = PKG / "csrc_probe" / "scmd_probe.cu"       # diagnostics, a library of their own (include/scmd_probe.h)
+PROBE_LIB = PKG / "libscmd_probe.so"
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v",
@@ -22,11 +24,20 @@ def sources():
 
 
 def needs_build() -> bool:
-    if not LIB.exists():
+    if not LIB.exists() or not PROBE_LIB.exists():
         return True
     cu, deps = sources()
+    probe_deps = [PROBE_SRC, PROBE_SRC.parent / "sc_probe.cuh", PKG.parent / "include" / "scmd_probe.h"]
     newest = max(p.stat().st_mtime for p in cu + deps + [Path(__file__)])
-    return LIB.stat().st_mtime < newest
+    return LIB.stat().st_mtime < newest or PROBE_LIB.stat().st_mtime < max(newest, *(p.stat().st_mtime for p in probe_deps))
+
+
+def build_probe(log_text: list) -> int:
+    """libscmd_probe.so: one translation unit, linked on its own (it shares only csrc/sc_device.cuh with libscmd)."""
+    cmd = ["nvcc", *NVCC_FLAGS, "-shared", str(PROBE_SRC), "-o", str(PROBE_LIB), "-lcudart"]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    log_text.append(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return res.returncode
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
@@ -56,6 +67,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         res = subprocess.run(cmd, capture_output=True, text=True)
         text.append(" ".join(cmd) + "\n" + res.stdout + res.stderr)
         rc = res.returncode
+    if rc == 0:
+        rc = build_probe(text)
     log.write_text("\n".join(text))
     if verbose or rc != 0:
         sys.stderr.write("\n".join(text))

@@ -17,7 +17,7 @@
 // Sums.  part[b][j] (j >= first row of block b: triangular storage) holds block b's reaction sums, self[i] the
 // row sums of i's own block, one per j segment; a finalize kernel adds self[0..][i] + part[0..block(i)][i] in that fixed order, so the
 // result is bit-reproducible.  Storage: ~N^2 / (2 RB) records of 32 bytes (0.54 GB at N = 65536), which is what
-// limits the variant to N <= 131072.
+// limits the variant to N <= 262144 (8.6 GB there; kN3MaxAtoms in scmd.cu).
 #pragma once
 #include "sc_allpairs.cuh"
 #include "sc_device.cuh"

@@ -736,8 +736,11 @@ __global__ void iota_kernel(int *__restrict__ perm, int N) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < N) perm[k] = k;
 }
+// new positions, a new row capacity or a new cell size: the rows are rebuilt at the next evaluation, and an overflow
+// recorded for the old ones says nothing about the new ones
 __global__ void reset_list_state_kernel(unsigned long long *__restrict__ counters, double *__restrict__ scal) {
     counters[kCntListValid] = 0ull;
+    counters[kCntOverflow] = 0ull;
     scal[kSlotMaxDisp2] = 0.0;
 }
 __global__ void zero_u64_kernel(unsigned long long *p) { *p = 0ull; }

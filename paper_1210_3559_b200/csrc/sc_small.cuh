@@ -37,6 +37,7 @@ struct SmallStepArgs {
                             //     phase A of step k + 1 never overwrites records another CTA still stages
     double *vel, *force, *rho;
     FPair *xf;              // MIXED: the packed records of the multi-launch sweeps, refreshed at exit (may be NULL)
+    RecF *xfr;              // MIXED: ... and the split records of the Newton's-third-law sweeps (may be NULL)
     double *part_emb, *part_pair, *part_ke;   // [gridDim.x]
     double *sprime;         // [N] s' of the current step, contiguous (phase C re-stages only these 8 bytes per atom)
     unsigned long long *barrier;      // grid barrier counter; grows by gridDim.x per barrier
@@ -416,6 +417,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         a.rho[i] = my_rho;
         a.xs[i] = make_double4(px, py, pz, sp);             // after the last barrier: nobody stages any more
         if (a.xf) store_split_record(a.xf, i, px, py, pz, float(sp));
+        if (a.xfr) a.xfr[i] = split_record(make_double4(px, py, pz, sp));
     }
     if (t == 0) { a.part_emb[blockIdx.x] = e_emb; a.part_pair[blockIdx.x] = e_pair; }
     grid_sync();

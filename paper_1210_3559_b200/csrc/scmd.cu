@@ -16,7 +16,6 @@
 #include "sc_dispatch.h"
 #include "sc_device.cuh"
 #include "sc_integrate.cuh"
-#include "sc_probe.cuh"
 #include "sc_small.cuh"
 #include "sc_analysis.cuh"
 #include "sc_allpairs_n3.cuh"
@@ -134,6 +133,13 @@ bool params_ok(const sc_params *p) {
            std::isfinite(p->r_cut);
 }
 
+bool create_options_ok(const sc_create_options *o) {
+    if (!o) return true;
+    for (int r : o->reserved)
+        if (r != 0) return false;
+    return o->neighbour_capacity >= 0 && (o->newton3_storage == 0 || o->newton3_storage == 2);
+}
+
 constexpr int kMaxCoopBlocks = 4096;
 
 inline int round_up(int64_t v, int64_t q) { return int((v + q - 1) / q * q); }
@@ -163,7 +169,8 @@ constexpr int kN3RowsPerThread = 4;
 constexpr int kN3MaxSegments = 25;                             // j segments of the longest row block
 
 // one place that lays the workspace out; base == nullptr only measures
-size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin) {
+size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin,
+             const sc_create_options *opt) {
     Carver w(base);
     const size_t n = size_t(N);
     double4 *xs = w.take<double4>(n + kTileAtoms);
@@ -192,7 +199,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         unsigned long long *bar = w.take<unsigned long long>(2);
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
     }
-    if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms) {
+    if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms && !(opt && opt->newton3_storage == 2)) {
         double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
         double4 *ns = w.take<double4>((n + 32) * kN3MaxSegments);
         RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
@@ -203,7 +210,10 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         if (c && base) c->xf = xf;
     }
     if (prm->r_cut > 0.0) {
-        const int kmax = default_kmax(prm, N, skin), md = cutoff_max_dim(N);
+        const int kmax = opt && opt->neighbour_capacity > 0
+                             ? round_up(std::min<int64_t>(opt->neighbour_capacity, std::max<int64_t>(N - 1, 1)), 32)
+                             : default_kmax(prm, N, skin);
+        const int md = cutoff_max_dim(N);
         const size_t ncell = size_t(md) * md * md + 2;
         double4 *xa = w.take<double4>(n + kTileAtoms);
         RecF *xfr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;
@@ -480,11 +490,16 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     return SC_OK;
 }
 
+// all pairs: do the sweeps run the Newton's-third-law kernels (sc_allpairs_n3.cuh) for this context as configured?
+bool n3_wanted(const sc_ctx *c) {
+    if (c->cutoff || !c->n3_part || c->opt_n3 == 2) return false;
+    return c->opt_n3 == 1 || (c->N >= (c->precision == SC_PREC_MIXED ? kN3DefaultMinAtomsMixed : kN3DefaultMinAtoms) &&
+                              !c->opt_it && !c->opt_tpr);
+}
+
 sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     if (c->cutoff) return run_sweep_cutoff(c, force, energy);
-    if (c->n3_part && c->opt_n3 != 2 && (c->opt_n3 == 1 || (c->N >= (c->precision == SC_PREC_MIXED ? kN3DefaultMinAtomsMixed : kN3DefaultMinAtoms) &&
-                            !c->opt_it && !c->opt_tpr)))
-        return run_sweep_n3(c, force, energy);
+    if (n3_wanted(c)) return run_sweep_n3(c, force, energy);
     TileChoice tc = choose_tile(c, force, energy);
     const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);
     if (!fn) return fail(c, SC_ERR_INVALID, "all-pairs sweep: no kernel for this tile shape%s");
@@ -602,7 +617,7 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
         c->small_ctas = c->sm_count;                    // one CTA per SM: the barrier cost grows with the CTA count
     }
     SmallStepArgs a{};
-    a.xs = c->xs; a.xs_b = c->xs_b; a.xf = c->xf; a.vel = c->vel; a.force = c->force; a.rho = c->rho;
+    a.xs = c->xs; a.xs_b = c->xs_b; a.xf = c->xf; a.xfr = c->xfr; a.vel = c->vel; a.force = c->force; a.rho = c->rho;
     a.part_emb = c->part_a; a.part_pair = c->part_b; a.part_ke = c->part_ke; a.scal = c->scal;
     a.sprime = c->sprime; a.barrier = c->small_barrier; a.barrier_base = c->small_barrier_count;
     a.n_atoms = N;
@@ -672,6 +687,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     for (int64_t k = 1; k <= nsteps; ++k) {
         kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, c->cutoff ? c->xs_ref : nullptr,
                                                         c->xf, c->xfr, N, hk, dt);
+        SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
         c->list_checked = false;
@@ -700,8 +716,8 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
             c->launches += 1;
             if (thermo == SC_THERMO_RESCALE) c->lambda_pending = true;
         }
+        SC_CUDA_CHECK(c, cudaGetLastError());       // the integrator launches of this step
     }
-    SC_CUDA_CHECK(c, cudaGetLastError());
     sc_status fl = flush_lambda(c);
     if (fl != SC_OK) return fl;
     return check_flags(c);          // cutoff path only: one synchronisation per sc_step call
@@ -718,22 +734,33 @@ const char *sc_version(void) { return "libscmd 0.1 (sm_100a)"; }
 
 const char *sc_last_error(const sc_ctx *ctx) { return ctx ? ctx->err : "null context"; }
 
-size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t precision, double skin) {
+size_t sc_workspace_bytes_ex(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
+                             const sc_create_options *options) {
     if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return 0;
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
-    if (!(skin >= 0.0)) return 0;
-    return carve(nullptr, nullptr, n_atoms, params, precision, skin);
+    if (!(skin >= 0.0) || !create_options_ok(options)) return 0;
+    return carve(nullptr, nullptr, n_atoms, params, precision, skin, options);
+}
+
+size_t sc_workspace_bytes(const sc_params *params, int64_t n_atoms, int32_t precision, double skin) {
+    return sc_workspace_bytes_ex(params, n_atoms, precision, skin, nullptr);
 }
 
 sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision, double skin, void *d_workspace,
                     size_t workspace_bytes, void *cuda_stream, sc_ctx **out) {
+    return sc_create_ex(params, n_atoms, precision, skin, nullptr, d_workspace, workspace_bytes, cuda_stream, out);
+}
+
+sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precision, double skin,
+                       const sc_create_options *options, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                       sc_ctx **out) {
     if (!out) return SC_ERR_INVALID;
     *out = nullptr;
     if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return SC_ERR_INVALID;
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return SC_ERR_INVALID;
-    if (!(skin >= 0.0) || !d_workspace) return SC_ERR_INVALID;
+    if (!(skin >= 0.0) || !d_workspace || !create_options_ok(options)) return SC_ERR_INVALID;
     if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
-    const size_t need = sc_workspace_bytes(params, n_atoms, precision, skin);
+    const size_t need = sc_workspace_bytes_ex(params, n_atoms, precision, skin, options);
     if (workspace_bytes < need) return SC_ERR_NOMEM;
     int dev = 0, count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) return SC_ERR_CUDA;
@@ -743,7 +770,7 @@ sc_status sc_create(const sc_params *params, int64_t n_atoms, int32_t precision,
     c->p = *params; c->N = n_atoms; c->precision = precision; c->skin = skin;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    carve(c, d_workspace, n_atoms, params, precision, skin);
+    carve(c, d_workspace, n_atoms, params, precision, skin, options);
     const double a_n = ipow_host(params->a, params->n), a_m = ipow_host(params->a, params->m);
     c->consts.am = a_m;
     c->consts.An = params->eps * params->n * a_n;
@@ -827,6 +854,8 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
                 c->kmax = value ? (value < 32 ? 32 : int(value) / 32 * 32) : c->kmax_cap;   // rows are padded to 32
                 c->list_checked = false;
                 reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
+                SC_CUDA_CHECK(c, cudaGetLastError());
+                c->launches += 1;
                 c->density_valid = c->forces_valid = c->energy_valid = false;
             }
             break;
@@ -839,6 +868,8 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
             if (c->cutoff) {
                 c->list_checked = false;
                 reset_list_state_kernel<<<1, 1, 0, c->stream>>>(c->counters, c->scal);
+                SC_CUDA_CHECK(c, cudaGetLastError());
+                c->launches += 1;
                 c->density_valid = c->forces_valid = c->energy_valid = false;
             }
             break;
@@ -859,6 +890,31 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
             return fail(c, SC_ERR_INVALID, "unknown option%s");
     }
     if (c->opt_it == 4 && c->opt_tpr > 4) return fail(c, SC_ERR_INVALID, "4 rows per thread needs lanes per row <= 4%s");
+    return SC_OK;
+}
+
+sc_status sc_get_option(sc_ctx *c, int32_t option, int64_t *value) {
+    if (!c || !value) return fail(c, SC_ERR_INVALID, "sc_get_option: NULL argument%s");
+    switch (option) {
+        case SC_OPT_ROWS_PER_THREAD: *value = c->opt_it; break;
+        case SC_OPT_LANES_PER_ROW: *value = c->opt_tpr; break;
+        case SC_OPT_WARPS_PER_CTA: *value = c->opt_warps; break;
+        case SC_OPT_PERSISTENT: *value = c->opt_persistent; break;
+        case SC_OPT_ENERGY_EVERY_STEP: *value = c->opt_energy_every; break;
+        case SC_OPT_NEIGHBOUR_CAPACITY: *value = c->opt_kmax; break;
+        case SC_OPT_LANGEVIN_STEP: *value = int64_t(c->langevin_step); break;
+        case SC_OPT_CELLS_PER_RADIUS: *value = c->opt_fine; break;
+        case SC_OPT_ATOMS_PER_CTA: *value = c->opt_apc; break;
+        case SC_OPT_NEWTON3: *value = c->opt_n3; break;
+        case SC_OPT_CUTOFF_SHIFT: *value = c->opt_shift; break;
+        case SC_INFO_STEP_PATH:
+            *value = c->cutoff ? 3 : (small_path_wanted(c) ? 2 : (n3_wanted(c) ? 1 : 0));
+            break;
+        case SC_INFO_NEIGHBOUR_CAPACITY: *value = c->cutoff ? c->kmax : 0; break;
+        case SC_INFO_NEIGHBOUR_CAPACITY_MAX: *value = c->cutoff ? c->kmax_cap : 0; break;
+        default:
+            return fail(c, SC_ERR_INVALID, "sc_get_option: unknown option%s");
+    }
     return SC_OK;
 }
 
@@ -1130,68 +1186,6 @@ sc_status sc_profile_read(sc_ctx *c, double *h_ms_density, double *h_ms_force) {
         return fail(c, SC_ERR_STATE, "sc_profile_read: no profiled sweep recorded%s");
     if (h_ms_density) *h_ms_density = a;
     if (h_ms_force) *h_ms_force = b;
-    return SC_OK;
-}
-
-sc_status sc_probe_throughput(int32_t kind, void *cuda_stream, void *d_scratch, size_t scratch_bytes,
-                              double *h_inst_per_s, double *h_sm_clock_mhz) {
-    if (kind < 0 || kind > 8 || !d_scratch || !h_inst_per_s) return SC_ERR_INVALID;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int grid = sms * 8, block = 256;
-    if (scratch_bytes < sizeof(double) * 8 + sizeof(long long) * size_t(grid)) return SC_ERR_NOMEM;
-    double *out = static_cast<double *>(d_scratch);
-    long long *cyc = reinterpret_cast<long long *>(out + 8);
-    const int iters = (kind == 3 || kind == 4) ? 2048 : 16384;
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return SC_ERR_CUDA;
-    auto run = [&](int it) {
-        switch (kind) {
-            case 0: probe_kernel<0><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 1: probe_kernel<1><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 2: probe_kernel<2><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 3: probe_kernel<3><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 4: probe_kernel<4><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 5: probe_kernel<5><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 6: probe_kernel<6><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            case 7: probe_kernel<7><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-            default: probe_kernel<8><<<grid, block, 0, st>>>(out, cyc, it, 1.0); break;
-        }
-    };
-    run(iters / 8);   // warm-up
-    run(iters);
-    cudaEventRecord(e0, st);
-    run(iters);
-    cudaEventRecord(e1, st);
-    sc_status rc = SC_OK;
-    float ms = 0.f;
-    long long cycles0 = 0;
-    if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess ||
-        cudaMemcpy(&cycles0, cyc, sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess)
-        rc = SC_ERR_CUDA;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (rc != SC_OK) return rc;
-    const double per_thread = double(iters) * kProbeChains * ((kind == 2 || kind == 7 || kind == 8) ? 2.0 : 1.0);
-    *h_inst_per_s = per_thread * double(grid) * block / (double(ms) * 1e-3);
-    // a block's own span in SM cycles; 8 blocks per SM run concurrently, so span ~ kernel time
-    if (h_sm_clock_mhz) *h_sm_clock_mhz = double(cycles0) / (double(ms) * 1e3);
-    return SC_OK;
-}
-
-sc_status sc_probe_reciprocal(double lo, double hi, int32_t n_samples, void *cuda_stream, void *d_scratch,
-                              size_t scratch_bytes, double *h_err4) {
-    if (!(lo > 0.0) || !(hi > lo) || n_samples < 1 || !d_scratch || scratch_bytes < 4 * sizeof(double) || !h_err4)
-        return SC_ERR_INVALID;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double *out = static_cast<double *>(d_scratch);
-    if (cudaMemsetAsync(out, 0, 4 * sizeof(double), st) != cudaSuccess) return SC_ERR_CUDA;
-    reciprocal_error_kernel<<<296, 256, 0, st>>>(lo, hi, n_samples, out);
-    if (cudaGetLastError() != cudaSuccess) return SC_ERR_CUDA;
-    if (cudaMemcpyAsync(h_err4, out, 4 * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess) return SC_ERR_CUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return SC_ERR_CUDA;
     return SC_OK;
 }
 

@@ -1,8 +1,9 @@
-// sc_probe.cuh -- register-only throughput probes (sc_probe_throughput): dependent FMA chains
+// sc_probe.cuh -- kernels of libscmd_probe.so (include/scmd_probe.h), a diagnostics library that only bench.py and
+// the tests load; not part of libscmd.  Register-only throughput probes (sc_probe_throughput): dependent FMA chains
 // with 8-way ILP per thread, one wave of resident CTAs on every SM.  Gives the measured figure
 // that bench.py prints beside the nominal ALU peak, and the SM clock held under that load.
 #pragma once
-#include "sc_device.cuh"
+#include "../csrc/sc_device.cuh"
 
 namespace scmd {
 

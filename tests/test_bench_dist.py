@@ -76,3 +76,53 @@ def test_reference_arm_prints_one_json_line_and_other_ranks_stay_silent():
     out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0"],
                          capture_output=True, text=True, env=dict(env, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1"), timeout=60)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_gpus_flag_starts_the_ranks_itself(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun re-executes itself under torch.distributed.run with N ranks
+    (one per GPU) on 127.0.0.1; under torchrun it must find WORLD_SIZE == N."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    calls = []
+
+    class Done:
+        returncode = 0
+
+    def fake_run(cmd, env=None, **kw):
+        calls.append((cmd, env))
+        return Done()
+
+    monkeypatch.setattr(bench.subprocess, "run", fake_run)
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK"):
+        monkeypatch.delenv(k, raising=False)
+    with pytest.raises(SystemExit) as ei:
+        bench.main(["--gpus", "4", "--steps", "7", "--warmup", "3"])
+    assert ei.value.code == 0 and len(calls) == 1
+    cmd, env = calls[0]
+    assert cmd[:3] == [sys.executable, "-m", "torch.distributed.run"]
+    assert "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-6:] == ["--gpus", "4", "--steps", "7", "--warmup", "3"] and cmd[-7].endswith("bench.py")
+    assert "NCCL_DEBUG" in env
+    # under torchrun with the wrong world size: refuse rather than mislabel the line
+    monkeypatch.setenv("WORLD_SIZE", "2"); monkeypatch.setenv("RANK", "0"); monkeypatch.setenv("LOCAL_RANK", "0")
+    with pytest.raises(SystemExit) as ei:
+        bench.main(["--gpus", "4"])
+    assert "WORLD_SIZE" in str(ei.value.code)
+
+
+def test_reference_arm_under_torchrun_world2():
+    """The driver's launch of the reference arm at N = 2: torchrun starts two ranks, rank 0 alone runs and prints."""
+    env = dict(os.environ, OMP_NUM_THREADS="4")
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK"):
+        env.pop(k, None)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), str(ROOT / "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+           "--warmup", "0", "--workload", "Ni1415-fcc-allpairs-fp64"]
+    out = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["config"]["n_atoms"] == 1415
+    assert set(d["config"]) >= {"workload", "n_atoms", "pairs_per_step", "r_cut", "skin", "parallelism", "step"}

@@ -111,17 +111,56 @@ def test_evaporated_atoms_and_generic_exponents(scmd, oracle_ld):
     check(scmd, oracle_ld, pos, 7.0, n=7, m=3, eps=0.02, c=30.0, a=3.3, precision=1)
 
 
-def test_capacity_overflow_is_reported(scmd):
+def test_capacity_overflow_is_reported_and_recoverable(scmd, oracle_ld):
+    """A row longer than its capacity is reported (never truncated); raising the capacity, or new positions, clears
+    the condition: the next evaluation rebuilds the rows and is correct."""
     import torch
     w = W.config_c2()
+    P = oracle_ld.params(r_cut=10.0)
+    _, f_o, (e_o, _, _) = oracle_ld.energy_forces(w.pos, P)
     sc = scmd.SuttonChen(1415, r_cut=10.0, skin=1.0)
+    cap_max = sc.sc_get_option(scmd.SC_INFO_NEIGHBOUR_CAPACITY_MAX)
     sc.sc_set_option(scmd.SC_OPT_NEIGHBOUR_CAPACITY, 64)
+    assert sc.sc_get_option(scmd.SC_INFO_NEIGHBOUR_CAPACITY) == 64
     sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"))
     with pytest.raises(scmd.ScError) as ei:
         sc.sc_energy()
     assert ei.value.status == 6                                        # SC_ERR_CAPACITY
     with pytest.raises(scmd.ScError):
         sc.sc_set_option(scmd.SC_OPT_NEIGHBOUR_CAPACITY, 1 << 20)      # beyond what the workspace holds
+    sc.sc_set_option(scmd.SC_OPT_NEIGHBOUR_CAPACITY, 0)                # back to what the workspace was sized for
+    assert sc.sc_get_option(scmd.SC_INFO_NEIGHBOUR_CAPACITY) == cap_max
+    assert rel(sc.sc_energy(), e_o) < 1e-12 and rel_l2(sc.sc_forces().cpu().numpy(), f_o) < 1e-10
+    assert sc.sc_stats()["n_rebuilds"] == 2
+    # overflow again, then sparser positions (2 atoms per row at most) under the same small capacity
+    sc.sc_set_option(scmd.SC_OPT_NEIGHBOUR_CAPACITY, 64)
+    with pytest.raises(scmd.ScError):
+        sc.sc_energy()
+    far = w.pos * 4.0
+    sc.sc_set_state(torch.as_tensor(far, device="cuda"))
+    assert rel(sc.sc_energy(), oracle_ld.energy(far, P)) < 1e-12
+    sc.close()
+
+
+def test_dense_system_needs_a_create_time_capacity(scmd, oracle_ld):
+    """1.9 x the fcc density (lattice compressed to 0.807 a): the default rows (1.3 x fcc) overflow; a context created
+    with the capacity sc_stats reported evaluates it (sc_create_ex / sc_create_options.neighbour_capacity)."""
+    import torch
+    pos = W.fcc_cluster(3000, 300.0, seed=41).pos * 0.807
+    P = oracle_ld.params(r_cut=10.0)
+    _, f_o, (e_o, _, _) = oracle_ld.energy_forces(pos, P)
+    sc = scmd.SuttonChen(3000, r_cut=10.0, skin=1.0)
+    sc.sc_set_state(torch.as_tensor(pos, device="cuda"))
+    with pytest.raises(scmd.ScError) as ei:
+        sc.sc_energy()
+    assert ei.value.status == 6
+    sc.close()
+    sc = scmd.SuttonChen(3000, r_cut=10.0, skin=1.0, neighbour_capacity=1100)
+    assert sc.sc_get_option(scmd.SC_INFO_NEIGHBOUR_CAPACITY) == 1120    # rounded up to a multiple of 32
+    sc.sc_set_state(torch.as_tensor(pos, device="cuda"))
+    assert rel(sc.sc_energy(), e_o) < 1e-12 and rel_l2(sc.sc_forces().cpu().numpy(), f_o) < 1e-10
+    stats = sc.sc_stats()
+    assert 672 < stats["max_neighbours"] <= 1100 and stats["n_pairs_in_cut"] == oracle_ld.count_pairs(pos, 10.0)
     sc.close()
 
 
@@ -225,19 +264,4 @@ def test_c4_ni65536_rc10_full_size(scmd, c4_cut_oracle, precision):
     assert rel(e, e_o) < ENERGY_TOL[precision]
 
 
-def test_n2pow20_sampled_rows(scmd, oracle_ld):
-    """The largest sweep size (N = 1,048,576): sampled rows against the oracle, plus the invariants
-    that hold at any size (net force ~ 0, pair count symmetric => even)."""
-    w = W.config_c5(10)
-    sc, rho, f, e = gpu_eval(scmd, w.pos, r_cut=10.0, skin=1.0)
-    stats = sc.sc_stats()
-    sc.close()
-    rows = np.unique(np.linspace(0, w.n_atoms - 1, 48).astype(np.int64))
-    P = oracle_ld.params(r_cut=10.0)
-    rho_rows = oracle_ld.density_rows(w.pos, P, rows)
-    assert np.max(np.abs(rho[rows] - rho_rows) / rho_rows) < 1e-12
-    f_rows, _ = oracle_ld.forces_rows(w.pos, P, rho, rows)
-    assert rel_l2(f[rows], f_rows) < 1e-10
-    assert stats["n_pairs_in_cut"] % 2 == 0
-    assert np.abs(f.sum(axis=0)).max() < 1e-9 * np.abs(f).sum()
-    assert -4.45 < e / w.n_atoms < -4.30                                # approaches the bulk -4.4401 eV
+# the largest sweep sizes (N = 262144 and 2^20) are in tests/test_gpu_large.py

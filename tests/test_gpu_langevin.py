@@ -82,6 +82,15 @@ def test_langevin_limits_and_errors(scmd):
         sc.sc_step(1.0, 1, langevin_thermostat(-5.0, 300.0, 0.01, 1))
     with pytest.raises(scmd.ScError):
         sc.sc_set_option(scmd.SC_OPT_LANGEVIN_STEP, -1)
+    # the generator step is readable (exact resume without the caller counting): one-launch loop and multi-launch path
+    assert sc.sc_get_option(scmd.SC_OPT_LANGEVIN_STEP) == 0
+    sc.sc_step(1.0, 7, langevin_thermostat(300.0, 300.0, 0.01, 1))
+    assert sc.sc_get_option(scmd.SC_OPT_LANGEVIN_STEP) == 7
+    sc.sc_set_option(scmd.SC_OPT_PERSISTENT, 2)
+    sc.sc_step(1.0, 5, langevin_thermostat(300.0, 300.0, 0.01, 1))
+    assert sc.sc_get_option(scmd.SC_OPT_LANGEVIN_STEP) == 12
+    sc.sc_step(1.0, 3)                                                  # NVE steps do not advance it
+    assert sc.sc_get_option(scmd.SC_OPT_LANGEVIN_STEP) == 12
     sc.close()
 
 

@@ -140,3 +140,21 @@ def test_c4_ni65536_full_size_mixed(scmd, oracle_ld):
     errs = (float(np.max(np.abs(rho - rho_o) / rho_o)), rel_l2(f, f_o), rel(e, e_o))
     print("mixed N=65536 errors (rho max, force L2, energy):", errs)
     assert errs[0] < RHO_TOL and errs[1] < FORCE_TOL and errs[2] < ENERGY_TOL, errs
+
+
+def test_split_records_refreshed_by_the_one_launch_loop(scmd, oracle_ld):
+    """Mixed N = 2057 (the one-launch loop by default): after sc_step, switching the sweeps to Newton's third law
+    (which read the RecF split records) and re-evaluating WITHOUT new positions must see the stepped positions."""
+    import torch
+    w = W.mackay_cluster(8, 1000.0, 1001)
+    sc = scmd.SuttonChen(w.n_atoms, precision=scmd.SC_PREC_MIXED)
+    sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"), torch.as_tensor(w.vel, device="cuda"))
+    assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == 2
+    sc.sc_step(1.0, 25)
+    pos, _ = sc.sc_get_state()
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3, 1)                           # invalidates forces, repacks nothing
+    f = sc.sc_forces().cpu().numpy()
+    e = sc.sc_energy()
+    sc.close()
+    _, f_o, (e_o, _, _) = oracle_ld.energy_forces(pos.cpu().numpy(), oracle_ld.params())
+    assert rel_l2(f, f_o) < FORCE_TOL and rel(e, e_o) < ENERGY_TOL
