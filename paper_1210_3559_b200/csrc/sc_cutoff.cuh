@@ -2,15 +2,21 @@
 // cutoffs as work in progress): cell binning by counting sort, Verlet neighbour
 // rows with a skin, and the two list-driven sweeps.
 //
-// Design constraint (measured, profiles/ncu_cutoff_r1.md): a list-driven FP64 sweep on sm_100a is
-// bound by L1 wavefronts (one per distinct 128-byte line a warp-wide gather touches), not by the
-// FP64 pipe, unless the 32 lanes of a warp gather ADJACENT records.  Hence:
+// Design constraints (measured, profiles/ncu_cutoff_r1.md, profiles/ncu_cutoff_r2.md): a list-driven FP64 sweep on
+// sm_100a is bound by the FP64 pipe only if (i) the 32 lanes of a warp gather ADJACENT records (one L1 wavefront
+// per distinct 128-byte line), (ii) every fetched record is used for more than one row i, and (iii) the index
+// stream does not come from DRAM one 4-byte entry per pair (round 1: 78 MB per sweep at N = 65536, 25x the
+// algorithmic bytes, and a dependent DRAM -> L2 load chain in the hot loop).  Hence:
 //   * atoms are sorted into FINE cells (edge = list radius / G, G = 4 by default), x fastest, so the
 //     in-range neighbours of an atom are ~60 contiguous runs of the internal order;
-//   * one WARP walks one neighbour row (rows are row-major, ascending in j, padded to a multiple of
-//     32 with the index of a dummy record at infinity): index loads are 128 contiguous bytes and a
-//     record gather touches ~1 line per 3 entries;
-//   * records are fetched with one 256-bit load (SASS LDG.E.ENL2.256).
+//   * a neighbour row belongs to a PAIR of consecutive atoms (the union of their neighbourhoods, ~1.2x one
+//     of them) and is stored RUN-LENGTH encoded: one 32-bit word (first index << 5 | length - 1) per run of
+//     up to 32 consecutive atoms -- ~70-90 words instead of ~560 entries per row (N = 65536: ~10 MB instead
+//     of 74 MB, L2-resident);
+//   * one WARP walks one row: it expands the runs into a shared-memory index list (a warp scan and a few
+//     stores per 32 runs), then works through it in dense batches of 32 entries, lane t taking entry
+//     32 b + t: adjacent lanes gather adjacent records with one 256-bit load each (SASS LDG.E.ENL2.256) and
+//     evaluate them against both atoms of the pair; the index stream never touches DRAM in the loop.
 //
 // rebuild_kernel: ONE cooperative launch per force evaluation.  It reads the device-side skin
 // criterion (largest squared displacement since the last build, written by kick_drift_kernel) and
@@ -28,19 +34,19 @@
 //       floating-point sum runs in an order that does not depend on atomics)
 //   P6  permute records, velocities, perm into cell order (into the alternate buffers)
 //   P7  copy back; the records at the build become the reference for the skin criterion
-//   P8  neighbour rows, one warp per atom: for each of the <= (2G+1)^2 rows of cells in y, z the
-//       x-run of cells that can hold a neighbour is one contiguous range of the internal order; the
-//       warp tests 32 candidates at a time and appends, in order, every j != k with
-//       r^2 < (r_c + skin)^2; rows never truncate silently (overflow flag -> SC_ERR_CAPACITY)
+//   P8  neighbour rows, one warp per atom pair: the <= (2G+1)^2 rows of cells in (y, z) that can hold a
+//       neighbour each contribute ONE contiguous index range; the ranges are computed 32 at a time (one per
+//       lane, all cell_start loads in flight together), expanded into a shared-memory candidate list and
+//       tested in dense batches of 32 candidates; every j within r_c + skin of EITHER atom goes into the row,
+//       as runs (ballot + bit scans); rows never truncate silently (overflow flag -> SC_ERR_CAPACITY)
 // After a build the library's internal atom order IS the cell order; perm[k] = caller's index.
 //
-// nlist_kernel: LPA lanes (32 by default) walk one row, gather the 32-byte record of j, apply the
-// strict binary64 test r^2 < r_c^2 (reading Q7: same decision value as the oracle) and accumulate
-// the same pair terms as the all-pairs sweeps.  MIXED: the rows gather split binary32 records (x = xh + xl)
-// and the whole pair term runs in binary32 -- no conversion, no binary64 instruction -- except that an entry
-// whose binary32 r^2 lies within 2e-6 r_c^2 of the cutoff takes its set-membership decision from the binary64
-// records (reading Q7: membership is the oracle's, bit for bit); partial sums are flushed into binary64 after
-// every batch.
+// nlist_kernel: applies the strict binary64 test r^2 < r_c^2 (reading Q7: same decision value as the oracle) to
+// every entry and accumulates the same pair terms as the all-pairs sweeps.  MIXED: the rows gather split binary32
+// records (x = xh + xl) and the whole pair term runs in binary32 -- no conversion, no binary64 instruction -- except
+// that an entry whose binary32 r^2 lies within 2e-6 r_c^2 of the cutoff takes its set-membership decision from the
+// binary64 records (reading Q7: membership is the oracle's, bit for bit); partial sums are flushed into binary64
+// after every batch.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -60,6 +66,12 @@ enum CounterSlot {
     kNumCounters = 8
 };
 
+constexpr bool kListRuns = true;  // rows as run-length words (true) or as one 32-bit index per entry (false): measured, DESIGN.md 6.3
+constexpr int kRunBits = 3;      // a run word = first index << kRunBits | (length - 1): runs of 1 .. 8 atoms (short runs keep
+                                 // the expansion loop of the sweeps short: every lane writes out one run)
+constexpr int kRunMaxLen = 1 << kRunBits;
+constexpr int64_t kCutoffMaxAtoms = int64_t(1) << (32 - kRunBits);   // first index must fit in 29 bits
+constexpr int kCandCap = 1024;   // rebuild P8: candidates expanded per chunk of 32 cell-row ranges, per warp
 constexpr int kFineMax = 4;      // G_max: fine cells per list radius (the grid falls back to coarser cells
                                  // when the fine grid would exceed the cell budget)
 constexpr double kFarAway = 1.0e150;   // coordinates of the dummy record that pads every neighbour row
@@ -81,7 +93,7 @@ struct RebuildArgs {
     int *cell_of, *slot_of, *cell_sorted;
     int *cell_count, *cell_start;   // [ncell_max + 1]
     int *order_tmp, *order;
-    int *nlist, *ncount;            // pair rows: nlist[g * 2 kmax + e], g = k / 2; padded with n_atoms to a multiple of 32
+    int *nlist, *ncount;            // pair rows g = k / 2: nlist[g * 2 kmax + r] = run r (start << 5 | len - 1), ncount[g] runs
     double *blockpart;              // [9 * gridDim.x]
     int *scanpart;                  // [gridDim.x + 1]
     CellGrid *grid;
@@ -305,13 +317,15 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
     // ---- P8: neighbour rows, one warp per PAIR of consecutive atoms (k0 = 2g, k1 = 2g + 1) ----
     // The row of a pair is the union of the two atoms' neighbourhoods (they sit in the same or in
     // adjacent fine cells, so the union is ~1.2x one neighbourhood): the sweeps fetch every record once
-    // for two rows i.  Capacity of a pair row: 2 * kmax entries.
+    // for two rows i.  Stored as runs of consecutive indices; capacity of a pair row: 2 * kmax words.
     const double rl2 = a.r_list * a.r_list;
     const double rl2_cells = rl2 * g.inv_edge * g.inv_edge;           // (list radius / edge)^2
     const int G = g.fine;
     // reach[ady][adz]: how many cells along x a neighbour can be away in a row of cells whose nearest points
     // are (ady, adz) cells away in y, z (-1: the row is out of reach)
     __shared__ int reach[kFineMax + 1][kFineMax + 1];
+    __shared__ int cand_all[8][kCandCap];
+    int *cand = cand_all[warp];
     if (tid < (kFineMax + 1) * (kFineMax + 1)) {
         const int ady = tid / (kFineMax + 1), adz = tid % (kFineMax + 1);
         const double rem = rl2_cells - double(adz * adz + ady * ady);
@@ -333,7 +347,10 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
         const int cx0 = c0 % g.nx, cy0 = (c0 / g.nx) % g.ny, cz0 = c0 / (g.nx * g.ny);
         const int cx1 = c1 % g.nx, cy1 = (c1 / g.nx) % g.ny, cz1 = c1 / (g.nx * g.ny);
         int *row = a.nlist + size_t(gp) * cap;
-        int cnt = 0, cnt0 = 0, cnt1 = 0;
+        // the row holds neither k0 nor k1: the sweeps add the term between the two themselves, in a free lane of the
+        // row's last batch, so no entry is ever an atom's own record and no sweep compares indices (the self term is
+        // excluded by index, reading Q11 -- here, once, at the build)
+        int nruns = 0, cnt0 = 0, cnt1 = 0;
         // x-range of cells of the row (yy, zz) that can hold a neighbour of an atom in cell (cx, cy, cz)
         auto xrange = [&](int cx, int cy, int cz, int yy, int zz, int &lo, int &hi) -> bool {
             if (abs(zz - cz) > G || abs(yy - cy) > G) return false;
@@ -342,64 +359,119 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
             lo = max(cx - mx, 0); hi = min(cx + mx, g.nx - 1);
             return true;
         };
-        auto scan = [&](int jb, int je) {
-            for (int j0 = jb; j0 < je; j0 += 32) {
-                const int j = j0 + lane;
-                bool in0 = false, in1 = false;
-                if (j < je) {
-                    const double4 q = a.xs[j];
-                    const double ax = p0.x - q.x, ay = p0.y - q.y, az = p0.z - q.z;
-                    const double bx = p1.x - q.x, by = p1.y - q.y, bz = p1.z - q.z;
-                    in0 = fma(az, az, fma(ay, ay, ax * ax)) < rl2;
-                    in1 = fma(bz, bz, fma(by, by, bx * bx)) < rl2;
+        // 32 candidates (consecutive entries of the candidate list; `valid` lanes only): distance tests against
+        // both atoms, then the accepted ones are appended to the row as runs of consecutive indices (never across a
+        // batch, never longer than kRunMaxLen).
+        auto batch = [&](int j, bool valid) {
+            bool in0 = false, in1 = false;
+            if (valid) {
+                const double4 q = a.xs[j];
+                const double ax = p0.x - q.x, ay = p0.y - q.y, az = p0.z - q.z;
+                const double bx = p1.x - q.x, by = p1.y - q.y, bz = p1.z - q.z;
+                in0 = fma(az, az, fma(ay, ay, ax * ax)) < rl2;
+                in1 = fma(bz, bz, fma(by, by, bx * bx)) < rl2;
+            }
+            const bool ok = (in0 || in1) && j != k0 && j != k1;         // never the pair itself (see above)
+            const int pj = __shfl_up_sync(0xffffffffu, j, 1);
+            const int pok = __shfl_up_sync(0xffffffffu, ok ? 1 : 0, 1);
+            const bool fresh = ok && (lane == 0 || !pok || pj != j - 1);       // a run of consecutive indices begins here
+            const unsigned fm = __ballot_sync(0xffffffffu, fresh);
+            // runs are cut after kRunMaxLen entries: position inside the run = lane - (last `fresh` lane at or before it)
+            const int since = lane - (31 - __clz(int(fm & (0xffffffffu >> (31 - lane)))));
+            const bool start = ok && (fresh || (since & (kRunMaxLen - 1)) == 0);
+            const unsigned s = __ballot_sync(0xffffffffu, start), o = __ballot_sync(0xffffffffu, ok);
+            if constexpr (kListRuns) {
+                if (start) {
+                    const unsigned cont = o & ~s;                        // lanes that continue the run of the lane before
+                    const unsigned x = lane == 31 ? 0u : (cont >> (lane + 1));
+                    const int len = __ffs(int(~x));                      // 1 + number of continuation lanes that follow
+                    const int at = nruns + __popc(s & lt_mask);
+                    if (at < cap) row[at] = int((unsigned(j) << kRunBits) | unsigned(len - 1));
                 }
-                const bool ok = in0 || in1;                             // includes k0 and k1 themselves: excluded
-                const unsigned m = __ballot_sync(0xffffffffu, ok);      // by index in the sweeps
-                const int at = cnt + __popc(m & lt_mask);
+                nruns += __popc(s);
+            } else {
+                const int at = nruns + __popc(o & lt_mask);              // one word per entry, ascending
                 if (ok && at < cap) row[at] = j;
-                cnt += __popc(m);
-                cnt0 += (in0 && j != k0) ? 1 : 0;                       // per lane; summed over the warp below
-                cnt1 += (in1 && j != k1) ? 1 : 0;
+                nruns += __popc(o);
+            }
+            cnt0 += (in0 && j != k0) ? 1 : 0;                            // per lane; summed over the warp below
+            cnt1 += (in1 && j != k1) ? 1 : 0;
+        };
+        // one contiguous index range per row of cells; ranges are computed 32 at a time (one per lane), expanded
+        // into the candidate list of this warp and tested in dense batches
+        auto sweep_box = [&](int ylo, int yhi, int zlo, int zhi, int which) {
+            const int nyb = yhi - ylo + 1, R = nyb * (zhi - zlo + 1);
+            for (int r0 = 0; r0 < R; r0 += 32) {
+                const int r = r0 + lane;
+                int jb = 0, len = 0;
+                if (r < R) {
+                    const int zz = zlo + r / nyb, yy = ylo + r % nyb;
+                    int lo0 = 0, hi0 = -1, lo1 = 0, hi1 = -1;
+                    const bool v0 = which != 1 && xrange(cx0, cy0, cz0, yy, zz, lo0, hi0);
+                    const bool v1 = which != 0 && has1 && xrange(cx1, cy1, cz1, yy, zz, lo1, hi1);
+                    if (v0 || v1) {
+                        const int lo = v0 ? (v1 ? min(lo0, lo1) : lo0) : lo1;
+                        const int hi = v0 ? (v1 ? max(hi0, hi1) : hi0) : hi1;
+                        const int rowc = (zz * g.ny + yy) * g.nx;
+                        jb = a.cell_start[rowc + lo];
+                        len = a.cell_start[rowc + hi + 1] - jb;
+                    }
+                }
+                int incl = len;
+#pragma unroll
+                for (int off = 1; off < 32; off <<= 1) {
+                    const int v = __shfl_up_sync(0xffffffffu, incl, off);
+                    if (lane >= off) incl += v;
+                }
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                if (total == 0) continue;
+                if (total <= kCandCap) {
+                    int longest = len;
+#pragma unroll
+                    for (int off = 16; off > 0; off >>= 1) longest = max(longest, __shfl_xor_sync(0xffffffffu, longest, off));
+                    const int base = incl - len;
+                    for (int k = 0; k < longest; ++k)
+                        if (k < len) cand[base + k] = jb + k;
+                    __syncwarp();
+                    for (int q0 = 0; q0 < total; q0 += 32) {
+                        const int q = q0 + lane;
+                        const bool valid = q < total;
+                        batch(valid ? cand[q] : 0, valid);
+                    }
+                    __syncwarp();
+                } else {
+                    // very long ranges (clamped boundary cells, compressed matter): range by range
+                    for (int rr = 0; rr < 32; ++rr) {
+                        const int jb_r = __shfl_sync(0xffffffffu, jb, rr), len_r = __shfl_sync(0xffffffffu, len, rr);
+                        for (int t0 = 0; t0 < len_r; t0 += 32) batch(jb_r + t0 + lane, t0 + lane < len_r);
+                    }
+                }
             }
         };
         const bool near = abs(cx0 - cx1) <= 2 * G && abs(cy0 - cy1) <= 2 * G && abs(cz0 - cz1) <= 2 * G;
         if (near) {
             // one pass over the bounding box of the two stencils, each row of cells once
-            for (int zz = max(min(cz0, cz1) - G, 0); zz <= min(max(cz0, cz1) + G, g.nz - 1); ++zz)
-                for (int yy = max(min(cy0, cy1) - G, 0); yy <= min(max(cy0, cy1) + G, g.ny - 1); ++yy) {
-                    int lo0, hi0, lo1, hi1;
-                    const bool v0 = xrange(cx0, cy0, cz0, yy, zz, lo0, hi0);
-                    const bool v1 = has1 && xrange(cx1, cy1, cz1, yy, zz, lo1, hi1);
-                    if (!v0 && !v1) continue;
-                    const int lo = v0 ? (v1 ? min(lo0, lo1) : lo0) : lo1;
-                    const int hi = v0 ? (v1 ? max(hi0, hi1) : hi0) : hi1;
-                    const int rowc = (zz * g.ny + yy) * g.nx;
-                    scan(a.cell_start[rowc + lo], a.cell_start[rowc + hi + 1]);
-                }
+            sweep_box(max(min(cy0, cy1) - G, 0), min(max(cy0, cy1) + G, g.ny - 1), max(min(cz0, cz1) - G, 0),
+                      min(max(cz0, cz1) + G, g.nz - 1), 2);
         } else {
             // the stencils are disjoint (the pair straddles the end of a row of cells): one pass each
-            for (int which = 0; which < 2; ++which) {
-                const int cx = which ? cx1 : cx0, cy = which ? cy1 : cy0, cz = which ? cz1 : cz0;
-                for (int zz = max(cz - G, 0); zz <= min(cz + G, g.nz - 1); ++zz)
-                    for (int yy = max(cy - G, 0); yy <= min(cy + G, g.ny - 1); ++yy) {
-                        int lo, hi;
-                        if (!xrange(cx, cy, cz, yy, zz, lo, hi)) continue;
-                        const int rowc = (zz * g.ny + yy) * g.nx;
-                        scan(a.cell_start[rowc + lo], a.cell_start[rowc + hi + 1]);
-                    }
-            }
+            sweep_box(max(cy0 - G, 0), min(cy0 + G, g.ny - 1), max(cz0 - G, 0), min(cz0 + G, g.nz - 1), 0);
+            if (has1) sweep_box(max(cy1 - G, 0), min(cy1 + G, g.ny - 1), max(cz1 - G, 0), min(cz1 + G, g.nz - 1), 1);
         }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             cnt0 += __shfl_xor_sync(0xffffffffu, cnt0, off);
             cnt1 += __shfl_xor_sync(0xffffffffu, cnt1, off);
         }
-        const int kept = min(cnt, cap);
-        const int padded = min((kept + 31) & ~31, cap);
-        if (kept + lane < padded) row[kept + lane] = N;                 // pad with the dummy record
-        if (lane == 0) a.ncount[gp] = kept;
+        if constexpr (!kListRuns) {
+            // one free slot for the term between the two atoms of the pair, then the dummy record up to a whole batch
+            const int padded = min((nruns + 32) & ~31, cap);
+            if (nruns + lane < padded) row[nruns + lane] = N;
+            my_overflow = my_overflow || nruns + 1 > cap;
+        }
+        if (lane == 0) a.ncount[gp] = min(nruns, cap);
         my_max = max(my_max, max(cnt0, cnt1));
-        my_overflow = my_overflow || cnt > cap;
+        my_overflow = my_overflow || nruns > cap;
     }
     if (lane == 0 && (my_overflow || my_max > a.kmax)) atomicExch(&a.counters[kCntOverflow], 1ull);
     // counters[kCntMaxRow] is reset below by the one thread that also bumps the build count; a max
@@ -423,10 +495,12 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
 struct NlistArgs {
     double4 *xs;              // [N + 1] (x, y, z, s'), internal order; xs[N] = the dummy record at infinity
     RecF *xfr;                // MIXED: [N + 1] split binary32 records (same order, same dummy); sweep 1 stores fl32(s') here
-    const int *nlist;         // [ceil(N/2)][2 * kmax] pair rows, padded with N to a multiple of 32
-    const int *ncount;        // [ceil(N/2)]
+    const int *nlist;         // [ceil(N/2)][2 * kmax] pair rows of run words (first index << 5 | length - 1)
+    const int *ncount;        // [ceil(N/2)] runs per row
     int n_atoms, kmax;
-    int pairs_per_cta;        // consecutive atom pairs one CTA works through (multiple of warps * 32 / LPA)
+    int pairs_per_cta;        // consecutive atom pairs in one block of rows (a multiple of the warps per CTA); CTA c takes
+                              //   the blocks c, c + gridDim.x, ...
+    int idx_cap;              // ints of shared memory per warp for the expanded row: >= 2 kmax + 64
     double *rho;              // [N]    sweep 1
     double *force;            // [N*3]  sweep 2
     double *partial;          // [gridDim.x]
@@ -436,7 +510,8 @@ struct NlistArgs {
     PairConsts c;
 };
 
-constexpr int kNlistMaxBlock = 256;   // threads per CTA of the list sweeps: 32 * warps, chosen by the host
+constexpr int kNlistMaxBlock = 128;   // threads per CTA of the list sweeps: 32 * warps (<= 4), chosen by the host
+constexpr int kNlistMinBlocks = 6;    // resident CTAs per SM the register allocation must allow (<= 85 registers)
 
 // one 32-byte record with a single 256-bit load (SASS LDG.E.ENL2.256): one L1 wavefront per line touched
 __device__ __forceinline__ double4 load_record(const double4 *p) {
@@ -553,17 +628,146 @@ __device__ __forceinline__ void nlist_term_f(const RecF &pi, const RecF &p, Pair
     }
 }
 
-// LPA lanes per atom PAIR (32 / LPA pairs per warp at a time).  A CTA works through pairs_per_cta
-// consecutive pairs of the internal (cell) order, its warps interleaved, so that the records its
-// gathers touch stay in L1.  Every fetched record serves both atoms of the pair.
+// The same terms for entries that cannot be the atom itself (every batch but the first of a row): no index compare,
+// and ONE select per term instead of five -- the MUFU seed of the reciprocal (square root) comes with a zero low word,
+// so an entry that fails the test gets the seed's high word replaced by 0 and every later product is an exact 0
+// (r^2 of two different atoms is a positive finite number: no 0 x inf on the way; the dummy record gives r^2 = 3e300).
+__device__ __forceinline__ double seed_or_zero(double seed, bool keep) {
+    return __hiloint2double(keep ? __double2hiint(seed) : 0, 0);
+}
+template <int NE, int ME, bool FORCE, bool ENERGY>
+__device__ __forceinline__ void nlist_term_lean(const double4 &pi, const double4 &p, double rc2, double An, int n_exp,
+                                                int m_exp, double (&acc)[4], int &npairs) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = r2 < rc2;
+    if constexpr (!FORCE) {
+        npairs += in ? 1 : 0;
+        if constexpr (ME > 0 && ME % 2 == 0) {
+            const double y0 = seed_or_zero(rcp_seed(r2), in);
+            const double e = fma(-r2, y0, 1.0);
+            const double w = fma(y0, fma(e, e, e), y0);
+            if constexpr (ME == 6) acc[0] = fma(w * w, w, acc[0]);
+            else acc[0] += ipow_c<ME / 2>(w);
+        } else {
+            const double y0 = seed_or_zero(rsqrt_seed(r2), in);
+            const double t = r2 * y0, e = fma(-t, y0, 1.0);
+            const double y = fma(y0, e * fma(0.375, e, 0.5), y0);
+            acc[0] += (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+        }
+    } else {
+        const double y0 = seed_or_zero(rsqrt_seed(r2), in);
+        const double t = r2 * y0, e = fma(-t, y0, 1.0);
+        const double y = fma(y0, e * fma(0.375, e, 0.5), y0);
+        const double w = y * y;
+        const double ss = pi.w + p.w;
+        double coef;
+        if constexpr (NE == 9 && ME == 6) {
+            const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
+            coef = w4 * fma(An, y3, -ss);
+            if constexpr (ENERGY) acc[3] = fma(w4, y, acc[3]);
+        } else {
+            const double pm = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+            const double pn = (NE > 0) ? ipow_c<(NE > 0 ? NE : 1)>(y) : ipow_rt(y, n_exp);
+            coef = w * fma(An, pn, -ss * pm);
+            if constexpr (ENERGY) acc[3] += pn;
+        }
+        acc[0] = fma(coef, dx, acc[0]);
+        acc[1] = fma(coef, dy, acc[1]);
+        acc[2] = fma(coef, dz, acc[2]);
+    }
+}
+template <int NE, int ME, bool FORCE, bool ENERGY>
+__device__ __forceinline__ void nlist_term_f_lean(const RecF &pi, const RecF &p, PairGeomF g, bool in, float Anf, int n_exp,
+                                                  int m_exp, float (&f)[4], int &npairs) {
+    // binary32: g.q2 of the dummy record is 3e36 (finite), of two different atoms > 0
+    if constexpr (!FORCE) {
+        npairs += in ? 1 : 0;
+        if constexpr (ME > 0 && ME % 2 == 0) {
+            float y0;
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(g.q2));
+            y0 = in ? y0 : 0.f;
+            const float w = fmaf(y0, fmaf(-g.q2, y0, 1.0f), y0);
+            if constexpr (ME == 6) f[0] = fmaf(w * w, w, f[0]);
+            else f[0] += ipow_cf<ME / 2>(w);
+        } else {
+            float y0;
+            asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(g.q2));
+            y0 = in ? y0 : 0.f;
+            const float y = fmaf(y0 * fmaf(-(g.q2 * y0), y0, 1.0f), 0.5f, y0);
+            f[0] += (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+        }
+    } else {
+        float y0;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(g.q2));
+        y0 = in ? y0 : 0.f;
+        const float y = fmaf(y0 * fmaf(-(g.q2 * y0), y0, 1.0f), 0.5f, y0);
+        const float w = y * y;
+        const float ss = pi.s + p.s;
+        float coef;
+        if constexpr (NE == 9 && ME == 6) {
+            const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+            coef = w4 * fmaf(Anf, y3, -ss);
+            if constexpr (ENERGY) f[3] = fmaf(w4, y, f[3]);
+        } else {
+            const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+            const float pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+            coef = w * fmaf(Anf, pn, -ss * pm);
+            if constexpr (ENERGY) f[3] += pn;
+        }
+        f[0] = fmaf(coef, g.fx, f[0]);
+        f[1] = fmaf(coef, g.fy, f[1]);
+        f[2] = fmaf(coef, g.fz, f[2]);
+    }
+}
+
+// One warp per atom PAIR.  A CTA works through pairs_per_cta consecutive pairs of the internal (cell) order, its
+// warps interleaved, so that the records its gathers touch stay in L1.
+//
+// Row walk.  The run words of a row arrive in registers one row AHEAD (fetched while the row before is in the FP64
+// pipe: the list never stalls the loop on DRAM).  The warp expands them into its shared-memory index list -- a warp
+// scan of the lengths, then every lane writes out its run of <= 8 indices -- pads the last batch with the index of
+// the dummy record and works through the list in batches of 32 entries, lane t taking entry 32 b + t: adjacent
+// lanes gather adjacent records with one 256-bit load each (SASS LDG.E.ENL2.256), and every fetched record serves
+// both atoms of the pair.  The rows hold no atom's own record (the build excludes the pair itself), so no term
+// compares indices; the term BETWEEN the two atoms of the pair rides in the first free lane of the last batch, whose
+// "record" is the other atom of the pair.  Issue slots matter as much as the FP64 pipe here (round 1: 101 instructions
+// per batch for 46 FP64 ones; now ~57): one select per term, no compares, no register moves.
 // SHIFT (sweep 1 only): energy-shifted cutoff -- the in-range entries are counted per atom and the epilogue takes
 // count * r_c^-m off the sum (a separate instantiation: the per-atom counters cost the plain sweep 5 %).
-template <int LPA, int NE, int ME, bool FORCE, bool ENERGY, bool MIXED, bool SHIFT = false>
-__global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a) {
-    constexpr int AW = 32 / LPA;                         // pairs per warp
+constexpr int kNlistCH = 4;           // batches of 32 entries per loop iteration: 2 kNlistCH independent chains per lane
+constexpr bool kNlistPF = false;      // records of iteration t + 1 in flight (registers) while iteration t is in the pipe
+constexpr int kNlistL1PF = 0;         // records of iteration t + kNlistL1PF are prefetched into L1 (0: off)
+constexpr int kNlistRW = 4;           // run words per lane fetched a row ahead (rows of up to 128 runs: fcc rows have ~100)
+
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// sum of V values over the 32 lanes in V / 2 + V / 4 + ... + 1 + (remaining stages) shuffles instead of 5 V: at every
+// halving stage a lane keeps one half of its values and hands the other half to its partner.  On return v[0] of lane L
+// holds the total of value number L / (32 / V); fixed order, same bits every run.
+template <int V>
+__device__ __forceinline__ void transpose_sum(double (&v)[V]) {
+    const int lane = threadIdx.x & 31;
+    int off = 16;
+#pragma unroll
+    for (int n = V; n > 1; n >>= 1, off >>= 1) {
+        const bool upper = (lane & off) != 0;
+#pragma unroll
+        for (int k = 0; k < n / 2; ++k) {
+            const double keep = upper ? v[n / 2 + k] : v[k], give = upper ? v[k] : v[n / 2 + k];
+            v[k] = keep + __shfl_xor_sync(0xffffffffu, give, off);
+        }
+    }
+    for (; off > 0; off >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], off);
+}
+
+template <int NE, int ME, bool FORCE, bool ENERGY, bool MIXED, bool SHIFT = false>
+__global__ void __launch_bounds__(kNlistMaxBlock, kNlistMinBlocks) nlist_kernel(const NlistArgs a) {
+    constexpr int CH = kNlistCH, RW = kNlistRW;
+    extern __shared__ int idx_all[];
     __shared__ double scratch[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int g = lane / LPA, q = lane % LPA;            // group g of the warp takes one pair, q strides its row
+    int *idx = idx_all + size_t(warp) * a.idx_cap;
     const int N = a.n_atoms, NP = (N + 1) >> 1;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An, rc2 = a.rc2;
@@ -571,37 +775,109 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
     const size_t stride = 2 * size_t(a.kmax);
     double contrib = 0.0;
     int npairs = 0;
+    // records: binary64 (x, y, z, s') or, MIXED, their split binary32 twins -- both 32 bytes, fetched alike
+    const double4 *recs = MIXED ? reinterpret_cast<const double4 *>(a.xfr) : a.xs;
 
-    const int base = blockIdx.x * a.pairs_per_cta;
-    const int end = min(NP, base + a.pairs_per_cta);
+    // Persistent CTAs: the grid is one wave; CTA c works through the blocks c, c + gridDim.x, ... of pairs_per_cta
+    // consecutive pairs (static, so every sum keeps a fixed order; strided, so surface and bulk rows mix in every CTA).
     const int nwarps = blockDim.x >> 5;
-    for (int g0 = base + warp * AW; g0 < end; g0 += nwarps * AW) {
-        const int gp = g0 + g;
-        const bool live = gp < end;
-        const int i0 = live ? 2 * gp : N, i1 = (live && 2 * gp + 1 < N) ? 2 * gp + 1 : N;   // N = the dummy record
-        // records: binary64 (x, y, z, s') or, MIXED, their split binary32 twins -- both 32 bytes, fetched alike
-        const double4 *recs = MIXED ? reinterpret_cast<const double4 *>(a.xfr) : a.xs;
-        const double4 pa = recs[i0], pb = recs[i1];
-        const int cnt = live ? a.ncount[gp] : 0;
-        const int niter = (cnt + LPA - 1) / LPA;         // rows are padded to a multiple of 32 >= LPA
-        const int *row = a.nlist + size_t(live ? gp : 0) * stride + q;
+    const int ppc = a.pairs_per_cta;
+    const int cap = int(stride);
+    const int lim = 2 * a.kmax + 32;         // a row that passed the capacity check expands to <= 2 kmax entries; one that
+                                             // did not (SC_ERR_CAPACITY is on its way) is cut here: no write beyond idx_cap
+    auto next_row = [&](int g) {             // the row this warp takes after row g
+        const int n = g + nwarps;
+        return (n % ppc) < nwarps && n % ppc == warp ? n + (int(gridDim.x) - 1) * ppc : n;
+    };
+    int nr = 0;
+    unsigned rw[RW];
+    auto fetch_row = [&](int g, int &n_runs, unsigned (&w)[RW]) {
+        if (g < NP) {
+            n_runs = a.ncount[g];
+            const int *rp = a.nlist + size_t(g) * stride;
+#pragma unroll
+            for (int u = 0; u < RW; ++u) w[u] = (u * 32 + lane < cap) ? unsigned(rp[u * 32 + lane]) : 0u;
+            if (lane < 2 && 2 * g + lane < N) prefetch_l1(recs + 2 * g + lane);   // the two atoms of that pair
+        }
+    };
+    fetch_row(blockIdx.x * ppc + warp, nr, rw);
+    for (int gp = blockIdx.x * ppc + warp; gp < NP; gp = next_row(gp)) {
+        const int i0 = 2 * gp, i1 = (2 * gp + 1 < N) ? 2 * gp + 1 : N;      // N = the dummy record
+        const double4 pa = recs[i0];
+        double4 pb = recs[i1];
+        if (i1 == N) {
+            // odd N: the last pair has a phantom second atom.  It must be far from every atom AND from the dummy record
+            // that pads the batches (no term compares indices): the dummy mirrored through the origin
+            if constexpr (MIXED) {
+                RecF ph{-kFarAwayF, -kFarAwayF, -kFarAwayF, 0.f, 0.f, 0.f, 0.f, 0.f};
+                pb = reinterpret_cast<const double4 &>(ph);
+            } else {
+                pb = make_double4(-kFarAway, -kFarAway, -kFarAway, 0.0);
+            }
+        }
+        const int *rowp = a.nlist + size_t(gp) * stride;
+        int nr_next = 0;
+        unsigned rw_next[RW];
+        fetch_row(next_row(gp), nr_next, rw_next);
+        nr = __shfl_sync(0xffffffffu, nr, 0);                                // the same in every lane: say so
+
+        int fill = 0;
+        const int *list;                                                     // the row's entries, one index per word
+      if constexpr (kListRuns) {
+        // ---- expand the runs ----
+        __syncwarp();                                                        // the previous row's readers are done
+        auto expand = [&](unsigned run, bool live) {
+            int len = live ? int(run & (kRunMaxLen - 1)) + 1 : 0;
+            const int first = int(run >> kRunBits);
+            int incl = len;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, off);
+                if (lane >= off) incl += v;
+            }
+            const int at = fill + incl - len;
+            len = min(len, max(lim - at, 0));
+            int *dst = idx + at;
+#pragma unroll
+            for (int k = 0; k < kRunMaxLen; ++k)
+                if (k < len) dst[k] = first + k;
+            fill = min(fill + __shfl_sync(0xffffffffu, incl, 31), lim);
+        };
+#pragma unroll
+        for (int u = 0; u < RW; ++u)
+            if (u * 32 < nr) expand(rw[u], u * 32 + lane < nr);
+        for (int r0 = RW * 32; r0 < nr; r0 += 32)                            // rows longer than the prefetched part
+            expand(r0 + lane < nr ? unsigned(rowp[r0 + lane]) : 0u, r0 + lane < nr);
+        // the last batch: entries, then ONE lane for the term between the two atoms of the pair, then the dummy record
+        if (lane >= (fill & 31)) idx[fill - (fill & 31) + lane] = N;
+        __syncwarp();
+        list = idx;
+      } else {
+        fill = min(nr, cap - 1);                                             // the build padded the row the same way
+        list = rowp;
+      }
+        const int lpair = fill & 31;
+        const int nb32 = (fill >> 5) + 1, nwhole = (nb32 - 1) / CH;          // nwhole iterations of CH batches, then 1 .. CH batches
+
         double acc0[4] = {0.0, 0.0, 0.0, 0.0}, acc1[4] = {0.0, 0.0, 0.0, 0.0};
         float f0[4] = {0.f, 0.f, 0.f, 0.f}, f1[4] = {0.f, 0.f, 0.f, 0.f};
         int np0 = 0, np1 = 0;                            // sweep 1: in-range entries (SHIFT: of each atom of the pair)
         bool unsure = false;
 
-        auto entry = [&](int j, const double4 &p) {
+        // one fetched record against both atoms of the pair (qa = qb = the record), or -- the pair lane of the last
+        // batch -- each atom against the other (qa = pb, qb = pa)
+        auto entry2 = [&](const double4 &qa, const double4 &qb) {
             if constexpr (MIXED) {
                 // binary32 decision; entries too close to the cutoff to trust it only raise `unsure`
                 const RecF &fa = reinterpret_cast<const RecF &>(pa), &fb = reinterpret_cast<const RecF &>(pb);
-                const RecF &fp = reinterpret_cast<const RecF &>(p);
-                const PairGeomF ga = nlist_geom_f(fa, fp), gb = nlist_geom_f(fb, fp);
+                const RecF &ga_ = reinterpret_cast<const RecF &>(qa), &gb_ = reinterpret_cast<const RecF &>(qb);
+                const PairGeomF ga = nlist_geom_f(fa, ga_), gb = nlist_geom_f(fb, gb_);
                 unsure = unsure || fabsf(ga.q2 - rc2f) <= band || fabsf(gb.q2 - rc2f) <= band;
-                nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, ga, ga.q2 < rc2f && j != i0, Anf, n_exp, m_exp, f0, np0);
-                nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, gb, gb.q2 < rc2f && j != i1, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
+                nlist_term_f_lean<NE, ME, FORCE, ENERGY>(fa, ga_, ga, ga.q2 < rc2f, Anf, n_exp, m_exp, f0, np0);
+                nlist_term_f_lean<NE, ME, FORCE, ENERGY>(fb, gb_, gb, gb.q2 < rc2f, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
             } else {
-                nlist_term<NE, ME, FORCE, ENERGY>(pa, p, j != i0, rc2, An, n_exp, m_exp, acc0, np0);
-                nlist_term<NE, ME, FORCE, ENERGY>(pb, p, j != i1, rc2, An, n_exp, m_exp, acc1, SHIFT ? np1 : np0);
+                nlist_term_lean<NE, ME, FORCE, ENERGY>(pa, qa, rc2, An, n_exp, m_exp, acc0, np0);
+                nlist_term_lean<NE, ME, FORCE, ENERGY>(pb, qb, rc2, An, n_exp, m_exp, acc1, SHIFT ? np1 : np0);
             }
         };
         auto flush = [&]() {
@@ -613,33 +889,78 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 }
             }
         };
-        // Software pipeline over batches of CH entries per lane: while batch t is in the FP64 pipe the
-        // records of batch t + 1 (indices fetched an iteration earlier) and the indices of batch t + 2
-        // (streamed from HBM) are in flight.  Slots beyond the row read the dummy record.
-        constexpr int CH = 4;
-        const int nbatch = (niter + CH - 1) / CH;
-        auto load_idx = [&](int b, int (&jj)[CH]) {
+        auto gather = [&](const int *ip, double4 (&p)[CH]) {
 #pragma unroll
             for (int u = 0; u < CH; ++u) {
-                const int it = b * CH + u;
-                jj[u] = it < niter ? row[it * LPA] : N;
+                p[u] = load_record(recs + ip[32 * u]);
             }
         };
-        int jc[CH], j1[CH], j2[CH];
-        double4 pc[CH], pn[CH];
-        load_idx(0, jc);
-        load_idx(1, j1);
+        auto compute = [&](const double4 (&p)[CH]) {
 #pragma unroll
-        for (int u = 0; u < CH; ++u) pc[u] = load_record(recs + jc[u]);
-        for (int b = 0; b < nbatch; ++b) {
-            load_idx(b + 2, j2);
-#pragma unroll
-            for (int u = 0; u < CH; ++u) pn[u] = load_record(recs + j1[u]);
-#pragma unroll
-            for (int u = 0; u < CH; ++u) entry(jc[u], pc[u]);
+            for (int u = 0; u < CH; ++u) entry2(p[u], p[u]);
             flush();
+        };
+        // ---- whole iterations of CH batches: 2 CH independent chains per lane, no branches.  With kNlistPF the loop is
+        //      unrolled by two so that two register sets alternate (no moves): the gathers of the next iteration are in
+        //      flight while this one is in the pipe; past the last whole iteration the gather re-reads the last one. ----
+        const int *ip = list + lane;
+        if constexpr (!kListRuns && !kNlistPF) {
+            static_assert(kNlistRW >= kNlistCH, "the words fetched a row ahead hold the first iteration's indices");
+            int jc[CH], jn[CH];
 #pragma unroll
-            for (int u = 0; u < CH; ++u) { jc[u] = j1[u]; j1[u] = j2[u]; pc[u] = pn[u]; }
+            for (int u = 0; u < CH; ++u) jc[u] = int(rw[u]);
+            for (int it = 0; it < nwhole; ++it) {
+                const int *nx = ip + min(it + 1, nwhole - 1) * (32 * CH);   // indices of the next whole iteration, in flight
+#pragma unroll
+                for (int u = 0; u < CH; ++u) jn[u] = nx[32 * u];
+                double4 pc[CH];
+#pragma unroll
+                for (int u = 0; u < CH; ++u) pc[u] = load_record(recs + jc[u]);
+                compute(pc);
+#pragma unroll
+                for (int u = 0; u < CH; ++u) jc[u] = jn[u];
+            }
+        } else if constexpr (kNlistPF) {
+            if (nwhole > 0) {
+                double4 pA[CH], pB[CH];
+                const int *last = ip + (nwhole - 1) * (32 * CH);
+                gather(ip, pA);
+                for (int it = 0; it < nwhole; it += 2) {
+                    gather(ip + 32 * CH < last ? ip + 32 * CH : last, pB);
+                    compute(pA);
+                    if (it + 1 < nwhole) {
+                        gather(ip + 64 * CH < last ? ip + 64 * CH : last, pA);
+                        compute(pB);
+                    }
+                    ip += 64 * CH;
+                }
+            }
+        } else {
+            if constexpr (kNlistL1PF > 0) {
+                // the first iterations' records (the list is padded, so reading a little past the whole iterations is harmless)
+                const int ahead = min(kNlistL1PF * CH, nb32);
+                for (int b = 0; b < ahead; ++b) prefetch_l1(recs + ip[32 * b]);
+            }
+            for (int it = 0; it < nwhole; ++it, ip += 32 * CH) {
+                double4 pc[CH];
+                if constexpr (kNlistL1PF > 0) {
+                    if ((it + kNlistL1PF) * CH < nb32) {
+#pragma unroll
+                        for (int u = 0; u < CH; ++u)
+                            if ((it + kNlistL1PF) * CH + u < nb32) prefetch_l1(recs + ip[32 * (kNlistL1PF * CH + u)]);
+                    }
+                }
+                gather(ip, pc);
+                compute(pc);
+            }
+        }
+        // ---- the remaining 1 .. CH batches, one at a time; the last one carries the pair term in lane `lpair` ----
+        for (int b = nwhole * CH; b < nb32; ++b) {
+            const double4 p = load_record(recs + list[b * 32 + lane]);
+            const bool pair_lane = b == nb32 - 1 && lane == lpair;
+            const double4 qa = pair_lane ? pb : p, qb = pair_lane ? pa : p;
+            entry2(qa, qb);
+            flush();
         }
 
         if constexpr (MIXED) {
@@ -651,56 +972,60 @@ __global__ void __launch_bounds__(kNlistMaxBlock) nlist_kernel(const NlistArgs a
                 for (int c = 0; c < 4; ++c) { acc0[c] = 0.0; acc1[c] = 0.0; f0[c] = 0.f; f1[c] = 0.f; }
                 np0 = 0; np1 = 0;
                 const RecF &fa = reinterpret_cast<const RecF &>(pa), &fb = reinterpret_cast<const RecF &>(pb);
-                for (int it = 0; it < niter; ++it) {
-                    const int j = row[it * LPA];
+                for (int b = 0; b < nb32; ++b) {
+                    const bool pair_lane = b == nb32 - 1 && lane == lpair;
+                    const int j = list[b * 32 + lane];
+                    const int ja = pair_lane ? i1 : j, jb = pair_lane ? i0 : j;     // the record each atom meets
                     const double4 p = load_record(recs + j);
-                    const RecF &fp = reinterpret_cast<const RecF &>(p);
-                    const bool in0 = j != i0 && nlist_exact_in_range(a.xs, i0, j, rc2);
-                    const bool in1 = j != i1 && nlist_exact_in_range(a.xs, i1, j, rc2);
-                    nlist_term_f<NE, ME, FORCE, ENERGY>(fa, fp, nlist_geom_f(fa, fp), in0, Anf, n_exp, m_exp, f0, np0);
-                    nlist_term_f<NE, ME, FORCE, ENERGY>(fb, fp, nlist_geom_f(fb, fp), in1, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
-                    if ((it & 3) == 3) flush();                  // same flush points as the fast loop
+                    const double4 qa = pair_lane ? pb : p, qb = pair_lane ? pa : p;
+                    const RecF &ga_ = reinterpret_cast<const RecF &>(qa), &gb_ = reinterpret_cast<const RecF &>(qb);
+                    const bool in0 = ja < N && nlist_exact_in_range(a.xs, i0, ja, rc2);
+                    const bool in1 = i1 < N && jb < N && nlist_exact_in_range(a.xs, i1, jb, rc2);
+                    nlist_term_f_lean<NE, ME, FORCE, ENERGY>(fa, ga_, nlist_geom_f(fa, ga_), in0, Anf, n_exp, m_exp, f0, np0);
+                    nlist_term_f_lean<NE, ME, FORCE, ENERGY>(fb, gb_, nlist_geom_f(fb, gb_), in1, Anf, n_exp, m_exp, f1, SHIFT ? np1 : np0);
+                    // the flush points of the fast loops: after every whole iteration, after every remaining batch
+                    if (b >= nwhole * CH || (b % CH) == CH - 1) flush();
                 }
                 flush();
             }
         }
         npairs += np0 + np1;
         if constexpr (!FORCE && SHIFT) {
-            // per-atom neighbour counts over the LPA lanes (integers: exact), for the shifted density
+            // per-atom neighbour counts over the 32 lanes (integers: exact), for the shifted density
 #pragma unroll
-            for (int off = LPA / 2; off > 0; off >>= 1) {
+            for (int off = 16; off > 0; off >>= 1) {
                 np0 += __shfl_xor_sync(0xffffffffu, np0, off);
                 np1 += __shfl_xor_sync(0xffffffffu, np1, off);
             }
         }
 
-        // ---- reduce over the LPA lanes of the pair (fixed order) ----
-        constexpr int NV = FORCE ? (ENERGY ? 4 : 3) : 1;
-#pragma unroll
-        for (int c = 0; c < NV; ++c) { acc0[c] = group_sum<LPA>(acc0[c]); acc1[c] = group_sum<LPA>(acc1[c]); }
-        if (live && q == 0) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int i = h ? i1 : i0;
-                const double *acc = h ? acc1 : acc0;
-                if (i >= N) continue;
-                if constexpr (!FORCE) {
-                    // shifted cutoff: every in-range term loses r_c^-m
-                    const double rho = SHIFT ? a.c.am * fma(-double(h ? np1 : np0), a.shift_m, acc[0]) : a.c.am * acc[0];
-                    a.rho[i] = rho;
-                    const double root = rho > 0.0 ? sqrt(rho) : 0.0;       // reading Q9
-                    const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;
-                    a.xs[i].w = sp;
-                    if constexpr (MIXED) a.xfr[i].s = float(sp);
-                    contrib += root;
-                } else {
-                    a.force[3 * size_t(i)] = acc[0];
-                    a.force[3 * size_t(i) + 1] = acc[1];
-                    a.force[3 * size_t(i) + 2] = acc[2];
-                    contrib += acc[3];
-                }
+        // ---- sums over the 32 lanes (fixed order), each total lands in its own lane, which stores it ----
+        if constexpr (!FORCE) {
+            double v[2] = {acc0[0], acc1[0]};
+            transpose_sum<2>(v);
+            const int h = lane >> 4, i = h ? i1 : i0;
+            if ((lane & 15) == 0 && i < N) {
+                // shifted cutoff: every in-range term loses r_c^-m
+                const double rho = SHIFT ? a.c.am * fma(-double(h ? np1 : np0), a.shift_m, v[0]) : a.c.am * v[0];
+                a.rho[i] = rho;
+                const double root = rho > 0.0 ? sqrt(rho) : 0.0;           // reading Q9
+                const double sp = rho > 0.0 ? a.c.Bm / root : 0.0;
+                a.xs[i].w = sp;
+                if constexpr (MIXED) a.xfr[i].s = float(sp);
+                contrib += root;
+            }
+        } else {
+            double v[8] = {acc0[0], acc0[1], acc0[2], acc0[3], acc1[0], acc1[1], acc1[2], acc1[3]};
+            transpose_sum<8>(v);
+            const int q = lane >> 2, h = q >> 2, c = q & 3, i = h ? i1 : i0;   // lane 4 q holds value q = (atom h, component c)
+            if ((lane & 3) == 0 && i < N) {
+                if (c < 3) a.force[3 * size_t(i) + c] = v[0];
+                else contrib += v[0];
             }
         }
+        nr = nr_next;
+#pragma unroll
+        for (int u = 0; u < RW; ++u) rw[u] = rw_next[u];
     }
     if constexpr (!FORCE) {
 #pragma unroll

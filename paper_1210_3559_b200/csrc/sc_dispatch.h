@@ -16,8 +16,8 @@ const void *allpairs64_fn_generic(int it, int tpr, bool force, bool energy);
 const void *allpairs32_fn_96(int it, int tpr, bool force, bool energy);
 const void *allpairs32_fn_generic(int it, int tpr, bool force, bool energy);
 
-// list-driven sweeps: LPA = 8, 16 or 32 lanes per atom pair, `block` threads per CTA
-cudaError_t launch_nlist_96(int lpa, int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st);
-cudaError_t launch_nlist_generic(int lpa, int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st);
+// list-driven sweeps: one warp per atom pair, `grid` persistent CTAs of `block` threads
+cudaError_t launch_nlist_96(int grid, int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st);
+cudaError_t launch_nlist_generic(int grid, int block, const NlistArgs &a, bool force, bool energy, bool mixed, cudaStream_t st);
 
 }  // namespace scmd

@@ -347,29 +347,30 @@ sc_status ensure_list(sc_ctx *c) {
     return SC_OK;
 }
 
-// lanes per atom of the list sweeps: one warp per row (adjacent lanes gather adjacent records)
-int choose_lpa(const sc_ctx *c) {
-    if (c->opt_tpr) return c->opt_tpr < 8 ? 8 : c->opt_tpr;
-    return 32;
-}
 // list sweeps: warps per CTA and consecutive atom pairs per CTA.  The warps of a CTA work on adjacent
 // pairs at the same time, so the records they gather are the same L1 lines.
 int choose_nlist_warps(const sc_ctx *c) { return c->opt_warps ? c->opt_warps : 4; }
-int choose_pairs_per_cta(const sc_ctx *c, int lpa, int warps) {
-    const int step = warps * (32 / lpa);
-    int64_t ppc = c->opt_apc ? (c->opt_apc + 1) / 2 : (c->N >= 262144 ? 32 : 2 * step);   // measured
-    ppc = ppc / step * step;
-    return int(ppc < step ? step : ppc);
+int choose_pairs_per_cta(const sc_ctx *c, int warps) {
+    int64_t ppc = c->opt_apc ? (c->opt_apc + 1) / 2 : 2 * warps;
+    ppc = ppc / warps * warps;
+    return int(ppc < warps ? warps : ppc);
+}
+// grid of the list sweeps: CTA c takes the row blocks c, c + grid, ...  Measured at N = 65536: one
+// resident wave (6 CTAs per SM) and one CTA per block perform alike (84.7 + 105.5 against 82.5 + 104.2 us); the cap
+// only keeps the per-CTA partial sums few at N = 2^20.
+int choose_nlist_grid(const sc_ctx *c, int ppc) {
+    const int blocks = ceil_div((c->N + 1) / 2, ppc);
+    return std::min(blocks, c->sm_count * 32);
 }
 
 sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
     sc_status st = ensure_list(c);
     if (st != SC_OK) return st;
-    const int lpa = choose_lpa(c);
     NlistArgs a{};
     a.xs = c->xs; a.xfr = c->xfr; a.nlist = c->nlist; a.ncount = c->ncount; a.n_atoms = int(c->N); a.kmax = c->kmax;
     const int warps = choose_nlist_warps(c);
-    a.pairs_per_cta = choose_pairs_per_cta(c, lpa, warps);
+    a.pairs_per_cta = choose_pairs_per_cta(c, warps);
+    a.idx_cap = 2 * c->kmax + 64;
     a.rho = c->rho; a.force = c->force; a.partial = force ? c->part_b : c->part_a;
     a.pairs_in_cut = c->counters + kCntPairsInCut;
     a.rc2 = c->p.r_cut * c->p.r_cut;
@@ -381,12 +382,12 @@ sc_status run_sweep_cutoff(sc_ctx *c, bool force, bool energy) {
         c->pairs_zeroed = false;
     }
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    cudaError_t e = fast ? launch_nlist_96(lpa, warps * 32, a, force, energy, mixed, c->stream)
-                         : launch_nlist_generic(lpa, warps * 32, a, force, energy, mixed, c->stream);
+    const int grid = choose_nlist_grid(c, a.pairs_per_cta);
+    cudaError_t e = fast ? launch_nlist_96(grid, warps * 32, a, force, energy, mixed, c->stream)
+                         : launch_nlist_generic(grid, warps * 32, a, force, energy, mixed, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "list sweep launch: %s", cudaGetErrorString(e));
     c->launches += 1;
     if (!force || energy) {
-        const int grid = ceil_div((c->N + 1) / 2, a.pairs_per_cta);
         if (!force) {
             c->emb_pending = grid;                                // totalled when an energy is asked for (ensure_forces)
         } else {
@@ -739,6 +740,7 @@ size_t sc_workspace_bytes_ex(const sc_params *params, int64_t n_atoms, int32_t p
     if (!params_ok(params) || n_atoms < 1 || n_atoms > (int64_t(1) << 30)) return 0;
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
     if (!(skin >= 0.0) || !create_options_ok(options)) return 0;
+    if (params->r_cut > 0.0 && n_atoms > kCutoffMaxAtoms) return 0;       // run words hold 29-bit indices
     return carve(nullptr, nullptr, n_atoms, params, precision, skin, options);
 }
 
@@ -760,6 +762,7 @@ sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precisi
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return SC_ERR_INVALID;
     if (!(skin >= 0.0) || !d_workspace || !create_options_ok(options)) return SC_ERR_INVALID;
     if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
+    if (params->r_cut > 0.0 && n_atoms > kCutoffMaxAtoms) return SC_ERR_INVALID;
     const size_t need = sc_workspace_bytes_ex(params, n_atoms, precision, skin, options);
     if (workspace_bytes < need) return SC_ERR_NOMEM;
     int dev = 0, count = 0;
