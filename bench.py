@@ -521,6 +521,98 @@ def run_ours(args):
 ALSO_WORKLOADS = ["Ni65536-fcc-allpairs-mixed", "Ni65536-fcc-cutoff10-fp64"]
 
 
+def run_rows(args):
+    """`--parallel rows`: ONE cluster split by rows over the ranks (paper_1210_3559_b200/distributed.py):
+    strong scaling.  Per step two all-gathers (positions, densities) on NCCL; every rank runs the one-sided sweeps on
+    its rows.  All pairs only."""
+    import torch
+    import torch.distributed as dist
+    import paper_1210_3559_b200 as scmd
+
+    rank, local_rank, world = dist_env()
+    spec = Spec(args.workload)
+    if spec.r_cut > 0:
+        raise SystemExit("--parallel rows is the all-pairs split; the list path runs as replicas")
+    torch.cuda.set_device(local_rank if world > 1 else 0)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    scmd.load_library()
+    w = spec.generate(0)                                               # the same cluster on every rank
+    N = w.n_atoms
+    prec = scmd.SC_PREC_MIXED if spec.prec == "mixed" else scmd.SC_PREC_FP64
+    rs = scmd.RowSplitSuttonChen(N, rank, world, precision=prec)
+    h_pos, h_vel = torch.as_tensor(w.pos).pin_memory(), torch.as_tensor(w.vel).pin_memory()
+    rs.set_state(h_pos.to(dev), h_vel.to(dev))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(dev.index or 0) if rank == 0 else None
+    if sampler is not None:
+        sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        rs.step(1.0, 1)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    if sampler is not None:
+        sampler.mark()
+    launches0 = rs.ctx.sc_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.zero_()
+        ev[k][0].record(stream)
+        rs.step(1.0, 1)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = rs.ctx.sc_launch_count() - launches0
+    clocks = sampler.stop() if sampler is not None else None
+    local_ms = sum(a.elapsed_time(b) for a, b in ev)
+    rows = rs.end - rs.begin
+    total_ms, total_pairs = aggregate(local_ms, float(rows) * (N - 1) * args.steps, world)
+    # end to end: positions from pinned host memory, one force evaluation (both sweeps + the density all-gather),
+    # this rank's forces back to the host
+    h_force = torch.empty(rows, 3, dtype=torch.float64).pin_memory()
+    e2e_steps, t_e2e = max(3, min(args.steps, 10)), 0.0
+    for k in range(e2e_steps + 1):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        rs.set_state(h_pos.to(dev, non_blocking=True), h_vel.to(dev, non_blocking=True))
+        h_force.copy_(rs.own_forces(), non_blocking=True)
+        torch.cuda.synchronize()
+        if k > 0:
+            t_e2e += time.perf_counter() - t0
+    e2e_ms, e2e_pairs = aggregate(t_e2e * 1e3, float(rows) * (N - 1) * e2e_steps, world)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    i_both = I_FORCE_ENERGY[spec.prec] + I_DENSITY[spec.prec]
+    peak = PEAK_TFLOPS[spec.prec] * world
+    achieved = i_both * 2.0 * float(N) * (N - 1) / (total_ms * 1e-3 / args.steps) / 1e12
+    cfg = config_dict(spec, N, float(N) * (N - 1), world, 1)
+    cfg["parallelism"] = f"rows{world}: one cluster, contiguous row ranges, 2 all-gathers per step (positions, densities)"
+    line = {"metric": METRIC, "value": total_pairs / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64" if spec.prec == "fp64" else "f32 pair math, f64 accumulation", "data": "synthetic",
+            "md_steps_per_s": args.steps / (total_ms * 1e-3), "config": cfg, "path": "one-sided rows",
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 48 * N,
+                    "d2h_bytes_per_step": 24 * rows, "call": "RowSplitSuttonChen.set_state + own_forces (pinned host buffers)",
+                    "ms_per_call": e2e_ms / e2e_steps},
+            "roofline": {"bound": "alu", "kernel": "allpairs kernels, both sweeps, whole step incl. the two all-gathers",
+                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                         "alu_inst_per_pair": i_both,
+                         "peak_source": f"nominal per GPU x {world} (DESIGN.md section 6)"},
+            "exchanges_per_step": 2, "exchange_bytes_per_step": 32 * N,
+            "cpu_baseline": cpu_baseline(w, 0.0, 1.0)}
+    print(json.dumps(line), flush=True)
+
+
 def launcher_command(args, argv: list[str], port: int) -> list[str]:
     """`--gpus N` without a torchrun environment: the command that starts the N ranks (one per GPU, NCCL)."""
     return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
@@ -537,6 +629,9 @@ def main(argv=None):
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--one-sided", action="store_true",
                     help="all pairs: force the one-sided sweeps (SC_OPT_NEWTON3 = 2) where Newton's third law is the default")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "rows"],
+                    help="N > 1 GPUs: independent replicas (weak scaling, the paper's use) or ONE cluster split by rows "
+                         "(strong scaling, two all-gathers per step)")
     ap.add_argument("--no-also", dest="also", action="store_false",
                     help="default workload only: skip the mixed and cutoff-list variants reported in `also`")
     args = ap.parse_args(argv)
@@ -556,6 +651,8 @@ def main(argv=None):
         raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE = {world}: launch with --nproc-per-node {args.gpus}")
     if args.impl == "reference":
         run_reference(args)
+    elif args.parallel == "rows":
+        run_rows(args)
     else:
         run_ours(args)
 

@@ -151,7 +151,11 @@ typedef struct {
     int32_t newton3_storage;      /* all pairs: 0 = carve the ~N^2 / 8 bytes of partial sums of the Newton's-third-law
                                      sweeps where they apply (2048 <= N <= 262144), 2 = never (SC_OPT_NEWTON3 is then
                                      fixed at 2: one-sided sweeps, O(N) workspace)                                      */
-    int32_t reserved[6];          /* must be 0                                                                          */
+    int32_t row_begin, row_end;   /* all pairs over several GPUs: this context is ONE RANK of a row split
+                                     and computes / integrates the atoms [row_begin, row_end) only, against all N atoms
+                                     (see sc_step_rows).  0, 0 = all rows (one GPU).  Needs r_cut <= 0; the sweeps are the
+                                     one-sided ones (a reaction term would have to cross GPUs)                           */
+    int32_t reserved[4];          /* must be 0                                                                          */
 } sc_create_options;
 
 /* Bytes of device workspace sc_create needs for these arguments (0 on invalid arguments). */
@@ -198,6 +202,27 @@ sc_status sc_kinetic(sc_ctx *ctx, double *h_ke, double *h_temperature);
 /* nsteps velocity-Verlet steps of dt_fs femtoseconds; thermostat NULL = NVE.
  * SC_ERR_STATE if velocities were never set. */
 sc_status sc_step(sc_ctx *ctx, double dt_fs, const sc_thermostat *thermostat, int64_t nsteps);
+/*
+ * One velocity-Verlet step of a ROW SPLIT over several GPUs (PAPER.md:127's two sweeps each
+ * need one exchange).  Every rank holds all N positions and owns the atoms [row_begin, row_end) of its
+ * sc_create_options; the exchanges are the caller's (NCCL all-gathers over NVLink on the caller's communicator and
+ * stream; the library allocates nothing and knows no communicator).  d_pos_all [N*3] and d_rho_all [N] are the
+ * caller's all-atoms arrays.  Per step, on every rank:
+ *   phase 0  first half kick + drift of the own atoms; their new positions are written into d_pos_all (own rows only)
+ *            -> all-gather d_pos_all
+ *   phase 1  all N positions are read from d_pos_all; sweep 1 over the own rows, all j; rho of the own rows is
+ *            written into d_rho_all  -> all-gather d_rho_all
+ *   phase 2  rho^-1/2 of every atom from d_rho_all; sweep 2 over the own rows (and their share of the pair energy);
+ *            second half kick of the own atoms [+ Langevin update, which is local to an atom]
+ * sc_energy / sc_kinetic then return THIS RANK'S SHARE of U and KE (sum over its atoms; the temperature is the
+ * caller's arithmetic on the all-reduced KE), sc_forces / sc_density / sc_get_state the all-atoms arrays with the own
+ * rows current.  Before the first step: sc_set_state (all positions, velocities of at least the own atoms), then
+ * phases 1 and 2 with dt_fs = 0 evaluate the forces.  SC_THERMO_RESCALE needs the global temperature between the
+ * kick and the scale and is refused here (SC_ERR_INVALID).  dt_fs = 0 in phase 2 skips the kick.
+ */
+sc_status sc_step_rows(sc_ctx *ctx, int32_t phase, double dt_fs, const sc_thermostat *thermostat, double *d_pos_all,
+                       double *d_rho_all);
+
 /* Cutoff-path bookkeeping since sc_create: number of list builds; in-range ordered pairs
  * (r_ij^2 < r_cut^2) at the last force evaluation (N(N-1) for all pairs); longest neighbour
  * row at the last build.  Any pointer may be NULL. */

@@ -5,6 +5,7 @@ energy sweep, velocity-Verlet, thermostat) runs in t
 kernels under csrc/.  PyTorch is used for device memory and streams.  There is no CPU
 fallback: if libscmd.so is missing or no CUDA device is present, calls raise.
 """
+from .distributed import RowSplitSuttonChen, row_range  # noqa: F401
 from .binding import (  # noqa: F401
     SC_OK, SC_ERR_INVALID, SC_ERR_CUDA, SC_ERR_NOMEM, SC_ERR_STATE, SC_ERR_NONFINITE, SC_ERR_CAPACITY,
     SC_PREC_FP64, SC_PREC_MIXED, SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN,

@@ -33,7 +33,7 @@ class ScParams(ctypes.Structure):
 
 class ScCreateOptions(ctypes.Structure):
     _fields_ = [("neighbour_capacity", ctypes.c_int32), ("newton3_storage", ctypes.c_int32),
-                ("reserved", ctypes.c_int32 * 6)]
+                ("row_begin", ctypes.c_int32), ("row_end", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4)]
 
 
 class ScThermostat(ctypes.Structure):
@@ -89,6 +89,7 @@ def load_library() -> ctypes.CDLL:
         "sc_energy": (i32, [vp, DP]),
         "sc_kinetic": (i32, [vp, DP, DP]),
         "sc_step": (i32, [vp, dbl, TP, i64]),
+        "sc_step_rows": (i32, [vp, i32, dbl, TP, vp, vp]),
         "sc_stats": (i32, [vp, IP, IP, IP]),
         "sc_eval_host": (i32, [vp, vp, vp, vp, DP]),
         "sc_step_host": (i32, [vp, vp, vp, dbl, TP, i64, DP]),
@@ -161,7 +162,7 @@ class SuttonChen:
 
     def __init__(self, n_atoms: int, *, n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69, r_cut=0.0,
                  precision: int = SC_PREC_FP64, skin: float = 0.0, device=None, stream=None, poison: bool = False,
-                 neighbour_capacity: int = 0, newton3_storage: int = 0):
+                 neighbour_capacity: int = 0, newton3_storage: int = 0, row_begin: int = 0, row_end: int = 0):
         torch = _torch()
         self.lib = load_library()
         self.n_atoms = int(n_atoms)
@@ -169,7 +170,7 @@ class SuttonChen:
         self.params = ScParams(int(n), int(m), float(eps), float(c), float(a), float(mass), float(r_cut))
         self.precision = int(precision)
         self._ctx = ctypes.c_void_p()
-        opts = ScCreateOptions(int(neighbour_capacity), int(newton3_storage))
+        opts = ScCreateOptions(int(neighbour_capacity), int(newton3_storage), int(row_begin), int(row_end))
         with torch.cuda.device(self.device):
             nbytes = self.lib.sc_workspace_bytes_ex(ctypes.byref(self.params), self.n_atoms, self.precision, float(skin),
                                                     ctypes.byref(opts))
@@ -255,6 +256,18 @@ class SuttonChen:
     def sc_step(self, dt_fs: float, nsteps: int, thermostat: ScThermostat | None = None):
         th = ctypes.byref(thermostat) if thermostat is not None else None
         self._check(self.lib.sc_step(self._ctx, float(dt_fs), th, int(nsteps)), "sc_step")
+
+    def sc_step_rows(self, phase: int, dt_fs: float, d_pos_all, d_rho_all, thermostat: ScThermostat | None = None):
+        """One phase of a row-split step (include/scmd.h): d_pos_all [>= N*3], d_rho_all [>= N] are the caller's
+        all-atoms device arrays (they may be longer: padded for equal all-gather chunks)."""
+        torch = _torch()
+        for t_, n_ in ((d_pos_all, 3 * self.n_atoms), (d_rho_all, self.n_atoms)):
+            if t_ is not None and not (t_.is_cuda and t_.dtype == torch.float64 and t_.is_contiguous() and t_.numel() >= n_):
+                raise ScError(SC_ERR_INVALID, "sc_step_rows", f"need a contiguous CUDA float64 tensor of >= {n_} elements")
+        th = ctypes.byref(thermostat) if thermostat is not None else None
+        self._check(self.lib.sc_step_rows(self._ctx, int(phase), float(dt_fs), th,
+                                          0 if d_pos_all is None else d_pos_all.data_ptr(),
+                                          0 if d_rho_all is None else d_rho_all.data_ptr()), "sc_step_rows")
 
     def sc_stats(self):
         a, b, c = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()

@@ -42,6 +42,7 @@ struct PairConsts {
 struct AllPairsArgs {
     double4 *xs;          // [N] (x, y, z, s')
     int n_atoms;
+    int row_begin, row_end;   // rows i this launch computes: [row_begin, row_end) (all of them: 0, N); j always runs over all N
     double *rho;          // [N]    sweep 1 output
     double *force;        // [N*3]  sweep 2 output
     double *partial;      // [gridDim.x] per-CTA partial: sum sqrt(rho) (sweep 1) / sum r^-n (sweep 2)
@@ -99,7 +100,7 @@ __global__ void __launch_bounds__((kMaxConsumerWarps + 1) * 32, 1) allpairs64_ke
 
     // ---- consumer warps ----
     const int g = lane / TPR, q = lane % TPR;
-    const int row0 = blockIdx.x * RPC;
+    const int row0 = a.row_begin + blockIdx.x * RPC;
     int irow[IT];
     double xi[IT], yi[IT], zi[IT], si[IT];
     double acc0[IT], acc1[IT], acc2[IT], acc3[IT];
@@ -206,7 +207,7 @@ __global__ void __launch_bounds__((kMaxConsumerWarps + 1) * 32, 1) allpairs64_ke
             for (int c = 0; c < NV; ++c) v[c] += red[(size_t(w) * RPC + r) * NV + c];
         const int i = row0 + r;
         double contrib = 0.0;
-        if (i < N) {
+        if (i < a.row_end) {
             if constexpr (!FORCE) {
                 const double rho = a.c.am * v[0];
                 if (a.rho) a.rho[i] = rho;
@@ -284,6 +285,7 @@ struct AllPairs32Args {
     FPair *xf;            // [(N + kTileAtoms) / 2 + 1] packed records (negated split coordinates, -s')
     double4 *xs;          // [N] binary64 records: sweep 1 stores s' here too
     int n_atoms;
+    int row_begin, row_end;   // rows i this launch computes (see AllPairsArgs)
     double *rho;
     double *force;
     double *partial;
@@ -327,7 +329,7 @@ __global__ void __launch_bounds__((kMaxConsumerWarps + 1) * 32, 1) allpairs32_ke
     }
 
     const int g = lane / TPR, q = lane % TPR;
-    const int row0 = blockIdx.x * RPC;
+    const int row0 = a.row_begin + blockIdx.x * RPC;
     int irow[IT];
     f2 xh[IT], yh[IT], zh[IT], xl[IT], yl[IT], zl[IT], nsi[IT];      // row values duplicated into both halves
     f2 f0[IT], f1[IT], f2_[IT], f3[IT];
@@ -508,7 +510,7 @@ __global__ void __launch_bounds__((kMaxConsumerWarps + 1) * 32, 1) allpairs32_ke
             for (int c = 0; c < NV; ++c) v[c] += red[(size_t(w) * RPC + r) * NV + c];
         const int i = row0 + r;
         double contrib = 0.0;
-        if (i < N) {
+        if (i < a.row_end) {
             if constexpr (!FORCE) {
                 const double rho = a.c.am * -v[0];                     // the sweep accumulates -r^-m
                 if (a.rho) a.rho[i] = rho;

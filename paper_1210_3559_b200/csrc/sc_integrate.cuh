@@ -40,13 +40,36 @@ __global__ void unpack_positions_kernel(const double4 *__restrict__ xs, double *
     }
 }
 
+// Row split over several GPUs (scmd.h: sc_step_rows): positions of atoms [first, last) out of the records into the
+// caller's all-atoms array, and s' of EVERY record from the all-atoms densities the ranks exchanged (the same
+// expression as the sweep-1 epilogues, so every rank forms the same bits).
+__global__ void export_rows_kernel(const double4 *__restrict__ xs, double *__restrict__ pos_all, int first, int last) {
+    const int i = first + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < last) {
+        const double4 p = xs[i];
+        pos_all[3 * size_t(i)] = p.x; pos_all[3 * size_t(i) + 1] = p.y; pos_all[3 * size_t(i) + 2] = p.z;
+    }
+}
+__global__ void import_density_kernel(const double *__restrict__ rho_all, double4 *__restrict__ xs, FPair *__restrict__ xf,
+                                      RecF *__restrict__ xfr, double *__restrict__ rho, int N, double Bm) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) {
+        const double r = rho_all[i];
+        const double sp = r > 0.0 ? Bm / sqrt(r) : 0.0;                  // reading Q9
+        xs[i].w = sp;
+        rho[i] = r;
+        if (xf) reinterpret_cast<float *>(xf + (i >> 1))[6 + (i & 1)] = -float(sp);
+        if (xfr) xfr[i].s = float(sp);
+    }
+}
+
 // first half kick + drift:  v <- lambda v (pending thermostat scale);  v += hk F;  x += dt v
 // (hk = dt/2 * ACC / m).  ref (may be NULL): positions at the last list build; the largest squared
 // displacement from it goes to scal[kSlotMaxDisp2] through an integer atomicMax (order-free).
 __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__ vel, const double *__restrict__ force,
                                   double *__restrict__ scal, const double4 *__restrict__ ref, FPair *__restrict__ xf, RecF *__restrict__ xfr,
-                                  int N, double hk, double dt) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+                                  int first, int N, double hk, double dt) {
+    const int i = first + blockIdx.x * blockDim.x + threadIdx.x;       // atoms [first, N)
     double d2 = 0.0;
     if (i < N) {
         const double lambda = scal[kSlotLambda];
@@ -81,9 +104,9 @@ __global__ void kick_drift_kernel(double4 *__restrict__ xs, double *__restrict__
 
 // second half kick + per-block sum of |v|^2 -> part[blockIdx.x]
 __global__ void kick_ke_kernel(double *__restrict__ vel, const double *__restrict__ force, double *__restrict__ part,
-                               int N, double hk) {
+                               int first, int N, double hk) {
     __shared__ double scratch[32];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = first + blockIdx.x * blockDim.x + threadIdx.x;       // atoms [first, N)
     double v2 = 0.0;
     if (i < N) {
         double vx = fma(hk, force[3 * size_t(i)], vel[3 * size_t(i)]);
@@ -120,9 +143,9 @@ __device__ __forceinline__ double unit_open(uint32_t w) { return (double(w) + 0.
 
 // second half kick + Langevin update + per-block sum of |v|^2 -> part[blockIdx.x]
 __global__ void kick_langevin_ke_kernel(double *__restrict__ vel, const double *__restrict__ force,
-                                        double *__restrict__ part, int N, double hk, const LangevinArgs lg) {
+                                        double *__restrict__ part, int first, int N, double hk, const LangevinArgs lg) {
     __shared__ double scratch[32];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = first + blockIdx.x * blockDim.x + threadIdx.x;       // atoms [first, N)
     double v2 = 0.0;
     if (i < N) {
         double vx = fma(hk, force[3 * size_t(i)], vel[3 * size_t(i)]);
@@ -145,10 +168,10 @@ __global__ void kick_langevin_ke_kernel(double *__restrict__ vel, const double *
 }
 
 // per-block sum of |v|^2 without a kick (sc_kinetic)
-__global__ void sum_v2_kernel(const double *__restrict__ vel, double *__restrict__ part, int N, double lambda_apply,
+__global__ void sum_v2_kernel(const double *__restrict__ vel, double *__restrict__ part, int first, int N, double lambda_apply,
                               const double *__restrict__ scal) {
     __shared__ double scratch[32];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = first + blockIdx.x * blockDim.x + threadIdx.x;       // atoms [first, N)
     double v2 = 0.0;
     if (i < N) {
         const double l = lambda_apply != 0.0 ? scal[kSlotLambda] : 1.0;

@@ -48,6 +48,8 @@ inline int ceil_div(int64_t a, int64_t b) { return int((a + b - 1) / b); }
 struct sc_ctx {
     sc_params p{};
     int64_t N = 0;
+    int row_begin = 0, row_end = 0;   // rows this context computes and integrates ([0, N) unless created as one rank of a row split)
+    bool split = false;               // one rank of a row split over several GPUs (sc_step_rows)
     int32_t precision = 0;
     double skin = 0.0;
     cudaStream_t stream = nullptr;
@@ -137,8 +139,10 @@ bool create_options_ok(const sc_create_options *o) {
     if (!o) return true;
     for (int r : o->reserved)
         if (r != 0) return false;
-    return o->neighbour_capacity >= 0 && (o->newton3_storage == 0 || o->newton3_storage == 2);
+    return o->neighbour_capacity >= 0 && (o->newton3_storage == 0 || o->newton3_storage == 2) && o->row_begin >= 0 &&
+           o->row_end >= o->row_begin;
 }
+bool row_split(const sc_create_options *o) { return o && o->row_end > o->row_begin; }
 
 constexpr int kMaxCoopBlocks = 4096;
 
@@ -193,13 +197,13 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         c->part_ke = pk; c->scal = scal; c->stage_a = sa; c->stage_b = sb;
         c->rdf_counts = rc; c->rdf_refs = rr; c->rdf_meta = rm; c->msd_part = mp; c->msd_meta = mm;
     }
-    if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms) {
+    if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms && !row_split(opt)) {
         double4 *xb = w.take<double4>(n);
         double *spr = w.take<double>(n);
         unsigned long long *bar = w.take<unsigned long long>(2);
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
     }
-    if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms && !(opt && opt->newton3_storage == 2)) {
+    if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms && !(opt && opt->newton3_storage == 2) && !row_split(opt)) {
         double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
         double4 *ns = w.take<double4>((n + 32) * kN3MaxSegments);
         RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
@@ -278,7 +282,7 @@ int allpairs_residency(sc_ctx *c, const void *fn, int it, int tpr, int warps) {
 //    rows per CTA when it is a tie (x < 1: efficiency = x, i.e. the shape with the most CTAs, down to one row
 //    per CTA), discounted for the lanes that split j inside a warp.
 TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
-    const int64_t N = c->N;
+    const int64_t N = c->row_end - c->row_begin;       // rows to cover (the j range is always all atoms)
     TileChoice best{2, 1, 8};
     int warps_pref = 0;
     if (c->opt_it && c->opt_tpr) {
@@ -315,7 +319,7 @@ TileChoice choose_tile(sc_ctx *c, bool force, bool energy) {
         if (c->opt_tpr) best.tpr = c->opt_tpr;
     }
     int warps = warps_pref ? warps_pref : 8;
-    while (warps > 1 && N / (int64_t(warps) * best.tpr) < 8) warps /= 2;   // >= ~8 pairs per lane and row
+    while (warps > 1 && c->N / (int64_t(warps) * best.tpr) < 8) warps /= 2;   // >= ~8 pairs per lane and row
     if (c->opt_warps) warps = c->opt_warps;
     best.warps = warps;
     return best;
@@ -493,7 +497,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
 
 // all pairs: do the sweeps run the Newton's-third-law kernels (sc_allpairs_n3.cuh) for this context as configured?
 bool n3_wanted(const sc_ctx *c) {
-    if (c->cutoff || !c->n3_part || c->opt_n3 == 2) return false;
+    if (c->cutoff || !c->n3_part || c->opt_n3 == 2 || c->split) return false;
     return c->opt_n3 == 1 || (c->N >= (c->precision == SC_PREC_MIXED ? kN3DefaultMinAtomsMixed : kN3DefaultMinAtoms) &&
                               !c->opt_it && !c->opt_tpr);
 }
@@ -505,14 +509,14 @@ sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
     const void *fn = allpairs_fn(c, tc.it, tc.tpr, force, energy);
     if (!fn) return fail(c, SC_ERR_INVALID, "all-pairs sweep: no kernel for this tile shape%s");
     const int rpc = allpairs_rows_per_cta(tc.it, tc.tpr);
-    const int grid = ceil_div(c->N, rpc);
+    const int grid = ceil_div(c->row_end - c->row_begin, rpc);
     const size_t smem = allpairs_smem_bytes(tc.it, tc.tpr, tc.warps);
     AllPairsArgs a{};
-    a.xs = c->xs; a.n_atoms = int(c->N); a.rho = c->rho; a.force = c->force;
+    a.xs = c->xs; a.n_atoms = int(c->N); a.row_begin = c->row_begin; a.row_end = c->row_end; a.rho = c->rho; a.force = c->force;
     a.partial = force ? c->part_b : c->part_a;
     a.c = c->consts;
     AllPairs32Args a32{};
-    a32.xf = c->xf; a32.xs = c->xs; a32.n_atoms = a.n_atoms; a32.rho = a.rho; a32.force = a.force; a32.partial = a.partial;
+    a32.xf = c->xf; a32.xs = c->xs; a32.n_atoms = a.n_atoms; a32.row_begin = a.row_begin; a32.row_end = a.row_end; a32.rho = a.rho; a32.force = a.force; a32.partial = a.partial;
     a32.c = c->consts;
     void *params[1] = {c->precision == SC_PREC_MIXED ? static_cast<void *>(&a32) : static_cast<void *>(&a)};
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
@@ -531,6 +535,7 @@ sc_status run_sweep(sc_ctx *c, bool force, bool energy) {
 
 sc_status ensure_density(sc_ctx *c) {
     if (c->density_valid) return SC_OK;
+    if (c->split) return fail(c, SC_ERR_STATE, "row split: densities come from the exchange; run sc_step_rows phases 1 and 2 first%s");
     sc_status st = run_sweep(c, false, false);
     if (st == SC_OK) c->density_valid = true;
     return st;
@@ -538,6 +543,7 @@ sc_status ensure_density(sc_ctx *c) {
 
 sc_status ensure_forces(sc_ctx *c, bool energy) {
     if (c->forces_valid && (!energy || c->energy_valid)) return SC_OK;
+    if (c->split) return fail(c, SC_ERR_STATE, "row split: run sc_step_rows phases 1 and 2 to evaluate the forces%s");
     if (c->profile) cudaEventRecord(c->ev[0], c->stream);
     sc_status st = ensure_density(c);
     if (st != SC_OK) return st;
@@ -596,7 +602,7 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
 constexpr int64_t kSmallDefaultMaxAtoms = 4096, kSmallDefaultMaxAtomsMixed = 2304;
 
 bool small_path_wanted(const sc_ctx *c) {
-    if (c->cutoff || !c->xs_b || c->opt_persistent == 2 || c->profile) return false;
+    if (c->cutoff || !c->xs_b || c->opt_persistent == 2 || c->profile || c->split) return false;
     if (c->N > kSmallMaxAtoms) return false;
     return c->opt_persistent == 1 || c->N <= (c->precision == SC_PREC_MIXED ? kSmallDefaultMaxAtomsMixed : kSmallDefaultMaxAtoms);
 }
@@ -678,6 +684,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
             return fail(c, SC_ERR_INVALID, "sc_step: Langevin damping must be finite and >= 0 (1/fs)%s");
     }
     if (nsteps == 0) return SC_OK;
+    if (c->split) return fail(c, SC_ERR_STATE, "sc_step: this context is one rank of a row split; use sc_step_rows%s");
     sc_status st = ensure_forces(c, false);
     if (st != SC_OK) return st;
     if (small_path_wanted(c)) return run_small_steps(c, dt, th, thermo, nsteps);
@@ -687,7 +694,7 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     const double ndof = double(3 * c->N - 3);
     for (int64_t k = 1; k <= nsteps; ++k) {
         kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, c->cutoff ? c->xs_ref : nullptr,
-                                                        c->xf, c->xfr, N, hk, dt);
+                                                        c->xf, c->xfr, 0, N, hk, dt);
         SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
@@ -703,10 +710,10 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
             lg.key0 = uint32_t(th->seed); lg.key1 = uint32_t(th->seed >> 32);
             lg.step_lo = uint32_t(c->langevin_step); lg.step_hi = uint32_t(c->langevin_step >> 32);
             lg.perm = c->cutoff ? c->perm : nullptr;
-            kick_langevin_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk, lg);
+            kick_langevin_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, 0, N, hk, lg);
             c->langevin_step += 1;
         } else {
-            kick_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, N, hk);
+            kick_ke_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, 0, N, hk);
         }
         c->launches += 1;
         if (thermo == SC_THERMO_RESCALE || last) {
@@ -741,6 +748,7 @@ size_t sc_workspace_bytes_ex(const sc_params *params, int64_t n_atoms, int32_t p
     if (precision != SC_PREC_FP64 && precision != SC_PREC_MIXED) return 0;
     if (!(skin >= 0.0) || !create_options_ok(options)) return 0;
     if (params->r_cut > 0.0 && n_atoms > kCutoffMaxAtoms) return 0;       // run words hold 29-bit indices
+    if (row_split(options) && (params->r_cut > 0.0 || options->row_end > n_atoms)) return 0;   // the row split is all pairs only
     return carve(nullptr, nullptr, n_atoms, params, precision, skin, options);
 }
 
@@ -763,6 +771,7 @@ sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precisi
     if (!(skin >= 0.0) || !d_workspace || !create_options_ok(options)) return SC_ERR_INVALID;
     if (reinterpret_cast<uintptr_t>(d_workspace) % kAlign) return SC_ERR_INVALID;
     if (params->r_cut > 0.0 && n_atoms > kCutoffMaxAtoms) return SC_ERR_INVALID;
+    if (row_split(options) && (params->r_cut > 0.0 || options->row_end > n_atoms)) return SC_ERR_INVALID;
     const size_t need = sc_workspace_bytes_ex(params, n_atoms, precision, skin, options);
     if (workspace_bytes < need) return SC_ERR_NOMEM;
     int dev = 0, count = 0;
@@ -771,6 +780,8 @@ sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precisi
     sc_ctx *c = new (std::nothrow) sc_ctx();
     if (!c) return SC_ERR_NOMEM;
     c->p = *params; c->N = n_atoms; c->precision = precision; c->skin = skin;
+    c->row_begin = 0; c->row_end = int(n_atoms);
+    if (row_split(options)) { c->split = true; c->row_begin = options->row_begin; c->row_end = options->row_end; }
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
     carve(c, d_workspace, n_atoms, params, precision, skin, options);
@@ -1008,9 +1019,10 @@ sc_status sc_kinetic(sc_ctx *c, double *h_ke, double *h_temperature) {
     if (!c->have_vel) return fail(c, SC_ERR_STATE, "sc_kinetic: no velocities set%s");
     sc_status st = flush_lambda(c);
     if (st != SC_OK) return st;
-    const int N = int(c->N), nb = ceil_div(N, kBlock);
-    sum_v2_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->part_ke, N, 0.0, c->scal);
-    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->part_ke, nb, c->scal, c->p.mass, double(3 * c->N - 3), 0, 0.0);
+    // one rank of a row split: its own atoms' share of the kinetic energy; T is then the caller's arithmetic on the sum
+    const int nb = ceil_div(c->row_end - c->row_begin, kBlock);
+    sum_v2_kernel<<<nb, kBlock, 0, c->stream>>>(c->vel, c->part_ke, c->row_begin, c->row_end, 0.0, c->scal);
+    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->part_ke, nb, c->scal, c->p.mass, c->split ? 0.0 : double(3 * c->N - 3), 0, 0.0);
     SC_CUDA_CHECK(c, cudaGetLastError());
     c->launches += 2;
     double s[kSlotTemp + 1];
@@ -1025,6 +1037,76 @@ sc_status sc_kinetic(sc_ctx *c, double *h_ke, double *h_temperature) {
 sc_status sc_step(sc_ctx *c, double dt_fs, const sc_thermostat *thermostat, int64_t nsteps) {
     if (!c) return SC_ERR_INVALID;
     return do_step(c, dt_fs, thermostat, nsteps);
+}
+
+sc_status sc_step_rows(sc_ctx *c, int32_t phase, double dt, const sc_thermostat *th, double *d_pos_all, double *d_rho_all) {
+    if (!c) return SC_ERR_INVALID;
+    if (!c->split) return fail(c, SC_ERR_STATE, "sc_step_rows: the context was not created as a rank of a row split%s");
+    if (phase < 0 || phase > 2 || !(dt >= 0.0) || !std::isfinite(dt))
+        return fail(c, SC_ERR_INVALID, "sc_step_rows: phase must be 0, 1 or 2 and dt >= 0%s");
+    if (!c->have_pos) return fail(c, SC_ERR_STATE, "sc_step_rows: no positions set%s");
+    int thermo = th ? th->kind : SC_THERMO_NONE;
+    if (thermo != SC_THERMO_NONE && thermo != SC_THERMO_LANGEVIN)
+        return fail(c, SC_ERR_INVALID, "sc_step_rows: only NVE and the Langevin thermostat work rank by rank%s");
+    if (thermo == SC_THERMO_LANGEVIN && !(th->gamma >= 0.0 && std::isfinite(th->gamma) && th->T_end >= 0.0 && std::isfinite(th->T_end)))
+        return fail(c, SC_ERR_INVALID, "sc_step_rows: Langevin damping and temperature must be finite and >= 0%s");
+    const int N = int(c->N), rb = c->row_begin, re = c->row_end, rows = re - rb;
+    const int nb_rows = ceil_div(rows, kBlock), nb_all = ceil_div(N, kBlock);
+    const double hk = 0.5 * dt * kAcc / c->p.mass;
+    if (phase == 0) {
+        if (!d_pos_all) return fail(c, SC_ERR_INVALID, "sc_step_rows: d_pos_all is NULL%s");
+        if (!c->have_vel || !c->forces_valid)
+            return fail(c, SC_ERR_STATE, "sc_step_rows: phase 0 needs velocities and forces (phases 1, 2 with dt = 0 evaluate them)%s");
+        kick_drift_kernel<<<nb_rows, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, nullptr, c->xf, c->xfr, rb, re, hk, dt);
+        export_rows_kernel<<<nb_rows, kBlock, 0, c->stream>>>(c->xs, d_pos_all, rb, re);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 2;
+        c->density_valid = c->forces_valid = c->energy_valid = false;
+        return SC_OK;
+    }
+    if (phase == 1) {
+        if (!d_pos_all || !d_rho_all) return fail(c, SC_ERR_INVALID, "sc_step_rows: NULL all-atoms array%s");
+        pack_positions_kernel<<<nb_all, kBlock, 0, c->stream>>>(d_pos_all, c->xs, c->xf, c->xfr, N);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+        c->density_valid = c->forces_valid = c->energy_valid = false;
+        sc_status st = run_sweep(c, false, false);
+        if (st != SC_OK) return st;
+        SC_CUDA_CHECK(c, cudaMemcpyAsync(d_rho_all + rb, c->rho + rb, sizeof(double) * size_t(rows), cudaMemcpyDeviceToDevice, c->stream));
+        return SC_OK;
+    }
+    if (!d_rho_all) return fail(c, SC_ERR_INVALID, "sc_step_rows: d_rho_all is NULL%s");
+    import_density_kernel<<<nb_all, kBlock, 0, c->stream>>>(d_rho_all, c->xs, c->xf, c->xfr, c->rho, N, c->consts.Bm);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 1;
+    c->density_valid = true;
+    if (c->emb_pending) {
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, c->emb_pending, c->scal, kSlotEEmb, -c->consts.eps_c);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+        c->emb_pending = 0;
+    }
+    sc_status st = run_sweep(c, true, true);
+    if (st != SC_OK) return st;
+    c->forces_valid = c->energy_valid = true;
+    if (dt > 0.0) {
+        if (!c->have_vel) return fail(c, SC_ERR_STATE, "sc_step_rows: velocities were never set%s");
+        if (thermo == SC_THERMO_LANGEVIN) {
+            LangevinArgs lg{};
+            lg.c1 = std::exp(-th->gamma * dt);
+            lg.c2 = std::sqrt((1.0 - lg.c1 * lg.c1) * kBoltzmann * th->T_end * kAcc / c->p.mass);
+            lg.key0 = uint32_t(th->seed); lg.key1 = uint32_t(th->seed >> 32);
+            lg.step_lo = uint32_t(c->langevin_step); lg.step_hi = uint32_t(c->langevin_step >> 32);
+            lg.perm = nullptr;
+            kick_langevin_ke_kernel<<<nb_rows, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, rb, re, hk, lg);
+            c->langevin_step += 1;
+        } else {
+            kick_ke_kernel<<<nb_rows, kBlock, 0, c->stream>>>(c->vel, c->force, c->part_ke, rb, re, hk);
+        }
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return SC_OK;
 }
 
 sc_status sc_stats(sc_ctx *c, int64_t *n_rebuilds, int64_t *n_pairs_in_cut, int64_t *max_neighbours) {
