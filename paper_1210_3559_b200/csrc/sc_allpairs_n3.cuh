@@ -24,7 +24,7 @@
 
 namespace scmd {
 
-constexpr int kN3Warps = 12;
+constexpr int kN3Warps = 12;          // warps per SM the register allocation allows (168 registers): ONE CTA of 12 or TWO of 6
 constexpr double kN3Far = 1.0e100;
 
 struct N3Args {
@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     __shared__ double red[kN3Warps][IT][3][32];            // epilogue: per-warp row sums
     __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int NW = blockDim.x >> 5;                          // 12, or 6 (two CTAs per SM: finer tiles for mid-size clusters)
     const int N = a.n_atoms;
     const int row0 = blockIdx.x * RB;
     if ((row0 >> 5) + int(blockIdx.y) * a.seg_chunks >= ((a.n_atoms + 31) >> 5)) {   // no such segment in this block's triangle
@@ -86,7 +87,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
-    for (int c = c_begin + warp; c < c_end; c += kN3Warps) {
+    for (int c = c_begin + warp; c < c_end; c += NW) {
         int jidx = (c << 5) + lane;
         double xj, yj, zj, sj;
         if (jidx < N) {
@@ -173,10 +174,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         if (lane == 0) red_e[warp] = esum;
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < RB; r += kN3Warps * 32) {
+    for (int r = threadIdx.x; r < RB; r += NW * 32) {
         const int k = r >> 5, l = r & 31, i = row0 + r;
         double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        for (int w = 0; w < kN3Warps; ++w) {
+        for (int w = 0; w < NW; ++w) {
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     if constexpr (FORCE && ENERGY) {
         if (threadIdx.x == 0) {
             double tot = 0.0;
-            for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
+            for (int w = 0; w < NW; ++w) tot += red_e[w];
             a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;   // every unordered pair stands for two ordered ones
         }
     }
@@ -227,6 +228,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     __shared__ double red[kN3Warps][IT][3][32];
     __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int NW = blockDim.x >> 5;
     const int N = a.n_atoms;
     const int row0 = blockIdx.x * RB;
     // a.seg_chunks counts chunks of 32 atoms and is even here: segments of seg_chunks / 2 chunks of 64
@@ -262,7 +264,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         if (j < N) return a.xfr[j];
         return RecF{-kFarF * float((j & 63) + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
     };
-    for (int c = c_begin + warp; c < c_end; c += kN3Warps) {
+    for (int c = c_begin + warp; c < c_end; c += NW) {
         const int ja = (c << 6) + lane, jb = ja + 32;
         int jidx_a = ja, jidx_b = jb;
         const RecF pa = fetch(ja), pb = fetch(jb);
@@ -380,10 +382,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         if (lane == 0) red_e[warp] = esum;
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < RB; r += kN3Warps * 32) {
+    for (int r = threadIdx.x; r < RB; r += NW * 32) {
         const int k = r >> 5, l = r & 31, i = row0 + r;
         double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        for (int w = 0; w < kN3Warps; ++w) {
+        for (int w = 0; w < NW; ++w) {
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
@@ -392,7 +394,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     if constexpr (FORCE && ENERGY) {
         if (threadIdx.x == 0) {
             double tot = 0.0;
-            for (int w = 0; w < kN3Warps; ++w) tot += red_e[w];
+            for (int w = 0; w < NW; ++w) tot += red_e[w];
             a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;
         }
     }

@@ -109,6 +109,7 @@ struct sc_ctx {
     int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0, opt_shift = 0;
     int emb_pending = 0;          // sweep 1 left this many per-CTA sums of sqrt(rho) in part_a, not yet totalled into U_emb
     int n3_seg = 0;               // j-segment length of the Newton's-third-law sweeps (chunks of 32), chosen at first use
+    int n3_warps = 12;            // ... and their warps per CTA (12, or 6 with two CTAs per SM)
 
     // profiling
     bool profile = false;
@@ -427,31 +428,41 @@ sc_status check_flags(sc_ctx *c) {
 // 12 warps over the segment's chunks (mixed: chunks of 64, and a quarter unit of fixed cost: calibrated) -- and the
 // shortest makespan wins.  Against measurement the simulation picked the fastest candidate at 6 (FP64) and 5 (mixed)
 // of 8 sizes between 7000 and 32768 and was within 1 - 6 % at the others; above 49152 the choice is flat within 1 %.
-int choose_n3_segment(const sc_ctx *c) {
+// Returns the segment length; *warps_out = warps per CTA: 12.  TWO CTAs of 6 warps per SM (same registers, tiles half as
+// large, twice the slots: by this simulation the cure for N = 8000, where 252 tiles fill 296 slot-rounds to 80 %) were
+// measured in round 2 and are much SLOWER (N = 8000: 0.244 against 0.168 ms per step, N = 16384: 0.515 against 0.437):
+// SC_OPT_WARPS_PER_CTA <= 6 still selects them, the default never does.
+int choose_n3_segment(const sc_ctx *c, int *warps_out) {
     const int N = int(c->N), nch = ceil_div(N, 32), nb = ceil_div(N, 32 * kN3RowsPerThread);
     const int unit = c->precision == SC_PREC_MIXED ? 2 : 1;
     const double fixed = c->precision == SC_PREC_MIXED ? 0.25 : 1.0;
-    int best_seg = 0, last_seg = 0;
+    int best_seg = 0, best_w = kN3Warps;
     double best_t = 0.0;
-    for (int want : {8, 12, 16, 20, 24}) {
-        const int seg = round_up(ceil_div(nch, want), kN3Warps * unit), nseg = ceil_div(nch, seg);
-        if (nseg > kN3MaxSegments || seg == last_seg) continue;
-        last_seg = seg;
-        std::priority_queue<double, std::vector<double>, std::greater<double>> sm;
-        for (int k = 0; k < c->sm_count; ++k) sm.push(0.0);
-        double makespan = 0.0;
-        for (int y = 0; y < nseg; ++y)
-            for (int b = 0; b < nb; ++b) {
-                const int c_begin = b * kN3RowsPerThread + y * seg;
-                if (c_begin >= nch) continue;
-                const int chunks = ceil_div(std::min(nch, c_begin + seg) - c_begin, unit);
-                const double t = sm.top() + fixed + double(ceil_div(chunks, kN3Warps));
-                sm.pop();
-                sm.push(t);
-                makespan = std::max(makespan, t);
-            }
-        if (!best_seg || makespan < best_t) { best_seg = seg; best_t = makespan; }
+    for (int nw : {kN3Warps, kN3Warps / 2}) {
+        if (nw != ((c->opt_warps && c->opt_warps <= 6) ? 6 : 12)) continue;    // SC_OPT_WARPS_PER_CTA <= 6 forces 6
+        int last_seg = 0;
+        for (int want : {8, 12, 16, 20, 24}) {
+            const int seg = round_up(ceil_div(nch, want), nw * unit), nseg = ceil_div(nch, seg);
+            if (nseg > kN3MaxSegments || seg == last_seg) continue;
+            last_seg = seg;
+            std::priority_queue<double, std::vector<double>, std::greater<double>> sm;
+            for (int k = 0; k < c->sm_count * (kN3Warps / nw); ++k) sm.push(0.0);
+            double makespan = 0.0;
+            for (int y = 0; y < nseg; ++y)
+                for (int b = 0; b < nb; ++b) {
+                    const int c_begin = b * kN3RowsPerThread + y * seg;
+                    if (c_begin >= nch) continue;
+                    const int chunks = ceil_div(std::min(nch, c_begin + seg) - c_begin, unit);
+                    // a CTA of nw warps shares its SM's pipes with 12 / nw - 1 others: per-warp progress is the same
+                    const double t = sm.top() + fixed + double(ceil_div(chunks, nw));
+                    sm.pop();
+                    sm.push(t);
+                    makespan = std::max(makespan, t);
+                }
+            if (!best_seg || makespan < best_t - 1e-9) { best_seg = seg; best_t = makespan; best_w = nw; }
+        }
     }
+    *warps_out = best_w;
     return best_seg;
 }
 
@@ -471,12 +482,12 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     N3FArgs af{};
     af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
     // j segments cut the first row block's triangle; each a multiple of the 12 warps (choose_n3_segment)
-    if (!c->n3_seg) c->n3_seg = choose_n3_segment(c);
+    if (!c->n3_seg) c->n3_seg = choose_n3_segment(c, &c->n3_warps);
     const int nch = ceil_div(N, 32), seg = c->n3_seg, nseg = ceil_div(nch, seg);
     a.seg_chunks = seg;
     af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
     void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
-    cudaError_t e = cudaLaunchKernel(fn, dim3(nb, nseg), dim3(kN3Warps * 32), params, 0, c->stream);
+    cudaError_t e = cudaLaunchKernel(fn, dim3(nb, nseg), dim3(c->n3_warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
     N3FinalArgs f{};
     f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
@@ -854,7 +865,7 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
         case SC_OPT_WARPS_PER_CTA:
             if (value < 0 || value > (c->cutoff ? kNlistMaxBlock / 32 : kMaxConsumerWarps))
                 return fail(c, SC_ERR_INVALID, "warps per CTA must be 0..8%s");
-            c->opt_warps = int(value); break;
+            c->opt_warps = int(value); c->n3_seg = 0; break;
         case SC_OPT_PERSISTENT:
             if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "persistent must be 0, 1 or 2%s");
             c->opt_persistent = int(value); break;
