@@ -26,6 +26,7 @@ namespace scmd {
 
 constexpr int kN3Warps = 12;          // warps per SM the register allocation allows (168 registers): ONE CTA of 12 or TWO of 6
 constexpr double kN3Far = 1.0e100;
+constexpr float kN3FarTerm = 1.4901161193847656e-08f;   // 2^-26: r^-6 of a pair 20 A apart (mixed sweep 1: near / far sums)
 
 struct N3Args {
     const double4 *xs;      // [N] (x, y, z, s')
@@ -88,7 +89,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
     for (int c = c_begin + warp; c < c_end; c += NW) {
-        int jidx = (c << 5) + lane;
+        const int jidx = (c << 5) + lane;
         double xj, yj, zj, sj;
         if (jidx < N) {
             const double4 p = a.xs[jidx];
@@ -97,16 +98,20 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
             xj = -kN3Far * double(lane + 1); yj = kN3Far; zj = kN3Far; sj = 0.0;
         }
         const int jhome = jidx;
-        double g0 = 0.0, g1 = 0.0, g2 = 0.0;               // reaction sums travelling with the record
         const bool diag = c < cb + IT;                     // warp-uniform
-        auto step = [&](auto masked) {
-            // the record of the NEXT step is fetched first (positions do not change): its shuffle latency hides
+        // One rotation step: evaluate the IT rows against the record held (`in`), hand it on with the reaction sums
+        // accumulated on it so far (`out`).  Two register sets alternate (A -> B, B -> A): no value is ever moved back
+        // into a loop-carried register (10 moves per step when the step updated one set in place).
+        struct JRec { double x, y, z, s, g0, g1, g2; int j; };
+        auto step = [&](auto masked, const JRec &in, JRec &out) {
+            const double xj = in.x, yj = in.y, zj = in.z, sj = in.s;
+            const int jidx = in.j;
+            double g0 = in.g0, g1 = in.g1, g2 = in.g2;     // reaction sums travelling with the record
+            // the record of the NEXT step is sent first (positions do not change): its shuffle latency hides
             // behind this step's arithmetic; only the reaction sums have to wait for it
-            const double xn = rot1(xj), yn = rot1(yj), zn = rot1(zj);
-            double sn = 0.0;
-            if constexpr (FORCE) sn = rot1(sj);
-            int jn = 0;
-            if constexpr (decltype(masked)::value) jn = rot1(jidx);
+            out.x = rot1(xj); out.y = rot1(yj); out.z = rot1(zj);
+            if constexpr (FORCE) out.s = rot1(sj);
+            if constexpr (decltype(masked)::value) out.j = rot1(jidx);
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
                 const double dx = xi[k] - xj, dy = yi[k] - yj, dz = zi[k] - zj;
@@ -145,17 +150,25 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
                 }
             }
             // pass the sums on with the record
-            g0 = rot1(g0);
-            if constexpr (FORCE) { g1 = rot1(g1); g2 = rot1(g2); sj = sn; }
-            xj = xn; yj = yn; zj = zn;
-            if constexpr (decltype(masked)::value) jidx = jn;
+            out.g0 = rot1(g0);
+            if constexpr (FORCE) { out.g1 = rot1(g1); out.g2 = rot1(g2); }
         };
+        JRec A, B;
+        A.x = xj; A.y = yj; A.z = zj; A.s = sj; A.g0 = A.g1 = A.g2 = 0.0; A.j = jidx;
+        B = A;
         if (diag) {
-            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
+            for (int s = 0; s < 32; s += 2) {
+                step(std::integral_constant<bool, true>{}, A, B);
+                step(std::integral_constant<bool, true>{}, B, A);
+            }
         } else {
-#pragma unroll 4
-            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
+#pragma unroll 2
+            for (int s = 0; s < 32; s += 2) {
+                step(std::integral_constant<bool, false>{}, A, B);
+                step(std::integral_constant<bool, false>{}, B, A);
+            }
         }
+        const double g0 = A.g0, g1 = A.g1, g2 = A.g2;
         // the record is home again (32 rotations by one lane)
         if (jhome < N) {
             if constexpr (FORCE) part[jhome - row0] = make_double4(g0, g1, g2, 0.0);
@@ -218,8 +231,8 @@ struct N3FArgs {
 // halves of Blackwell's binary32 pair registers (PTX add / mul / fma.f32x2, SASS FADD2 / FMUL2 / FFMA2), j-side values
 // NEGATED so that only additions are needed; the rows i are duplicated into both halves once per launch.  One
 // rotation step is then 4 rows x 2 records = 8 pairs per lane for the instruction count of 4.
-__device__ __forceinline__ f2 rot1_f2(f2 v) {
-    return f2_make(rot1(f2_lo(v)), rot1(f2_hi(v)));
+__device__ __forceinline__ f2 rot1_f2(f2 v) {      // the 64-bit shuffle: two SHFL on the register pair, no repacking moves
+    return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31);
 }
 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
@@ -266,24 +279,29 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     };
     for (int c = c_begin + warp; c < c_end; c += NW) {
         const int ja = (c << 6) + lane, jb = ja + 32;
-        int jidx_a = ja, jidx_b = jb;
         const RecF pa = fetch(ja), pb = fetch(jb);
         // negated j records, (a, b) in the (low, high) halves
         f2 nxh = f2_make(-pa.xh, -pb.xh), nyh = f2_make(-pa.yh, -pb.yh), nzh = f2_make(-pa.zh, -pb.zh);
         f2 nxl = f2_make(-pa.xl, -pb.xl), nyl = f2_make(-pa.yl, -pb.yl), nzl = f2_make(-pa.zl, -pb.zl);
-        f2 sj = f2_make(pa.s, pb.s);
-        f2 g0 = zero2, g1 = zero2, g2 = zero2, gfar = zero2, e2 = zero2, e2far = zero2;
+        const f2 sj = f2_make(pa.s, pb.s);
         f2 f0[IT], f1[IT], f2v[IT], ffar[IT];
 #pragma unroll
         for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2v[k] = ffar[k] = zero2;
         const bool diag = c < cb + IT / 2;                 // the block's own rows span IT / 2 chunks of 64
-        auto step = [&](auto masked) {
-            const f2 xhn = rot1_f2(nxh), yhn = rot1_f2(nyh), zhn = rot1_f2(nzh);
-            const f2 xln = rot1_f2(nxl), yln = rot1_f2(nyl), zln = rot1_f2(nzl);
-            f2 sjn = zero2;
-            if constexpr (FORCE) sjn = rot1_f2(sj);
-            int jan = 0, jbn = 0;
-            if constexpr (decltype(masked)::value) { jan = rot1(jidx_a); jbn = rot1(jidx_b); }
+        // One rotation step: the lane evaluates its IT rows against the two records it holds (`in`) and hands them, with
+        // the sums accumulated on them, to the next lane (`out`).  Two register sets alternate (A -> B, B -> A), so no
+        // value has to be moved back into a loop-carried register (44 moves per two steps when written in place).
+        struct JRec { f2 xh, yh, zh, xl, yl, zl, s, g0, g1, g2, gf; int ja, jb; };
+        auto step = [&](auto masked, const JRec &in, JRec &out) {
+            const f2 nxh = in.xh, nyh = in.yh, nzh = in.zh, nxl = in.xl, nyl = in.yl, nzl = in.zl, sj = in.s;
+            const int jidx_a = in.ja, jidx_b = in.jb;
+            f2 g0 = in.g0, g1 = in.g1, g2 = in.g2, gfar = in.gf;
+            // the records do not change: send them on first, their shuffle latency hides behind the arithmetic
+            out.xh = rot1_f2(nxh); out.yh = rot1_f2(nyh); out.zh = rot1_f2(nzh);
+            out.xl = rot1_f2(nxl); out.yl = rot1_f2(nyl); out.zl = rot1_f2(nzl);
+            if constexpr (FORCE) out.s = rot1_f2(sj);
+            if constexpr (decltype(masked)::value) { out.ja = rot1(jidx_a); out.jb = rot1(jidx_b); }
+            f2 estep = zero2;                              // sum r^-n over the 2 IT pairs of this step
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
                 const f2 dx = f2_add(f2_add(xh[k], nxh), f2_add(xl[k], nxl));
@@ -307,10 +325,11 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
                         if constexpr (decltype(masked)::value) y = f2_make(ka ? f2_lo(y) : 0.f, kb ? f2_hi(y) : 0.f);
                         term = (ME > 0) ? f2_ipow_c<(ME > 0 ? ME : 1)>(y) : f2_ipow_rt(y, m_exp);
                     }
-                    // two sums per accumulator (pairs closer than 20 A / the rest): see the header of this section
-                    const bool fa = f2_lo(r2) > 400.0f, fb = f2_hi(r2) > 400.0f;
-                    const f2 tn = f2_make(fa ? 0.f : f2_lo(term), fb ? 0.f : f2_hi(term));
-                    const f2 tf = f2_make(fa ? f2_lo(term) : 0.f, fb ? f2_hi(term) : 0.f);
+                    // two sums per accumulator (see the header of this section), split WITHOUT selects: the part of a
+                    // term below 2^-26 A^-m (r^-6 at 20 A) goes to the far sum, what exceeds it to the near sum:
+                    // tf = min(term, T) is exact, tn = term - tf is 0 for a far term and one rounding for a near one
+                    const f2 tf = f2_make(fminf(f2_lo(term), kN3FarTerm), fminf(f2_hi(term), kN3FarTerm));
+                    const f2 tn = f2_fma(tf, mone2, term);
                     f0[k] = f2_add(f0[k], tn); ffar[k] = f2_add(ffar[k], tf);
                     g0 = f2_add(g0, tn); gfar = f2_add(gfar, tf);
                 } else {
@@ -330,28 +349,37 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
                         pnw = (NE > 0) ? f2_ipow_c<(NE > 0 ? NE : 1)>(y) : f2_ipow_rt(y, n_exp);
                         coef = f2_mul(w, f2_fma(An2, pnw, f2_mul(nss, pm)));
                     }
-                    if constexpr (ENERGY) {                 // two sums again: r^-9 of a pair beyond 10 A must not meet a
-                        const bool ea = f2_lo(r2) > 100.0f, eb = f2_hi(r2) > 100.0f;   // nearest-neighbour term
-                        e2 = f2_add(e2, f2_make(ea ? 0.f : f2_lo(pnw), eb ? 0.f : f2_hi(pnw)));
-                        e2far = f2_add(e2far, f2_make(ea ? f2_lo(pnw) : 0.f, eb ? f2_hi(pnw) : 0.f));
-                    }
+                    if constexpr (ENERGY) estep = f2_add(estep, pnw);
                     f0[k] = f2_fma(coef, dx, f0[k]); f1[k] = f2_fma(coef, dy, f1[k]); f2v[k] = f2_fma(coef, dz, f2v[k]);
                     const f2 ncoef = f2_mul(coef, mone2);
                     g0 = f2_fma(ncoef, dx, g0); g1 = f2_fma(ncoef, dy, g1); g2 = f2_fma(ncoef, dz, g2);
                 }
             }
-            g0 = rot1_f2(g0);
-            if constexpr (FORCE) { g1 = rot1_f2(g1); g2 = rot1_f2(g2); sj = sjn; }
-            else gfar = rot1_f2(gfar);
-            nxh = xhn; nyh = yhn; nzh = zhn; nxl = xln; nyl = yln; nzl = zln;
-            if constexpr (decltype(masked)::value) { jidx_a = jan; jidx_b = jbn; }
+            // The pair energy leaves binary32 after EVERY step (2 IT terms): a sum that lived for a whole chunk lost
+            // the far terms to the first nearest-neighbour term it met (1e-7 of the energy, measured in round 1, then
+            // cured by two selected sums per pair: 24 instructions per step; this is 3)
+            if constexpr (FORCE && ENERGY) esum += double(f2_lo(estep) + f2_hi(estep));
+            // the sums travel with the record
+            out.g0 = rot1_f2(g0);
+            if constexpr (FORCE) { out.g1 = rot1_f2(g1); out.g2 = rot1_f2(g2); }
+            else out.gf = rot1_f2(gfar);
         };
+        JRec A, B;
+        A.xh = nxh; A.yh = nyh; A.zh = nzh; A.xl = nxl; A.yl = nyl; A.zl = nzl; A.s = sj;
+        A.g0 = A.g1 = A.g2 = A.gf = zero2; A.ja = ja; A.jb = jb;
+        B = A;
         if (diag) {
-            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, true>{});
+            for (int s = 0; s < 32; s += 2) {
+                step(std::integral_constant<bool, true>{}, A, B);
+                step(std::integral_constant<bool, true>{}, B, A);
+            }
         } else {
-#pragma unroll 2
-            for (int s = 0; s < 32; ++s) step(std::integral_constant<bool, false>{});
+            for (int s = 0; s < 32; s += 2) {
+                step(std::integral_constant<bool, false>{}, A, B);
+                step(std::integral_constant<bool, false>{}, B, A);
+            }
         }
+        const f2 g0 = A.g0, g1 = A.g1, g2 = A.g2, gfar = A.gf;             // both records are home again
         // both records are home again
         if constexpr (FORCE) {
             if (ja < N) part[ja - row0] = make_double4(double(f2_lo(g0)), double(f2_lo(g1)), double(f2_lo(g2)), 0.0);
@@ -370,7 +398,6 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
                 F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
             }
         }
-        if constexpr (FORCE && ENERGY) esum += double(f2_lo(e2) + f2_hi(e2)) + double(f2_lo(e2far) + f2_hi(e2far));
     }
 #pragma unroll
     for (int k = 0; k < IT; ++k) {

@@ -430,7 +430,8 @@ sc_status check_flags(sc_ctx *c) {
 // of 8 sizes between 7000 and 32768 and was within 1 - 6 % at the others; above 49152 the choice is flat within 1 %.
 // Returns the segment length; *warps_out = warps per CTA: 12.  TWO CTAs of 6 warps per SM (same registers, tiles half as
 // large, twice the slots: by this simulation the cure for N = 8000, where 252 tiles fill 296 slot-rounds to 80 %) were
-// measured in round 2 and are much SLOWER (N = 8000: 0.244 against 0.168 ms per step, N = 16384: 0.515 against 0.437):
+// measured in round 2 (both resident) and are SLOWER (200-step calls: N = 6144 120 against 102, N = 8000 217 against 140,
+// N = 16384 479 against 401 us per step: a tile lasts as long as its slowest warp, and with 3 chunks per warp one diagonal chunk decides):
 // SC_OPT_WARPS_PER_CTA <= 6 still selects them, the default never does.
 int choose_n3_segment(const sc_ctx *c, int *warps_out) {
     const int N = int(c->N), nch = ceil_div(N, 32), nb = ceil_div(N, 32 * kN3RowsPerThread);
@@ -487,6 +488,8 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     a.seg_chunks = seg;
     af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
     void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
+    if (c->n3_warps < kN3Warps)       // two CTAs of 6 warps per SM need 2 x 37 KB of shared memory
+        cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, int(cudaSharedmemCarveoutMaxShared));
     cudaError_t e = cudaLaunchKernel(fn, dim3(nb, nseg), dim3(c->n3_warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
     N3FinalArgs f{};
