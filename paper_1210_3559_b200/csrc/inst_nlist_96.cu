@@ -12,7 +12,7 @@ cudaError_t launch_nlist_96(int grid, int block, const NlistArgs &a, bool force,
         // run-length rows: 6 resident CTAs x ~22 KB of expanded rows need the large shared-memory carve-out; index rows use
         // no shared memory and want all of it as L1 (the gathers of neighbouring rows hit the same lines)
         cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
-                             kListRuns ? int(cudaSharedmemCarveoutMaxShared) : int(cudaSharedmemCarveoutMaxL1));
+                             kListRuns ? 60 : int(cudaSharedmemCarveoutMaxL1));   // 60 % of 228 KB = 6 x 22.5 KB
         kernel<<<grid, block, smem, st>>>(a);
         return cudaGetLastError();
     };
