@@ -49,7 +49,9 @@ inline size_t n3_part_records(int n_atoms, int rb) {
     return n3_part_offset(nb, n_pad, rb);
 }
 
-__device__ __forceinline__ double rot1(double v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
+__device__ __forceinline__ double rot1(double v) {   // as a 64-bit integer: two SHFL on the register pair, no repacking
+    return __longlong_as_double(__shfl_sync(0xffffffffu, __double_as_longlong(v), (threadIdx.x + 1) & 31));
+}
 __device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
@@ -88,6 +90,11 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    // The 32 records of a chunk do not change while the warp rotates it: they sit in shared memory (1 KB per warp, in the
+    // space the epilogue's reduction uses afterwards; (x, y) and (z, s') as two 16-byte arrays: conflict-free), and at
+    // step s a lane READS the record of lane + s -- two LDS.128 instead of eight shuffles and the moves that go with
+    // them.  Only the reaction sums travel from lane to lane.
+    double2 *jxy = reinterpret_cast<double2 *>(&red[0][0][0][0]) + warp * 64, *jzs = jxy + 32;
     for (int c = c_begin + warp; c < c_end; c += NW) {
         const int jidx = (c << 5) + lane;
         double xj, yj, zj, sj;
@@ -102,16 +109,20 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         // One rotation step: evaluate the IT rows against the record held (`in`), hand it on with the reaction sums
         // accumulated on it so far (`out`).  Two register sets alternate (A -> B, B -> A): no value is ever moved back
         // into a loop-carried register (10 moves per step when the step updated one set in place).
-        struct JRec { double x, y, z, s, g0, g1, g2; int j; };
-        auto step = [&](auto masked, const JRec &in, JRec &out) {
+        struct JRec { double x, y, z, s, g0, g1, g2; };
+        __syncwarp();                                      // the previous chunk's readers are done
+        jxy[lane] = make_double2(xj, yj); jzs[lane] = make_double2(zj, sj);
+        __syncwarp();
+        const int jbase = c << 5;
+        auto step = [&](auto masked, int s, const JRec &in, JRec &out) {
             const double xj = in.x, yj = in.y, zj = in.z, sj = in.s;
-            const int jidx = in.j;
+            const int jidx = jbase + ((lane + s) & 31);
             double g0 = in.g0, g1 = in.g1, g2 = in.g2;     // reaction sums travelling with the record
-            // the record of the NEXT step is sent first (positions do not change): its shuffle latency hides
-            // behind this step's arithmetic; only the reaction sums have to wait for it
-            out.x = rot1(xj); out.y = rot1(yj); out.z = rot1(zj);
-            if constexpr (FORCE) out.s = rot1(sj);
-            if constexpr (decltype(masked)::value) out.j = rot1(jidx);
+            {   // the record of the NEXT step is fetched first: its latency hides behind this step's arithmetic
+                const int nx = (lane + s + 1) & 31;
+                const double2 pxy = jxy[nx], pzs = jzs[nx];
+                out.x = pxy.x; out.y = pxy.y; out.z = pzs.x; out.s = pzs.y;
+            }
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
                 const double dx = xi[k] - xj, dy = yi[k] - yj, dz = zi[k] - zj;
@@ -154,18 +165,18 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
             if constexpr (FORCE) { out.g1 = rot1(g1); out.g2 = rot1(g2); }
         };
         JRec A, B;
-        A.x = xj; A.y = yj; A.z = zj; A.s = sj; A.g0 = A.g1 = A.g2 = 0.0; A.j = jidx;
+        A.x = xj; A.y = yj; A.z = zj; A.s = sj; A.g0 = A.g1 = A.g2 = 0.0;
         B = A;
         if (diag) {
             for (int s = 0; s < 32; s += 2) {
-                step(std::integral_constant<bool, true>{}, A, B);
-                step(std::integral_constant<bool, true>{}, B, A);
+                step(std::integral_constant<bool, true>{}, s, A, B);
+                step(std::integral_constant<bool, true>{}, s + 1, B, A);
             }
         } else {
 #pragma unroll 2
             for (int s = 0; s < 32; s += 2) {
-                step(std::integral_constant<bool, false>{}, A, B);
-                step(std::integral_constant<bool, false>{}, B, A);
+                step(std::integral_constant<bool, false>{}, s, A, B);
+                step(std::integral_constant<bool, false>{}, s + 1, B, A);
             }
         }
         const double g0 = A.g0, g1 = A.g1, g2 = A.g2;
@@ -177,6 +188,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     }
 
     // ---- rows i: sum over the warps of the CTA in a fixed order ----
+    __syncthreads();                                       // every warp is done with its chunk records (same memory)
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
         red[warp][k][0][lane] = f0[k];
@@ -273,6 +285,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     }
     double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    ulonglong2 *jq = reinterpret_cast<ulonglong2 *>(&red[0][0][0][0]) + warp * 128;   // 4 x 32 x 16 B per warp, aliasing `red`
     auto fetch = [&](int j) -> RecF {
         if (j < N) return a.xfr[j];
         return RecF{-kFarF * float((j & 63) + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -291,16 +304,22 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         // One rotation step: the lane evaluates its IT rows against the two records it holds (`in`) and hands them, with
         // the sums accumulated on them, to the next lane (`out`).  Two register sets alternate (A -> B, B -> A), so no
         // value has to be moved back into a loop-carried register (44 moves per two steps when written in place).
-        struct JRec { f2 xh, yh, zh, xl, yl, zl, s, g0, g1, g2, gf; int ja, jb; };
-        auto step = [&](auto masked, const JRec &in, JRec &out) {
+        struct JRec { f2 xh, yh, zh, xl, yl, zl, s, g0, g1, g2, gf; };
+        // the 2 x 32 records of the chunk sit in shared memory (see the FP64 kernel): at step s a lane reads the pair of
+        // records of lane + s with four LDS.128 instead of fourteen shuffles; only the sums travel
+        __syncwarp();
+        jq[lane] = make_ulonglong2(nxh, nyh); jq[32 + lane] = make_ulonglong2(nzh, sj);
+        jq[64 + lane] = make_ulonglong2(nxl, nyl); jq[96 + lane] = make_ulonglong2(nzl, 0ull);
+        __syncwarp();
+        auto step = [&](auto masked, int s, const JRec &in, JRec &out) {
             const f2 nxh = in.xh, nyh = in.yh, nzh = in.zh, nxl = in.xl, nyl = in.yl, nzl = in.zl, sj = in.s;
-            const int jidx_a = in.ja, jidx_b = in.jb;
+            const int jidx_a = ja - lane + ((lane + s) & 31), jidx_b = jidx_a + 32;
             f2 g0 = in.g0, g1 = in.g1, g2 = in.g2, gfar = in.gf;
-            // the records do not change: send them on first, their shuffle latency hides behind the arithmetic
-            out.xh = rot1_f2(nxh); out.yh = rot1_f2(nyh); out.zh = rot1_f2(nzh);
-            out.xl = rot1_f2(nxl); out.yl = rot1_f2(nyl); out.zl = rot1_f2(nzl);
-            if constexpr (FORCE) out.s = rot1_f2(sj);
-            if constexpr (decltype(masked)::value) { out.ja = rot1(jidx_a); out.jb = rot1(jidx_b); }
+            {   // the records of the NEXT step first: their latency hides behind this step's arithmetic
+                const int nx = (lane + s + 1) & 31;
+                const ulonglong2 q0 = jq[nx], q1 = jq[32 + nx], q2 = jq[64 + nx], q3 = jq[96 + nx];
+                out.xh = q0.x; out.yh = q0.y; out.zh = q1.x; out.s = q1.y; out.xl = q2.x; out.yl = q2.y; out.zl = q3.x;
+            }
             f2 estep = zero2;                              // sum r^-n over the 2 IT pairs of this step
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
@@ -366,17 +385,17 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         };
         JRec A, B;
         A.xh = nxh; A.yh = nyh; A.zh = nzh; A.xl = nxl; A.yl = nyl; A.zl = nzl; A.s = sj;
-        A.g0 = A.g1 = A.g2 = A.gf = zero2; A.ja = ja; A.jb = jb;
+        A.g0 = A.g1 = A.g2 = A.gf = zero2;
         B = A;
         if (diag) {
             for (int s = 0; s < 32; s += 2) {
-                step(std::integral_constant<bool, true>{}, A, B);
-                step(std::integral_constant<bool, true>{}, B, A);
+                step(std::integral_constant<bool, true>{}, s, A, B);
+                step(std::integral_constant<bool, true>{}, s + 1, B, A);
             }
         } else {
             for (int s = 0; s < 32; s += 2) {
-                step(std::integral_constant<bool, false>{}, A, B);
-                step(std::integral_constant<bool, false>{}, B, A);
+                step(std::integral_constant<bool, false>{}, s, A, B);
+                step(std::integral_constant<bool, false>{}, s + 1, B, A);
             }
         }
         const f2 g0 = A.g0, g1 = A.g1, g2 = A.g2, gfar = A.gf;             // both records are home again
@@ -399,6 +418,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
             }
         }
     }
+    __syncthreads();                                       // every warp is done with its chunk records (same memory)
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
         red[warp][k][0][lane] = F0[k];
