@@ -123,8 +123,8 @@ __device__ __forceinline__ double warp0_sum_partials(const double *part, int n) 
 __device__ __forceinline__ void grid_barrier(unsigned long long *counter, unsigned long long target) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(counter, 1ull);
+        // release: the CTA's writes (ordered before this by the bar.sync above) are visible to whoever acquires the count
+        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(counter) : "memory");
         unsigned long long seen;
         do {
             asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(counter) : "memory");
