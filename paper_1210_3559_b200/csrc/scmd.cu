@@ -441,9 +441,20 @@ int choose_n3_segment(const sc_ctx *c, int *warps_out) {
     double best_t = 0.0;
     for (int nw : {kN3Warps, kN3Warps / 2}) {
         if (nw != ((c->opt_warps && c->opt_warps <= 6) ? 6 : 12)) continue;    // SC_OPT_WARPS_PER_CTA <= 6 forces 6
+        // candidates: every segment length that is a whole number of rounds of the CTA's warps and gives <= 25 segments
+        // (round 1 tried only 8 / 12 / 16 / 20 / 24 segments; for a mid-size cluster ONE tile per SM -- 3 or 4 long
+        // segments -- beats two short rounds: bench steps N = 6144 0.127 -> 0.108 ms, 8000 0.165 -> 0.161, 16384 0.425 -> 0.408,
+        // mixed 8000 0.140 -> 0.133).  Beyond 16384 atoms (mixed: 8192) the fine set measured 2 - 3 % WORSE than the coarse one
+        // (the cost model is not that good), and above 49152 the choice is flat within 1 %.
+        std::vector<int> cands;
+        if (N > (c->precision == SC_PREC_MIXED ? 8192 : 16384)) {
+            for (int want : {8, 12, 16, 20, 24}) cands.push_back(round_up(ceil_div(nch, want), nw * unit));
+        } else {
+            for (int seg = nw * unit; seg < nch + nw * unit; seg += nw * unit) cands.push_back(seg);
+        }
         int last_seg = 0;
-        for (int want : {8, 12, 16, 20, 24}) {
-            const int seg = round_up(ceil_div(nch, want), nw * unit), nseg = ceil_div(nch, seg);
+        for (int seg : cands) {
+            const int nseg = ceil_div(nch, seg);
             if (nseg > kN3MaxSegments || seg == last_seg) continue;
             last_seg = seg;
             std::priority_queue<double, std::vector<double>, std::greater<double>> sm;
