@@ -458,6 +458,12 @@ struct N3FinalArgs {
     double *rho, *force, *partial;      // partial: [gridDim.x = ceil(N / 32)] sum sqrt(rho) (density)
     int n_atoms, n_pad, rb, seg_chunks;
     PairConsts c;
+    // NVE steps inside sc_step (FORCE only): the thread that has just formed F_i also does the velocity-Verlet updates
+    // that follow, instead of two more launches.  fuse = 0: nothing; 1: second half kick of this step and the per-CTA
+    // sum of |v|^2 (the call's last step); 2: second half kick, then the first half kick and the drift of the NEXT step
+    int fuse;
+    double *vel, *part_ke;              // [N*3]; [gridDim.x]
+    double hk, dt;                      // dt/2 ACC/m; dt
 };
 
 constexpr int kN3FinAtoms = 32;         // atoms per CTA of the finalize kernel: one per lane
@@ -505,6 +511,22 @@ __global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3F
     if (i < a.n_atoms) {
         if constexpr (FORCE) {
             a.force[3 * size_t(i)] = v0; a.force[3 * size_t(i) + 1] = v1; a.force[3 * size_t(i) + 2] = v2;
+            if (a.fuse) {
+                // the same fused multiply-adds, in the same order, as kick_ke_kernel and kick_drift_kernel
+                double vx = fma(a.hk, v0, a.vel[3 * size_t(i)]), vy = fma(a.hk, v1, a.vel[3 * size_t(i) + 1]),
+                       vz = fma(a.hk, v2, a.vel[3 * size_t(i) + 2]);
+                if (a.fuse == 1) {
+                    contrib = fma(vz, vz, fma(vy, vy, vx * vx));
+                } else {
+                    vx = fma(a.hk, v0, vx); vy = fma(a.hk, v1, vy); vz = fma(a.hk, v2, vz);
+                    double4 p = a.xs[i];
+                    p.x = fma(a.dt, vx, p.x); p.y = fma(a.dt, vy, p.y); p.z = fma(a.dt, vz, p.z);
+                    a.xs[i] = p;
+                    if (a.xf) store_split_record(a.xf, i, p.x, p.y, p.z, float(p.w));
+                    if (a.xfr) a.xfr[i] = split_record(p);
+                }
+                a.vel[3 * size_t(i)] = vx; a.vel[3 * size_t(i) + 1] = vy; a.vel[3 * size_t(i) + 2] = vz;
+            }
         } else {
             const double rho = a.c.am * v0;
             if (a.rho) a.rho[i] = rho;
@@ -519,6 +541,11 @@ __global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3F
     if constexpr (!FORCE) {
         const double t = warp_sum(contrib);
         if (lane == 0) a.partial[blockIdx.x] = t;
+    } else {
+        if (a.fuse == 1) {
+            const double t = warp_sum(contrib);
+            if (lane == 0) a.part_ke[blockIdx.x] = t;
+        }
     }
 }
 #endif  // SCMD_MAIN_TU
