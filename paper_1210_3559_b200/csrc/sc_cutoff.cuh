@@ -160,12 +160,22 @@ __global__ void __launch_bounds__(256) rebuild_kernel(const RebuildArgs a) {
 
     // ---- P1: CTA 0 builds the cell grid ----
     if (blockIdx.x == 0) {
-        if (tid < 9) {
-            double v = a.blockpart[tid];
-            for (int b = 1; b < int(gridDim.x); ++b) {
-                const double o = a.blockpart[9 * b + tid];
-                v = tid < 3 ? v + o : (tid < 6 ? fmin(v, o) : fmax(v, o));
+        // the 9 quantities over all CTAs' partials: 28 threads per quantity stride the CTAs, then one thread per quantity
+        // combines the 28 in a fixed order (one thread walking all CTAs took 91 us of a 330 us build at N = 65536)
+        __shared__ double comb[9][28];
+        if (tid < 9 * 28) {
+            const int q = tid / 28, r = tid % 28;
+            double v = q < 3 ? 0.0 : (q < 6 ? 1e300 : -1e300);
+            for (int b = r; b < int(gridDim.x); b += 28) {
+                const double o = a.blockpart[9 * b + q];
+                v = q < 3 ? v + o : (q < 6 ? fmin(v, o) : fmax(v, o));
             }
+            comb[q][r] = v;
+        }
+        __syncthreads();
+        if (tid < 9) {
+            double v = comb[tid][0];
+            for (int r = 1; r < 28; ++r) v = tid < 3 ? v + comb[tid][r] : (tid < 6 ? fmin(v, comb[tid][r]) : fmax(v, comb[tid][r]));
             sh[tid][0] = v;
         }
         __syncthreads();
