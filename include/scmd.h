@@ -123,13 +123,19 @@ typedef enum {
                                      both atoms.  0: library default (on from N = 4097, mixed
                                      precision 4609), 1: on,
                                      2: off = the one-sided sweeps                               */
-    SC_OPT_CUTOFF_SHIFT = 11      /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
+    SC_OPT_CUTOFF_SHIFT = 11,     /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
                                      configs; 1 energy-shifted terms: inside r_cut every pair term
                                      loses its value at the cutoff, (a/r)^k -> (a/r)^k - (a/r_cut)^k
                                      for k = n in Eq. (1) and k = m in Eq. (2), so U is continuous
                                      when a pair crosses r_cut and NVE runs keep their energy; the
                                      force keeps its form, with rho_i the shifted density (DESIGN.md
                                      Q21).  Ignored without a cutoff.                            */
+    SC_OPT_NEWTON3_PIECES = 12    /* Newton's-third-law sweeps: how the triangle of unordered pairs is
+                                     handed to the CTAs.  0 (default): cut into pieces of equal cost,
+                                     one CTA each, one piece per SM;
+                                     1..16: that many pieces per SM; -1: a (row block x j segment)
+                                     grid with one segment length for all row blocks (rounds 1-2a).
+                                     Results are bit-reproducible for a given value, device and N  */
 } sc_option;
 
 /* Read-only queries (sc_get_option), beside the sc_option values themselves. */

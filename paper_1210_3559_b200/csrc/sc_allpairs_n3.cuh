@@ -28,16 +28,23 @@ constexpr int kN3Warps = 12;          // warps per SM the register allocation al
 constexpr double kN3Far = 1.0e100;
 constexpr float kN3FarTerm = 1.4901161193847656e-08f;   // 2^-26: r^-6 of a pair 20 A apart (mixed sweep 1: near / far sums)
 
+// A tile: chunks [c_begin, c_end) of row block b's part of the triangle (chunks of 32 atoms, the packed mixed kernel: of
+// 64), whose row sums go to self[slot].  The host cuts the triangle -- row block after row block, ~N^2 / 8192 chunks --
+// into one PIECE per CTA of equal cost, a piece being a few consecutive tiles (a long row block is cut into several
+// tiles, each with its own slot; a piece at the narrow end of the triangle holds several short row blocks).  Round 1 and
+// early round 2 launched a (row block, j segment) grid with ONE segment length for all row blocks: at N = 8000 that is 140
+// CTAs of 2 ... 6 rounds of the 12 warps each, and the sweep lasted as long as the 6-round ones.
+struct N3Tile { int b, c_begin, c_end, slot; };
+
 struct N3Args {
     const double4 *xs;      // [N] (x, y, z, s')
     int n_atoms, n_pad;     // n_pad = round_up(N, 32)
     double4 *part;          // triangular: block b at offset n3_part_offset(b), n_pad - b * RB records (FORCE) ...
     double *part_rho;       // ... or doubles (density sweep); the same memory
     double4 *self;          // [gridDim.y][n_pad] row sums per j segment (x, y, z) / (rho, -, -)
-    double *partial;        // [gridDim.y * gridDim.x] per-CTA sum r^-n over ORDERED pairs (FORCE && ENERGY)
-    int seg_chunks;         // chunks of 32 atoms per j segment: CTA (b, s) takes chunks cb(b) + s L .. + L of block b's
-                            //   triangle, so that all CTAs carry about the same work (a triangle cut by rows only leaves
-                            //   the SMs idle at the end: measured 6 % at N = 65536, 20 % at N = 32768)
+    double *partial;        // [gridDim.x] per-CTA sum r^-n over ORDERED pairs (FORCE && ENERGY)
+    const N3Tile *tiles;    // the plan (scmd.cu, plan_n3): CTA p works through tiles[piece_start[p] .. piece_start[p + 1])
+    const int *piece_start;
     PairConsts c;
 };
 
@@ -62,18 +69,17 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;                          // 12, or 6 (two CTAs per SM: finer tiles for mid-size clusters)
     const int N = a.n_atoms;
-    const int row0 = blockIdx.x * RB;
-    if ((row0 >> 5) + int(blockIdx.y) * a.seg_chunks >= ((a.n_atoms + 31) >> 5)) {   // no such segment in this block's triangle
-        if (FORCE && ENERGY && threadIdx.x == 0) a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 0.0;
-        return;
-    }
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
+    double esum = 0.0;
+    const int t_end = a.piece_start[blockIdx.x + 1];
+    for (int t = a.piece_start[blockIdx.x]; t < t_end; ++t) {
+    const N3Tile tile = a.tiles[t];
+    const int row0 = tile.b * RB;
 
     int irow[IT];
     double xi[IT], yi[IT], zi[IT], si[IT];
     double f0[IT], f1[IT], f2[IT];
-    double esum = 0.0;
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
         irow[k] = row0 + k * 32 + lane;
@@ -86,10 +92,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         f0[k] = f1[k] = f2[k] = 0.0;
     }
 
-    const int cb = row0 >> 5, nch = (N + 31) >> 5;
-    const int c_begin = cb + int(blockIdx.y) * a.seg_chunks, c_end = min(nch, c_begin + a.seg_chunks);
-    double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
-    double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    const int cb = row0 >> 5;
+    const int c_begin = tile.c_begin, c_end = tile.c_end;
+    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
+    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, RB);
     // The 32 records of a chunk do not change while the warp rotates it: they sit in shared memory (1 KB per warp, in the
     // space the epilogue's reduction uses afterwards; (x, y) and (z, s') as two 16-byte arrays: conflict-free), and at
     // step s a lane READS the record of lane + s -- two LDS.128 instead of eight shuffles and the moves that go with
@@ -194,10 +200,6 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         red[warp][k][0][lane] = f0[k];
         if constexpr (FORCE) { red[warp][k][1][lane] = f1[k]; red[warp][k][2][lane] = f2[k]; }
     }
-    if constexpr (FORCE && ENERGY) {
-        esum = warp_sum(esum);
-        if (lane == 0) red_e[warp] = esum;
-    }
     __syncthreads();
     for (int r = threadIdx.x; r < RB; r += NW * 32) {
         const int k = r >> 5, l = r & 31, i = row0 + r;
@@ -206,13 +208,18 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
-        if (i < N) a.self[size_t(blockIdx.y) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
+        if (i < N) a.self[size_t(tile.slot) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
     }
+    __syncthreads();                                       // the next tile's chunk records go into the same memory
+    }   // tiles of this CTA's piece
     if constexpr (FORCE && ENERGY) {
+        esum = warp_sum(esum);                             // over all tiles of the piece
+        if (lane == 0) red_e[warp] = esum;
+        __syncthreads();
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < NW; ++w) tot += red_e[w];
-            a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;   // every unordered pair stands for two ordered ones
+            a.partial[blockIdx.x] = 2.0 * tot;   // every unordered pair stands for two ordered ones
         }
     }
 }
@@ -235,7 +242,8 @@ struct N3FArgs {
     double *part_rho;
     double4 *self;
     double *partial;
-    int seg_chunks;
+    const N3Tile *tiles;    // chunks counted in units of 64 atoms here
+    const int *piece_start;
     PairConsts c;
 };
 
@@ -255,24 +263,21 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
     const int N = a.n_atoms;
-    const int row0 = blockIdx.x * RB;
-    // a.seg_chunks counts chunks of 32 atoms and is even here: segments of seg_chunks / 2 chunks of 64
-    const int seg64 = a.seg_chunks >> 1;
-    const int cb = row0 >> 6, nch = (N + 63) >> 6;
-    const int c_begin = cb + int(blockIdx.y) * seg64, c_end = min(nch, c_begin + seg64);
-    if (c_begin >= nch) {
-        if (FORCE && ENERGY && threadIdx.x == 0) a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 0.0;
-        return;
-    }
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const f2 An2 = f2_dup(float(a.c.An));
     const f2 zero2 = f2_dup(0.f), one2 = f2_dup(1.0f), mone2 = f2_dup(-1.0f), mhalf2 = f2_dup(-0.5f);
     constexpr float kFarF = 1.0e15f;
+    double esum = 0.0;
+    const int t_end = a.piece_start[blockIdx.x + 1];
+    for (int t = a.piece_start[blockIdx.x]; t < t_end; ++t) {
+    const N3Tile tile = a.tiles[t];
+    const int row0 = tile.b * RB;
+    const int cb = row0 >> 6;
+    const int c_begin = tile.c_begin, c_end = tile.c_end;   // chunks of 64 atoms
 
     int irow[IT];
     f2 xh[IT], yh[IT], zh[IT], xl[IT], yl[IT], zl[IT], si[IT];     // row values in both halves
     double F0[IT], F1[IT], F2[IT];
-    double esum = 0.0;
 #pragma unroll
     for (int k = 0; k < IT; ++k) {
         irow[k] = row0 + k * 32 + lane;
@@ -283,8 +288,8 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         xl[k] = f2_dup(p.xl); yl[k] = f2_dup(p.yl); zl[k] = f2_dup(p.zl); si[k] = f2_dup(p.s);
         F0[k] = F1[k] = F2[k] = 0.0;
     }
-    double4 *part = a.part + n3_part_offset(blockIdx.x, a.n_pad, RB);
-    double *part_rho = a.part_rho + n3_part_offset(blockIdx.x, a.n_pad, RB);
+    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
+    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, RB);
     ulonglong2 *jq = reinterpret_cast<ulonglong2 *>(&red[0][0][0][0]) + warp * 128;   // 4 x 32 x 16 B per warp, aliasing `red`
     auto fetch = [&](int j) -> RecF {
         if (j < N) return a.xfr[j];
@@ -424,10 +429,6 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         red[warp][k][0][lane] = F0[k];
         if constexpr (FORCE) { red[warp][k][1][lane] = F1[k]; red[warp][k][2][lane] = F2[k]; }
     }
-    if constexpr (FORCE && ENERGY) {
-        esum = warp_sum(esum);
-        if (lane == 0) red_e[warp] = esum;
-    }
     __syncthreads();
     for (int r = threadIdx.x; r < RB; r += NW * 32) {
         const int k = r >> 5, l = r & 31, i = row0 + r;
@@ -436,13 +437,18 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
-        if (i < N) a.self[size_t(blockIdx.y) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
+        if (i < N) a.self[size_t(tile.slot) * a.n_pad + i] = make_double4(v0, v1, v2, 0.0);
     }
+    __syncthreads();                                       // the next tile's chunk records go into the same memory
+    }   // tiles of this CTA's piece
     if constexpr (FORCE && ENERGY) {
+        esum = warp_sum(esum);                             // over all tiles of the piece
+        if (lane == 0) red_e[warp] = esum;
+        __syncthreads();
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < NW; ++w) tot += red_e[w];
-            a.partial[blockIdx.y * gridDim.x + blockIdx.x] = 2.0 * tot;
+            a.partial[blockIdx.x] = 2.0 * tot;
         }
     }
 }
@@ -456,7 +462,8 @@ struct N3FinalArgs {
     const double *part_rho;
     const double4 *self;
     double *rho, *force, *partial;      // partial: [gridDim.x = ceil(N / 32)] sum sqrt(rho) (density)
-    int n_atoms, n_pad, rb, seg_chunks;
+    int n_atoms, n_pad, rb;
+    const int *blk_slots;               // [row blocks] tiles (= self slots) of each row block in the plan
     PairConsts c;
     // NVE steps inside sc_step (FORCE only): the thread that has just formed F_i also does the velocity-Verlet updates
     // that follow, instead of two more launches.  fuse = 0: nothing; 1: second half kick of this step and the per-CTA
@@ -481,7 +488,7 @@ __global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3F
     double v0 = 0.0, v1 = 0.0, v2 = 0.0;
     if (i < a.n_atoms) {
         const int bi = i / a.rb;
-        const int nseg = (((a.n_atoms + 31) >> 5) - ((bi * a.rb) >> 5) + a.seg_chunks - 1) / a.seg_chunks;
+        const int nseg = a.blk_slots[bi];
         for (int sg = w; sg < nseg; sg += kN3FinWarps) {    // row sums of the segments of i's own block
             const double4 s = a.self[size_t(sg) * a.n_pad + i];
             v0 += s.x; v1 += s.y; v2 += s.z;

@@ -65,6 +65,8 @@ struct sc_ctx {
     double *msd_meta = nullptr;   // [kMsdMeta] centroids, rotation, totals
     double4 *n3_part = nullptr;   // Newton's-third-law sweeps: triangular reaction partials, row sums (else NULL)
     double4 *n3_self = nullptr;
+    N3Tile *n3_tiles = nullptr;   // ... and their plan (plan_n3): tiles, first tile of each CTA's piece, slots per row block
+    int *n3_piece_start = nullptr, *n3_blk_slots = nullptr;
     double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
     unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
     unsigned long long small_barrier_count = 0;
@@ -108,7 +110,8 @@ struct sc_ctx {
     // options (0 = default)
     int opt_it = 0, opt_tpr = 0, opt_warps = 0, opt_persistent = 0, opt_energy_every = 0, opt_kmax = 0, opt_fine = 0, opt_apc = 0, opt_n3 = 0, opt_shift = 0;
     int emb_pending = 0;          // sweep 1 left this many per-CTA sums of sqrt(rho) in part_a, not yet totalled into U_emb
-    int n3_seg = 0;               // j-segment length of the Newton's-third-law sweeps (chunks of 32), chosen at first use
+    int n3_seg = 0;               // Newton's-third-law sweeps: CTAs (= pieces) of the plan on the device; 0 = no plan yet
+    int opt_n3_pieces = 0;
     int n3_warps = 12;            // ... and their warps per CTA (12, or 6 with two CTAs per SM)
     int n3_fuse = 0;              // do_step -> run_sweep_n3: what the force finalize kernel integrates (N3FinalArgs::fuse)
     double n3_hk = 0.0, n3_dt = 0.0;
@@ -173,7 +176,11 @@ int cutoff_max_dim(int64_t N) {
 constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
 constexpr int64_t kN3DefaultMinAtoms = 4097, kN3DefaultMinAtomsMixed = 4609;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
-constexpr int kN3MaxSegments = 25;                             // j segments of the longest row block
+constexpr int kN3MaxSegments = 25;                             // j segments (tiles) of the longest row block
+constexpr int kN3MaxPieces = 4096;                             // CTAs of a balanced plan (16 per SM on 256 SMs)
+inline size_t n3_tile_capacity(int64_t N) {                    // the round-1 grid has up to 25 tiles per row block
+    return size_t(ceil_div(N, int64_t(32 * kN3RowsPerThread))) * kN3MaxSegments + kN3MaxPieces;
+}
 
 // one place that lays the workspace out; base == nullptr only measures
 size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t precision, double skin,
@@ -210,7 +217,10 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
         double4 *ns = w.take<double4>((n + 32) * kN3MaxSegments);
         RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
-        if (c && base) { c->n3_part = np; c->n3_self = ns; if (xr) c->xfr = xr; }
+        N3Tile *tl = w.take<N3Tile>(n3_tile_capacity(N));
+        int *ps = w.take<int>(n3_tile_capacity(N) + 1);
+        int *bs = w.take<int>(size_t(ceil_div(N, int64_t(32 * kN3RowsPerThread))));
+        if (c && base) { c->n3_part = np; c->n3_self = ns; c->n3_tiles = tl; c->n3_piece_start = ps; c->n3_blk_slots = bs; if (xr) c->xfr = xr; }
     }
     if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
         FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
@@ -422,6 +432,7 @@ sc_status check_flags(sc_ctx *c) {
     return SC_OK;
 }
 
+// GRID PLAN ONLY (SC_OPT_NEWTON3_PIECES = -1; the default is the balanced plan of plan_n3 below).
 // Segment length of the Newton's-third-law sweeps, in chunks of 32 atoms.  Their CTAs (row block x j segment; one CTA
 // per SM at 168 registers x 384 threads) are handed to the SMs in launch order as SMs fall free, so the sweep lasts as
 // long as the busiest SM of that greedy schedule: with a few hundred CTAs on 148 SMs a badly filled last wave costs
@@ -480,6 +491,107 @@ int choose_n3_segment(const sc_ctx *c, int *warps_out) {
     return best_seg;
 }
 
+// The plan of the Newton's-third-law sweeps: which CTA works through which tiles (sc_allpairs_n3.cuh, N3Tile).
+//
+// Balanced plan (the default).  The triangle, row block after row block, is cut into P = SMs x k pieces of equal COST,
+// one CTA each; k = 1 (one wave of resident CTAs: nothing is left to the order in which SMs fall free; measured against
+// k = 2 / 4 / 8 per SM, SC_OPT_NEWTON3_PIECES: N = 8000 103.7 / 110.1 us per step, N = 65536 5158 / 5157 / 5161 / 5180).
+// Cost of a tile of L chunks: ceil(L / 4) -- the CTA's 12 warps take the
+// chunks round-robin, warps w, w + 4, w + 8 share one SM sub-partition and its issue slot, so the tile lasts as long as
+// the ceil(L / 4) chunks of its busiest sub-partition -- plus a fixed 0.15 for the tile's row loads and its reduction
+// (two CTA barriers).  The smallest cost bound T for which the greedy cut (fill a piece up to T, never with a sliver
+// shorter than 4 chunks unless it ends the row block) needs <= P pieces is found by bisection.  N = 8000: 7938 chunks
+// on 148 SMs = 13.4 per sub-partition, the plan gives every CTA <= 14; the round-1 grid gave the longest 18 (6 rounds x
+// 3 warps) and the sweep lasted 78 us where 14 / 18 of that is 61 -- measured 61.2 (300-step calls, us per step, grid
+// plan -> balanced: N = 6144 73.7 -> 71.8, N = 8000 123.3 -> 103.7, mixed 99.0 -> 86.1, N = 16384 360.5 -> 346.9,
+// N = 65536 5251 -> 5158, mixed 3981 -> 3909).
+//
+// Grid plan (SC_OPT_NEWTON3_PIECES = -1; rounds 1 - 2a, kept for comparison): one tile per CTA, row block x j segment
+// with ONE segment length for all row blocks (choose_n3_segment), CTAs in launch order.
+struct N3Plan {
+    std::vector<N3Tile> tiles;
+    std::vector<int> piece_start, blk_slots;
+};
+
+// greedy cut for the cost bound T; false if it needs more than max_pieces pieces or a row block more than 25 tiles
+bool n3_cut(int nb, int nch, int cpb, double T, double fixed, int max_pieces, N3Plan *out) {
+    out->tiles.clear(); out->piece_start.assign(1, 0); out->blk_slots.assign(size_t(nb), 0);
+    double cur = 0.0;
+    auto close = [&]() {
+        if (int(out->tiles.size()) > out->piece_start.back()) out->piece_start.push_back(int(out->tiles.size()));
+        cur = 0.0;
+    };
+    for (int b = 0; b < nb; ++b) {
+        int cpos = b * cpb, slot = 0;
+        while (cpos < nch) {
+            const int rest = nch - cpos;
+            const double room = T - cur - fixed;
+            int fit = room >= 1.0 ? 4 * int(room + 1e-9) : 0;
+            if (fit < rest && fit < 4) fit = 0;
+            if (fit <= 0) {
+                if (cur == 0.0) return false;                  // T below one tile's cost
+                close();
+                continue;
+            }
+            const int len = std::min(fit, rest);
+            if (slot >= kN3MaxSegments) return false;
+            out->tiles.push_back(N3Tile{b, cpos, cpos + len, slot++});
+            cur += fixed + double(ceil_div(len, 4));
+            cpos += len;
+        }
+        out->blk_slots[size_t(b)] = slot;
+    }
+    close();
+    return int(out->piece_start.size()) - 1 <= max_pieces;
+}
+
+int choose_n3_segment(const sc_ctx *c, int *warps_out);
+
+sc_status plan_n3(sc_ctx *c) {
+    const int N = int(c->N), rb = 32 * kN3RowsPerThread, nb = ceil_div(N, rb);
+    const bool mixed = c->precision == SC_PREC_MIXED;
+    const int chunk = mixed ? 64 : 32, nch = ceil_div(N, chunk), cpb = rb / chunk;
+    N3Plan plan;
+    c->n3_warps = (c->opt_warps && c->opt_warps <= 6) ? 6 : kN3Warps;
+    if (c->opt_n3_pieces < 0) {
+        int warps = kN3Warps;
+        const int seg32 = choose_n3_segment(c, &warps), seg = seg32 * 32 / chunk, nseg = ceil_div(ceil_div(N, 32), seg32);
+        c->n3_warps = warps;
+        plan.piece_start.assign(1, 0); plan.blk_slots.assign(size_t(nb), 0);
+        for (int y = 0; y < nseg; ++y)
+            for (int b = 0; b < nb; ++b) {
+                const int c_begin = b * cpb + y * seg;
+                if (c_begin >= nch) continue;
+                plan.tiles.push_back(N3Tile{b, c_begin, std::min(nch, c_begin + seg), y});
+                plan.piece_start.push_back(int(plan.tiles.size()));
+                plan.blk_slots[size_t(b)] = y + 1;
+            }
+    } else {
+        const int per_sm = c->opt_n3_pieces ? c->opt_n3_pieces : 1;
+        const int P = std::min(std::min(kN3MaxPieces, N / 2), c->sm_count * (kN3Warps / c->n3_warps) * per_sm);   // part_b holds N + 1
+        const double fixed = 0.15;
+        double total = 0.0;
+        for (int b = 0; b < nb; ++b) total += fixed + double(ceil_div(nch - b * cpb, 4));
+        double lo = 1.0, hi = total + 2.0;                          // hi: everything in one piece, always feasible
+        N3Plan trial;
+        for (int it = 0; it < 48; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (n3_cut(nb, nch, cpb, mid, fixed, P, &trial)) hi = mid; else lo = mid;
+        }
+        if (!n3_cut(nb, nch, cpb, hi, fixed, P, &plan))
+            return fail(c, SC_ERR_INVALID, "Newton's-third-law sweeps: no plan for this size%s");
+    }
+    const int pieces = int(plan.piece_start.size()) - 1;
+    if (plan.tiles.size() > n3_tile_capacity(c->N) || pieces < 1)
+        return fail(c, SC_ERR_INVALID, "Newton's-third-law sweeps: plan exceeds the workspace carved for it%s");
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->n3_tiles, plan.tiles.data(), plan.tiles.size() * sizeof(N3Tile), cudaMemcpyHostToDevice, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->n3_piece_start, plan.piece_start.data(), plan.piece_start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    SC_CUDA_CHECK(c, cudaMemcpyAsync(c->n3_blk_slots, plan.blk_slots.data(), plan.blk_slots.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    SC_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));           // the vectors die with this call
+    c->n3_seg = pieces;
+    return SC_OK;
+}
+
 // all pairs, every unordered pair once (sc_allpairs_n3.cuh): sweep + finalize + scalar reduction
 sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
@@ -495,19 +607,21 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     a.partial = c->part_b; a.c = c->consts;
     N3FArgs af{};
     af.xfr = c->xfr; af.n_atoms = N; af.n_pad = a.n_pad; af.part = a.part; af.part_rho = a.part_rho; af.self = a.self;
-    // j segments cut the first row block's triangle; each a multiple of the 12 warps (choose_n3_segment)
-    if (!c->n3_seg) c->n3_seg = choose_n3_segment(c, &c->n3_warps);
-    const int nch = ceil_div(N, 32), seg = c->n3_seg, nseg = ceil_div(nch, seg);
-    a.seg_chunks = seg;
-    af.partial = a.partial; af.c = a.c; af.seg_chunks = seg;
+    if (!c->n3_seg) {
+        sc_status st = plan_n3(c);
+        if (st != SC_OK) return st;
+    }
+    const int pieces = c->n3_seg;
+    a.tiles = c->n3_tiles; a.piece_start = c->n3_piece_start;
+    af.partial = a.partial; af.c = a.c; af.tiles = a.tiles; af.piece_start = a.piece_start;
     void *params[1] = {mixed ? static_cast<void *>(&af) : static_cast<void *>(&a)};
     if (c->n3_warps < kN3Warps)       // two CTAs of 6 warps per SM need 2 x 37 KB of shared memory
         cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, int(cudaSharedmemCarveoutMaxShared));
-    cudaError_t e = cudaLaunchKernel(fn, dim3(nb, nseg), dim3(c->n3_warps * 32), params, 0, c->stream);
+    cudaError_t e = cudaLaunchKernel(fn, dim3(pieces), dim3(c->n3_warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law sweep launch: %s", cudaGetErrorString(e));
     N3FinalArgs f{};
     f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.part_rho; f.self = c->n3_self; f.rho = c->rho; f.force = c->force;
-    f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.seg_chunks = seg; f.c = c->consts;
+    f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.n_pad; f.rb = rb; f.blk_slots = c->n3_blk_slots; f.c = c->consts;
     f.fuse = force ? c->n3_fuse : 0; f.vel = c->vel; f.part_ke = c->stage_a; f.hk = c->n3_hk; f.dt = c->n3_dt;
     if (f.fuse && !mixed) { f.xf = nullptr; f.xfr = nullptr; }
     if (f.fuse && mixed) { f.xf = c->xf; f.xfr = c->xfr; }
@@ -518,7 +632,7 @@ sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     if (!force) {
         c->emb_pending = fb;
     } else if (energy) {
-        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, nb * nseg, c->scal, kSlotEPair, c->consts.En);
+        reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, pieces, c->scal, kSlotEPair, c->consts.En);
         c->launches += 1;
     }
     SC_CUDA_CHECK(c, cudaGetLastError());
@@ -946,6 +1060,11 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
         case SC_OPT_ATOMS_PER_CTA:
             if (value < 0 || value > 4096) return fail(c, SC_ERR_INVALID, "atoms per CTA must be 0..4096%s");
             c->opt_apc = int(value); break;
+        case SC_OPT_NEWTON3_PIECES:
+            if (value < -1 || value > 16) return fail(c, SC_ERR_INVALID, "Newton's-third-law pieces per SM must be -1..16%s");
+            c->opt_n3_pieces = int(value); c->n3_seg = 0;
+            c->density_valid = c->forces_valid = c->energy_valid = false;
+            break;
         default:
             return fail(c, SC_ERR_INVALID, "unknown option%s");
     }
@@ -967,6 +1086,7 @@ sc_status sc_get_option(sc_ctx *c, int32_t option, int64_t *value) {
         case SC_OPT_ATOMS_PER_CTA: *value = c->opt_apc; break;
         case SC_OPT_NEWTON3: *value = c->opt_n3; break;
         case SC_OPT_CUTOFF_SHIFT: *value = c->opt_shift; break;
+        case SC_OPT_NEWTON3_PIECES: *value = c->opt_n3_pieces; break;
         case SC_INFO_STEP_PATH:
             *value = c->cutoff ? 3 : (small_path_wanted(c) ? 2 : (n3_wanted(c) ? 1 : 0));
             break;

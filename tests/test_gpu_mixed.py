@@ -95,7 +95,7 @@ def test_generic_exponents_mixed(scmd, oracle_ld, n, m):
 
 
 @pytest.mark.parametrize("n_atoms,kw", [(8192, {}), (9001, {}), (8333, dict(n=12, m=6, eps=0.02, c=30.0, a=3.3)),
-                                        (13400, {}),             # 13400: the segment chooser takes 18 j segments
+                                        (13400, {}),
                                         (2048, {}), (4609, {}), (5003, {})])   # smallest carved size, the default's lower end
 def test_newton3_sweeps_mixed(scmd, oracle_ld, n_atoms, kw):
     """The Newton's-third-law sweeps in mixed precision (binary32 rotation on split records, binary64 sums):

@@ -104,6 +104,38 @@ def test_newton3_sweeps(scmd, oracle_ld, n_atoms, kw):
     assert np.array_equal(a[1], a2[1]) and np.array_equal(a[2], a2[2]) and a[3] == a2[3]      # bit-reproducible
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("n_atoms,pieces", [(2048, 16), (2051, 1), (5003, -1), (5003, 3), (5003, 16), (9001, 2),
+                                            (9001, -1), (20011, 1), (20011, 16)])
+def test_newton3_plans(scmd, oracle_ld, n_atoms, pieces, precision):
+    """SC_OPT_NEWTON3_PIECES: the triangle cut into pieces of equal cost (k per SM; several tiles per CTA at the narrow
+    end, several CTAs per row block at the wide end, slivers, one-chunk tiles) and the (row block x j segment) grid of
+    round 1, both precisions at BASELINE.json's tolerances; invalid values are refused."""
+    import torch
+    w = W.fcc_cluster(n_atoms, 1500.0, seed=85)
+    P = oracle_ld.params()
+    rho_o, f_o, (e_o, _, _) = oracle_ld.energy_forces(w.pos, P)
+    sc = scmd.SuttonChen(n_atoms, precision=precision)
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3, 1)
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3_PIECES, pieces)
+    assert sc.sc_get_option(scmd.SC_OPT_NEWTON3_PIECES) == pieces
+    assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == (2 if n_atoms <= 2304 else 1)  # sc_step at the two small sizes: one-launch loop
+    sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"))
+    rho, f, e = sc.sc_density().cpu().numpy(), sc.sc_forces().cpu().numpy(), sc.sc_energy()
+    tol = (RHO_TOL, FORCE_TOL, ENERGY_TOL) if precision == 0 else (2e-6, 1e-5, 1e-7)
+    assert np.max(np.abs(rho - rho_o) / rho_o) < tol[0]
+    assert rel_l2(f, f_o) < tol[1]
+    assert rel(e, e_o) < tol[2]
+    # the plan can change under a live context: next evaluation uses the new one, same results to rounding
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3_PIECES, 0)
+    f2, e2 = sc.sc_forces().cpu().numpy(), sc.sc_energy()
+    assert rel_l2(f2, f) < (1e-12 if precision == 0 else 1e-6) and rel(e2, e) < (1e-13 if precision == 0 else 1e-7)
+    for bad in (-2, 17):
+        with pytest.raises(scmd.ScError):
+            sc.sc_set_option(scmd.SC_OPT_NEWTON3_PIECES, bad)
+    sc.close()
+
+
 def test_newton3_trajectory(scmd, oracle_ld):
     """100 velocity-Verlet steps at N = 8192 through the Newton's-third-law sweeps: positions within 1e-8 A."""
     import torch
