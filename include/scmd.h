@@ -103,12 +103,16 @@ typedef enum {
                                      values are raised to 8; one-launch step loop: threads of a
                                      row inside one warp)                                        */
     SC_OPT_WARPS_PER_CTA = 3,     /* consumer warps per CTA (they split the j range): 1..8      */
-    SC_OPT_PERSISTENT = 4,        /* all pairs, N <= 6144: the whole sc_step loop (all nsteps) in ONE
-                                     cooperative launch, records staged in shared memory, grid
-                                     barriers between the phases of a step.  0: library default
-                                     (on for N <= 4096, mixed precision N <= 2304: the measured
-                                     crossovers), 1: on, 2: never (one launch per
-                                     sweep and per integrator stage).  Off while sc_profile is on. */
+    SC_OPT_PERSISTENT = 4,        /* all pairs: the whole sc_step loop (all nsteps) in ONE cooperative
+                                     launch with grid barriers between the phases of a step.  Two
+                                     such loops exist: the one-sided one with the records staged in
+                                     shared memory (N <= 6144, any thermostat), and the one through
+                                     the Newton's-third-law sweeps (NVE steps, 2048 <= N <= 12288).
+                                     0: library default (the first for N <= 2304, the second for NVE
+                                     steps where SC_OPT_NEWTON3 applies and N <= 12288: the measured
+                                     crossovers), 1: the first, 2: neither (one launch per sweep
+                                     and per integrator stage), 3: never the first.  Off while
+                                     sc_profile is on.                                          */
     SC_OPT_ENERGY_EVERY_STEP = 5, /* 1: accumulate pair energy on every step of sc_step          */
     SC_OPT_NEIGHBOUR_CAPACITY = 6,/* K_max entries per row of the Verlet list (cutoff path); rounded
                                      down to a multiple of 32 (at least 32)                      */
@@ -120,8 +124,7 @@ typedef enum {
     SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 2048 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
-                                     both atoms.  0: library default (on from N = 4097, mixed
-                                     precision 4609), 1: on,
+                                     both atoms.  0: library default (on from N = 2305), 1: on,
                                      2: off = the one-sided sweeps                               */
     SC_OPT_CUTOFF_SHIFT = 11,     /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
                                      configs; 1 energy-shifted terms: inside r_cut every pair term

@@ -61,19 +61,20 @@ __device__ __forceinline__ double rot1(double v) {   // as a 64-bit integer: two
 }
 __device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
 
+// One CTA's piece of a sweep (the whole of allpairs_n3_kernel; a phase of n3_loop_kernel, sc_n3_loop.cuh).
+// red: per-warp row sums of the epilogue, also the chunk records during the rotation; red_e: per-warp energy sums.
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
-__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3Args a) {
+__device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece, double (&red)[kN3Warps][IT][3][32],
+                                               double (&red_e)[kN3Warps]) {
     constexpr int RB = 32 * IT;
-    __shared__ double red[kN3Warps][IT][3][32];            // epilogue: per-warp row sums
-    __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;                          // 12, or 6 (two CTAs per SM: finer tiles for mid-size clusters)
     const int N = a.n_atoms;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
     double esum = 0.0;
-    const int t_end = a.piece_start[blockIdx.x + 1];
-    for (int t = a.piece_start[blockIdx.x]; t < t_end; ++t) {
+    const int t_end = a.piece_start[piece + 1];
+    for (int t = a.piece_start[piece]; t < t_end; ++t) {
     const N3Tile tile = a.tiles[t];
     const int row0 = tile.b * RB;
 
@@ -219,9 +220,16 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < NW; ++w) tot += red_e[w];
-            a.partial[blockIdx.x] = 2.0 * tot;   // every unordered pair stands for two ordered ones
+            a.partial[piece] = 2.0 * tot;        // every unordered pair stands for two ordered ones
         }
     }
+}
+
+template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
+__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3Args a) {
+    __shared__ double red[kN3Warps][IT][3][32];
+    __shared__ double red_e[kN3Warps];
+    n3_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, red, red_e);
 }
 
 // ---- mixed precision: the same rotation in binary32 on split records (x = xh + xl, RecF), binary64 accumulation ----
@@ -256,10 +264,9 @@ __device__ __forceinline__ f2 rot1_f2(f2 v) {      // the 64-bit shuffle: two SH
 }
 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
-__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3FArgs a) {
+__device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piece, double (&red)[kN3Warps][IT][3][32],
+                                                double (&red_e)[kN3Warps]) {
     constexpr int RB = 32 * IT;
-    __shared__ double red[kN3Warps][IT][3][32];
-    __shared__ double red_e[kN3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
     const int N = a.n_atoms;
@@ -268,8 +275,8 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
     const f2 zero2 = f2_dup(0.f), one2 = f2_dup(1.0f), mone2 = f2_dup(-1.0f), mhalf2 = f2_dup(-0.5f);
     constexpr float kFarF = 1.0e15f;
     double esum = 0.0;
-    const int t_end = a.piece_start[blockIdx.x + 1];
-    for (int t = a.piece_start[blockIdx.x]; t < t_end; ++t) {
+    const int t_end = a.piece_start[piece + 1];
+    for (int t = a.piece_start[piece]; t < t_end; ++t) {
     const N3Tile tile = a.tiles[t];
     const int row0 = tile.b * RB;
     const int cb = row0 >> 6;
@@ -448,9 +455,16 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < NW; ++w) tot += red_e[w];
-            a.partial[blockIdx.x] = 2.0 * tot;
+            a.partial[piece] = 2.0 * tot;
         }
     }
+}
+
+template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
+__global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3FArgs a) {
+    __shared__ double red[kN3Warps][IT][3][32];
+    __shared__ double red_e[kN3Warps];
+    n3p_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, red, red_e);
 }
 
 // ---- finalize: self[i] + part[0 .. block(i)][i] in that order ----
@@ -476,43 +490,67 @@ struct N3FinalArgs {
 constexpr int kN3FinAtoms = 32;         // atoms per CTA of the finalize kernel: one per lane
 constexpr int kN3FinWarps = 8;          // its warps share the segments and the row blocks of those atoms
 
-#ifdef SCMD_MAIN_TU
-// A CTA takes 32 consecutive atoms (one per lane: every load is a contiguous 256 B or 1 KB line run); warp w sums the
-// segments sg = w, w + 8, ... and the row blocks b = w, w + 8, ... <= block(i), then the 8 sums are added in warp order.
+// A group of 32 consecutive atoms (one per lane: every load is a contiguous 256 B or 1 KB line run): warp w < 8 sums
+// the tiles' row sums sg = w, w + 8, ... and the row blocks b = w, w + 8, ... <= block(i), then the 8 sums are added in
+// warp order.  Always 8 summing warps, whatever the CTA (n3_finalize_kernel: 8 warps, one group per CTA; n3_loop_kernel:
+// 12 warps, 4 of them idle in the first part), so that every path gives the same bits.
 // (One thread per atom walking all blocks left 32 CTAs on 148 SMs at N = 8000: 21 us for the force variant.)
-template <bool FORCE>
-__global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3FinalArgs a) {
-    __shared__ double red[kN3FinWarps][3][32];
+// Up to GB groups g0, g0 + gstride, ... at once: their loads are independent and issued together (the phase is a chain
+// of L2 latencies: one group after the other cost the loop kernel 2 us per group), warp u then finishes group u.
+template <bool FORCE, int GB>
+__device__ __forceinline__ void n3_finalize_groups(const N3FinalArgs &a, const int g0, const int gstride, const int cnt,
+                                                   double (*red)[kN3FinWarps][3][32]) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int i = blockIdx.x * kN3FinAtoms + lane;
-    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-    if (i < a.n_atoms) {
-        const int bi = i / a.rb;
-        const int nseg = a.blk_slots[bi];
-        for (int sg = w; sg < nseg; sg += kN3FinWarps) {    // row sums of the segments of i's own block
-            const double4 s = a.self[size_t(sg) * a.n_pad + i];
-            v0 += s.x; v1 += s.y; v2 += s.z;
-        }
-#pragma unroll 4
-        for (int b = w; b <= bi; b += kN3FinWarps) {
-            const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(i - b * a.rb);
-            if constexpr (FORCE) {
-                const double4 p = a.part[at];
-                v0 += p.x; v1 += p.y; v2 += p.z;
-            } else {
-                v0 += a.part_rho[at];
+    double v[GB][3];
+    int ii[GB], bi[GB], nseg[GB];
+    int bmax = -1, smax = 0;
+#pragma unroll
+    for (int u = 0; u < GB; ++u) {
+        v[u][0] = v[u][1] = v[u][2] = 0.0;
+        ii[u] = (g0 + u * gstride) * kN3FinAtoms + lane;
+        const bool live = u < cnt && ii[u] < a.n_atoms && w < kN3FinWarps;
+        bi[u] = live ? ii[u] / a.rb : -1;
+        nseg[u] = live ? a.blk_slots[bi[u]] : 0;
+        bmax = max(bmax, bi[u]); smax = max(smax, nseg[u]);
+    }
+    for (int sg = w; sg < smax; sg += kN3FinWarps) {        // row sums of the tiles of i's own block
+#pragma unroll
+        for (int u = 0; u < GB; ++u)
+            if (sg < nseg[u]) {
+                const double4 s = a.self[size_t(sg) * a.n_pad + ii[u]];
+                v[u][0] += s.x; v[u][1] += s.y; v[u][2] += s.z;
             }
+    }
+#pragma unroll 4
+    for (int b = w; b <= bmax; b += kN3FinWarps) {
+#pragma unroll
+        for (int u = 0; u < GB; ++u)
+            if (b <= bi[u]) {
+                const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(ii[u] - b * a.rb);
+                if constexpr (FORCE) {
+                    const double4 p = a.part[at];
+                    v[u][0] += p.x; v[u][1] += p.y; v[u][2] += p.z;
+                } else {
+                    v[u][0] += a.part_rho[at];
+                }
+            }
+    }
+    if (w < kN3FinWarps) {
+#pragma unroll
+        for (int u = 0; u < GB; ++u) {
+            red[u][w][0][lane] = v[u][0];
+            if constexpr (FORCE) { red[u][w][1][lane] = v[u][1]; red[u][w][2][lane] = v[u][2]; }
         }
     }
-    red[w][0][lane] = v0;
-    if constexpr (FORCE) { red[w][1][lane] = v1; red[w][2][lane] = v2; }
     __syncthreads();
-    if (w != 0) return;
-    v0 = 0.0; v1 = 0.0; v2 = 0.0;
+    if (w < cnt && w < GB) {                               // warp u finishes group u
+    const int group = g0 + w * gstride;
+    const int i = group * kN3FinAtoms + lane;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
 #pragma unroll
     for (int k = 0; k < kN3FinWarps; ++k) {
-        v0 += red[k][0][lane];
-        if constexpr (FORCE) { v1 += red[k][1][lane]; v2 += red[k][2][lane]; }
+        v0 += red[w][k][0][lane];
+        if constexpr (FORCE) { v1 += red[w][k][1][lane]; v2 += red[w][k][2][lane]; }
     }
     double contrib = 0.0;
     if (i < a.n_atoms) {
@@ -547,15 +585,36 @@ __global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3F
     }
     if constexpr (!FORCE) {
         const double t = warp_sum(contrib);
-        if (lane == 0) a.partial[blockIdx.x] = t;
+        if (lane == 0) a.partial[group] = t;
     } else {
         if (a.fuse == 1) {
             const double t = warp_sum(contrib);
-            if (lane == 0) a.part_ke[blockIdx.x] = t;
+            if (lane == 0) a.part_ke[group] = t;
         }
     }
+    }   // finishing warp
+    __syncthreads();                                       // red is free again
+}
+
+#ifdef SCMD_MAIN_TU
+template <bool FORCE>
+__global__ void __launch_bounds__(kN3FinWarps * 32) n3_finalize_kernel(const N3FinalArgs a) {
+    __shared__ double red[1][kN3FinWarps][3][32];
+    n3_finalize_groups<FORCE, 1>(a, blockIdx.x, 0, 1, red);
 }
 #endif  // SCMD_MAIN_TU
+
+// ---- the whole sc_step loop in one cooperative launch (sc_n3_loop.cuh, instantiated in inst_n3_loop.cu) ----
+struct N3LoopArgs {
+    N3Args s;                           // FP64 sweeps ...
+    N3FArgs sf;                         // ... or the mixed ones
+    N3FinalArgs f;                      // finalize (fuse is set by the kernel)
+    unsigned long long *barrier;        // grid barrier counter; the host tracks its value
+    unsigned long long barrier_base;
+    long long nsteps;
+    int energy_every;                   // 1: the pair energy on every step (SC_OPT_ENERGY_EVERY_STEP), else on the last only
+};
+const void *n3_loop_fn(bool fast, bool mixed);
 
 // instantiated in inst_allpairs_n3.cu; nullptr if this shape is not compiled
 const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy);

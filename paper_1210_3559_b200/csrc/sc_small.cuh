@@ -117,22 +117,6 @@ __device__ __forceinline__ double warp0_sum_partials(const double *part, int n) 
     return s;
 }
 
-// Grid-wide barrier on a monotonically increasing counter (all CTAs are resident: cooperative launch).
-// Release: every thread's writes -> bar.sync -> thread 0: fence + atomic add.  Acquire: thread 0 spins on
-// an acquire load until all CTAs of this generation have arrived -> bar.sync.
-__device__ __forceinline__ void grid_barrier(unsigned long long *counter, unsigned long long target) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        // release: the CTA's writes (ordered before this by the bar.sync above) are visible to whoever acquires the count
-        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(counter) : "memory");
-        unsigned long long seen;
-        do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(counter) : "memory");
-        } while (seen < target);
-    }
-    __syncthreads();
-}
-
 // one term of sweep 1: r^-m (self == true: the reciprocal is replaced by 0, so the term is exactly 0)
 template <int ME>
 __device__ __forceinline__ double small_density_term(const double4 &pi, const double4 &p, bool self, int m_exp) {

@@ -67,6 +67,8 @@ struct sc_ctx {
     double4 *n3_self = nullptr;
     N3Tile *n3_tiles = nullptr;   // ... and their plan (plan_n3): tiles, first tile of each CTA's piece, slots per row block
     int *n3_piece_start = nullptr, *n3_blk_slots = nullptr;
+    unsigned long long *n3_barrier = nullptr;      // grid barrier counter of n3_loop_kernel; the host tracks the value
+    unsigned long long n3_barrier_count = 0;
     double *sprime = nullptr;     // [N] s' of the current step (one-launch step loop)
     unsigned long long *small_barrier = nullptr;   // its grid barrier counter; the host tracks the value
     unsigned long long small_barrier_count = 0;
@@ -174,7 +176,7 @@ int cutoff_max_dim(int64_t N) {
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
 constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
-constexpr int64_t kN3DefaultMinAtoms = 4097, kN3DefaultMinAtomsMixed = 4609;   // measured crossovers
+constexpr int64_t kN3DefaultMinAtoms = 2305, kN3DefaultMinAtomsMixed = 2305;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;
 constexpr int kN3MaxSegments = 25;                             // j segments (tiles) of the longest row block
 constexpr int kN3MaxPieces = 4096;                             // CTAs of a balanced plan (16 per SM on 256 SMs)
@@ -220,7 +222,11 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         N3Tile *tl = w.take<N3Tile>(n3_tile_capacity(N));
         int *ps = w.take<int>(n3_tile_capacity(N) + 1);
         int *bs = w.take<int>(size_t(ceil_div(N, int64_t(32 * kN3RowsPerThread))));
-        if (c && base) { c->n3_part = np; c->n3_self = ns; c->n3_tiles = tl; c->n3_piece_start = ps; c->n3_blk_slots = bs; if (xr) c->xfr = xr; }
+        unsigned long long *nbar = w.take<unsigned long long>(2);
+        if (c && base) {
+            c->n3_part = np; c->n3_self = ns; c->n3_tiles = tl; c->n3_piece_start = ps; c->n3_blk_slots = bs; c->n3_barrier = nbar;
+            if (xr) c->xfr = xr;
+        }
     }
     if (precision == SC_PREC_MIXED && !(prm->r_cut > 0.0)) {
         FPair *xf = w.take<FPair>((n + kTileAtoms) / 2 + 1);
@@ -743,10 +749,13 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
 // measured crossovers with the multi-launch path (Newton's-third-law sweeps, FP64; one-sided packed sweeps, mixed):
 // FP64: N = 3000 43 us per step either way, N = 4096 62.5 (loop) against 61.5 us, N = 5000 129 against 68 us;
 // mixed: N = 2057 23 (loop) against 28 us, N = 2500 44 against 37 us
-constexpr int64_t kSmallDefaultMaxAtoms = 4096, kSmallDefaultMaxAtomsMixed = 2304;
+// round 2, after the balanced plan and n3_loop_kernel (500-step NVE calls, us per step, one-launch loop of sc_small.cuh
+// against the Newton's-third-law loop): FP64 N = 2057 20.5 / 24.3, 2304 22.0 / 24.7, 2560 37.5 / 24.5, 3072 43.9 / 30.5,
+// 4096 62.2 / 39.0; mixed 2304 21.7 / 23.4, 2560 38.0 / 23.6, 3072 44.7 / 30.9
+constexpr int64_t kSmallDefaultMaxAtoms = 2304, kSmallDefaultMaxAtomsMixed = 2304;
 
 bool small_path_wanted(const sc_ctx *c) {
-    if (c->cutoff || !c->xs_b || c->opt_persistent == 2 || c->profile || c->split) return false;
+    if (c->cutoff || !c->xs_b || c->opt_persistent >= 2 || c->profile || c->split) return false;
     if (c->N > kSmallMaxAtoms) return false;
     return c->opt_persistent == 1 || c->N <= (c->precision == SC_PREC_MIXED ? kSmallDefaultMaxAtomsMixed : kSmallDefaultMaxAtoms);
 }
@@ -814,6 +823,58 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
     return SC_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// NVE steps through the Newton's-third-law sweeps in one cooperative launch (sc_n3_loop.cuh)
+// ---------------------------------------------------------------------------------------------
+// Measured against the four launches per step (300-step calls, us per step): N = 4096 39.0 / 45.1, N = 8000 100.2 / 103.1,
+// mixed 82.6 / 87.9, N = 16384 353.7 / 352.6, N = 32768 1373 / 1328: beyond ~12000 atoms the finalize phases, which read
+// N^2 / 256 partial records with 8 warps per SM, cost more than the stand-alone finalize kernels (64 warps per SM) save.
+constexpr int64_t kN3LoopMaxAtoms = 12288;
+
+bool n3_loop_wanted(const sc_ctx *c, int thermo) {
+    return thermo == SC_THERMO_NONE && n3_wanted(c) && !c->profile && c->opt_persistent != 2 && c->n3_barrier &&
+           c->N <= kN3LoopMaxAtoms && !(c->opt_warps && c->opt_warps <= 6) && c->opt_n3_pieces >= 0 && c->opt_n3_pieces <= 1;
+}
+
+// positions already carry the first half kick + drift of the call's first step (kick_drift_kernel)
+sc_status run_n3_loop(sc_ctx *c, double dt, int64_t nsteps) {
+    const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
+    const int N = int(c->N), rb = 32 * kN3RowsPerThread;
+    if (!c->n3_seg) {
+        sc_status st = plan_n3(c);
+        if (st != SC_OK) return st;
+    }
+    const int pieces = c->n3_seg;
+    const void *fn = n3_loop_fn(fast, mixed);
+    N3LoopArgs a{};
+    a.s.xs = c->xs; a.s.n_atoms = N; a.s.n_pad = round_up(N, 32);
+    a.s.part = c->n3_part; a.s.part_rho = reinterpret_cast<double *>(c->n3_part); a.s.self = c->n3_self;
+    a.s.partial = c->part_b; a.s.tiles = c->n3_tiles; a.s.piece_start = c->n3_piece_start; a.s.c = c->consts;
+    a.sf.xfr = c->xfr; a.sf.n_atoms = N; a.sf.n_pad = a.s.n_pad; a.sf.part = a.s.part; a.sf.part_rho = a.s.part_rho;
+    a.sf.self = a.s.self; a.sf.partial = a.s.partial; a.sf.tiles = a.s.tiles; a.sf.piece_start = a.s.piece_start; a.sf.c = a.s.c;
+    N3FinalArgs &f = a.f;
+    f.xs = c->xs; f.xfr = mixed ? c->xfr : nullptr; f.xf = mixed ? c->xf : nullptr; f.part = c->n3_part; f.part_rho = a.s.part_rho;
+    f.self = c->n3_self; f.rho = c->rho; f.force = c->force; f.partial = c->part_a; f.n_atoms = N; f.n_pad = a.s.n_pad; f.rb = rb;
+    f.blk_slots = c->n3_blk_slots; f.c = c->consts; f.fuse = 0; f.vel = c->vel; f.part_ke = c->stage_a;
+    f.hk = 0.5 * dt * kAcc / c->p.mass; f.dt = dt;
+    a.barrier = c->n3_barrier; a.barrier_base = c->n3_barrier_count;
+    a.nsteps = nsteps; a.energy_every = c->opt_energy_every;
+    void *params[] = {&a};
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(pieces), dim3(kN3Warps * 32), params, 0, c->stream);
+    if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law step loop: %s", cudaGetErrorString(e));
+    c->launches += 1;
+    c->n3_barrier_count += (4 * uint64_t(nsteps) - 1) * uint64_t(pieces);
+    const int nfin = ceil_div(N, kN3FinAtoms);
+    reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, pieces, c->scal, kSlotEPair, c->consts.En);
+    reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, nfin, c->scal, kSlotEEmb, -c->consts.eps_c);
+    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->stage_a, nfin, c->scal, c->p.mass, double(3 * c->N - 3), SC_THERMO_NONE, 0.0);
+    SC_CUDA_CHECK(c, cudaGetLastError());
+    c->launches += 3;
+    c->emb_pending = 0;
+    c->density_valid = c->forces_valid = c->energy_valid = true;
+    return SC_OK;
+}
+
 sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps) {
     if (!c->have_pos || !c->have_vel) return fail(c, SC_ERR_STATE, "sc_step: positions and velocities must be set%s");
     if (!(dt > 0.0) || !std::isfinite(dt) || nsteps < 0) return fail(c, SC_ERR_INVALID, "sc_step: dt must be > 0, nsteps >= 0%s");
@@ -840,6 +901,13 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
     // the last step) the first half kick and the drift of the next step: 4 launches per step instead of 6
     const bool fused = thermo == SC_THERMO_NONE && n3_wanted(c) && !c->profile;
     const int nfin = ceil_div(N, kN3FinAtoms);
+    if (n3_loop_wanted(c, thermo)) {
+        kick_drift_kernel<<<nb, kBlock, 0, c->stream>>>(c->xs, c->vel, c->force, c->scal, nullptr, c->xf, c->xfr, 0, N, hk, dt);
+        SC_CUDA_CHECK(c, cudaGetLastError());
+        c->launches += 1;
+        c->density_valid = c->forces_valid = c->energy_valid = false;
+        return run_n3_loop(c, dt, nsteps);
+    }
     for (int64_t k = 1; k <= nsteps; ++k) {
         const bool last = (k == nsteps);
         if (!fused || k == 1) {
@@ -963,6 +1031,10 @@ sc_status sc_create_ex(const sc_params *params, int64_t n_atoms, int32_t precisi
     }
     reset_lambda_kernel<<<1, 1, 0, c->stream>>>(c->scal);
     if (cudaGetLastError() != cudaSuccess) { delete c; return SC_ERR_CUDA; }
+    if (c->n3_barrier && cudaMemsetAsync(c->n3_barrier, 0, 2 * sizeof(unsigned long long), c->stream) != cudaSuccess) {
+        delete c;
+        return SC_ERR_CUDA;
+    }
     if (c->small_barrier && cudaMemsetAsync(c->small_barrier, 0, 2 * sizeof(unsigned long long), c->stream) != cudaSuccess) {
         delete c;
         return SC_ERR_CUDA;
@@ -1016,7 +1088,7 @@ sc_status sc_set_option(sc_ctx *c, int32_t option, int64_t value) {
                 return fail(c, SC_ERR_INVALID, "warps per CTA must be 0..8%s");
             c->opt_warps = int(value); c->n3_seg = 0; break;
         case SC_OPT_PERSISTENT:
-            if (value < 0 || value > 2) return fail(c, SC_ERR_INVALID, "persistent must be 0, 1 or 2%s");
+            if (value < 0 || value > 3) return fail(c, SC_ERR_INVALID, "persistent must be 0, 1, 2 or 3%s");
             c->opt_persistent = int(value); break;
         case SC_OPT_ENERGY_EVERY_STEP:
             c->opt_energy_every = value ? 1 : 0; break;

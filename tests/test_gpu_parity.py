@@ -151,6 +151,39 @@ def test_newton3_trajectory(scmd, oracle_ld):
     sc.close()
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("n_atoms", [2305, 5003, 12288])
+def test_newton3_step_loop(scmd, oracle_ld, n_atoms, precision):
+    """n3_loop_kernel (csrc/sc_n3_loop.cuh): NVE sc_step calls through the Newton's-third-law sweeps in one cooperative
+    launch.  Same device functions, same sums in the same order as the four launches per step (SC_OPT_PERSISTENT = 2),
+    so positions, velocities, forces and energies agree bit for bit, also over split calls; and against the oracle."""
+    import torch
+    w = W.fcc_cluster(n_atoms, 1200.0, seed=86)
+    out = {}
+    for mode in (0, 2):
+        sc = scmd.SuttonChen(n_atoms, precision=precision)
+        sc.sc_set_option(scmd.SC_OPT_PERSISTENT, mode)
+        assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == 1
+        sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"), torch.as_tensor(w.vel, device="cuda"))
+        sc.sc_forces()
+        before = sc.sc_launch_count()
+        sc.sc_step(1.0, 7)
+        used = sc.sc_launch_count() - before
+        assert used == 5 if mode == 0 else used >= 4 * 7   # first half kick + drift, the loop, three scalar reductions
+        sc.sc_step(1.0, 1)
+        sc.sc_step(1.0, 12)
+        pos, vel = sc.sc_get_state()
+        out[mode] = (pos.cpu().numpy(), vel.cpu().numpy(), sc.sc_forces().cpu().numpy(), sc.sc_energy(), sc.sc_kinetic()[0],
+                     sc.sc_density().cpu().numpy())
+        sc.close()
+    for a, b in zip(out[0], out[2]):
+        assert np.array_equal(a, b)
+    ref = oracle_ld.run(w.pos, w.vel, oracle_ld.params(), dt=1.0, nsteps=20)
+    assert np.abs(out[0][0] - ref["pos"]).max() < (TRAJ_TOL if precision == 0 else 1e-5)
+    assert rel(out[0][3], ref["epot"][-1]) < (1e-10 if precision == 0 else 1e-7)
+    assert rel(out[0][4], ref["ekin"][-1]) < (1e-10 if precision == 0 else 1e-6)
+
+
 @pytest.mark.parametrize("n_atoms", [1, 2, 3, 31, 33, 511, 512, 513, 1025])
 def test_small_and_boundary_sizes(scmd, oracle_ld, n_atoms):
     """Degenerate and tile-boundary sizes.  N = 1: rho = 0, F = 0, U = 0 (reading Q9)."""
