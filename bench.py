@@ -306,14 +306,18 @@ def measure(scmd, spec: Spec, steps: int, warmup: int, rank: int, world: int, de
     # which kernels the library runs for this context is the library's choice: ask it (SC_INFO_STEP_PATH).
     # In the one-launch loop (small all-pairs clusters, csrc/sc_small.cuh) a bench step is one sc_step call of
     # MD_PER_CALL MD steps and the roofline kernel is the loop itself.
+    # Where the library runs all steps of a call in one launch (SC_INFO_ONE_LAUNCH: the one-sided loop for small
+    # clusters, the Newton's-third-law loop up to 12288 atoms) a bench step is one sc_step call of 100 MD steps and the
+    # roofline kernel is the loop itself: the WHOLE step (both sweeps, finalize phases, integrator, grid barriers) is
+    # set against the sweeps' instruction counts.
     step_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)
-    one_launch = step_path == 2
+    one_launch = sc.sc_get_option(scmd.SC_INFO_ONE_LAUNCH) == 1
     md_per_call = 100 if one_launch else 1
     if not one_launch:
         sc.sc_profile(True)
-        sweep_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)          # profiling forbids the loop: the path that is timed
+        sweep_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)          # profiling forbids the loops: the path that is timed
     else:
-        sweep_path = 2
+        sweep_path = step_path
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = torch.cuda.current_stream()
 
@@ -346,7 +350,9 @@ def measure(scmd, spec: Spec, steps: int, warmup: int, rank: int, world: int, de
         dist.barrier()
     launches = sc.sc_launch_count() - launches0
     if one_launch:
-        assert launches == steps, f"one-launch loop expected, {launches} launches in {steps} calls"
+        # the loop itself; on the Newton's-third-law path also the call's first half kick + drift and three scalar reductions
+        per_call = 1 if step_path == 2 else 5
+        assert launches == per_call * steps, f"one-launch loop expected, {launches} launches in {steps} calls"
     stats1 = sc.sc_stats()
     local_ms = sum(a.elapsed_time(b) for a, b in ev)
     out = dict(w=w, N=N, pairs_per_step=pairs_per_step, md_per_call=md_per_call, one_launch=one_launch,
@@ -405,7 +411,9 @@ def roofline_block(scmd, spec: Spec, m: dict, steps: int) -> dict:
                 if row["workload"] == spec.name:
                     traffic = float(row["force_sweep_dram_bytes_per_launch"])
                     traffic_source = "committed ncu reading, not measured in this run: " + row["source"]
-    if m["one_launch"]:
+    if m["one_launch"] and newton3:
+        kernel = "n3_loop_kernel (whole step loop: Newton's-third-law sweeps, their finalize phases with the integrator, grid barriers; one launch)"
+    elif m["one_launch"]:
         kernel = "small_step_kernel (whole step loop: both sweeps + integrator, one launch)"
     elif newton3:
         kernel = ("allpairs_n3_kernel" if spec.prec == "fp64" else "allpairs_n3p_kernel") + \
@@ -425,6 +433,8 @@ def roofline_block(scmd, spec: Spec, m: dict, steps: int) -> dict:
                 "alu_inst_per_pair": i_f, "ms_force_sweep": t_force * 1e3, "ms_density_sweep": t_density * 1e3,
                 "density_sweep_frac": i_d * 2.0 * pairs_per_step / t_density / 1e12 / peak,
                 "both_sweeps_frac": (i_d + i_f) * 2.0 * pairs_per_step / (t_force + t_density) / 1e12 / peak}
+    roofline["sweep_timing"] = ("whole MD step of the one-launch loop, split between the sweeps by instruction count" if m["one_launch"]
+                                else "library events inside the timed region")
     if newton3:
         # the same time measured against the ONE-SIDED instruction count (22 per ordered pair, the formulation
         # BASELINE.json's north_star names): a speed-up figure (> 1 = faster than a one-sided sweep at FP64 peak),

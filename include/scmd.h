@@ -147,7 +147,9 @@ typedef enum {
                                          0 one-sided all-pairs sweeps, 1 Newton's-third-law all-pairs sweeps,
                                          2 the one-launch step loop (sc_step only; its sc_forces is 0 or 1), 3 cutoff lists */
     SC_INFO_NEIGHBOUR_CAPACITY = 101, /* cutoff path: K_max entries per atom the rows hold now (0 for all pairs)       */
-    SC_INFO_NEIGHBOUR_CAPACITY_MAX = 102 /* ... and the largest value the workspace was sized for                        */
+    SC_INFO_NEIGHBOUR_CAPACITY_MAX = 102, /* ... and the largest value the workspace was sized for                       */
+    SC_INFO_ONE_LAUNCH = 103          /* 1 if an NVE sc_step call runs all its steps in one cooperative launch as the
+                                         context is configured now (SC_OPT_PERSISTENT), else 0                          */
 } sc_info;
 
 /* Optional create-time sizing (sc_workspace_bytes_ex / sc_create_ex).  Zero-initialise, then set what is needed;

@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
     SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY, SC_OPT_LANGEVIN_STEP, SC_OPT_CELLS_PER_RADIUS,
     SC_OPT_ATOMS_PER_CTA, SC_OPT_NEWTON3, SC_OPT_CUTOFF_SHIFT, SC_OPT_NEWTON3_PIECES,
-    SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX, ScCreateOptions, load_probe_library,
+    SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX, SC_INFO_ONE_LAUNCH, ScCreateOptions, load_probe_library,
     ScError, ScParams, ScThermostat, SuttonChen, load_library, library_path, exported_symbols,
     probe_throughput, probe_reciprocal, NI_PARAMS, rescale_thermostat, langevin_thermostat,
 )

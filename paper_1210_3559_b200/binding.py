@@ -17,7 +17,7 @@ SC_THERMO_NONE, SC_THERMO_RESCALE, SC_THERMO_LANGEVIN = 0, 1, 2
 (SC_OPT_ROWS_PER_THREAD, SC_OPT_LANES_PER_ROW, SC_OPT_WARPS_PER_CTA, SC_OPT_PERSISTENT,
  SC_OPT_ENERGY_EVERY_STEP, SC_OPT_NEIGHBOUR_CAPACITY, SC_OPT_LANGEVIN_STEP, SC_OPT_CELLS_PER_RADIUS,
  SC_OPT_ATOMS_PER_CTA, SC_OPT_NEWTON3, SC_OPT_CUTOFF_SHIFT, SC_OPT_NEWTON3_PIECES) = range(1, 13)
-SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX = 100, 101, 102
+SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX, SC_INFO_ONE_LAUNCH = 100, 101, 102, 103
 _STATUS_NAMES = ["SC_OK", "SC_ERR_INVALID", "SC_ERR_CUDA", "SC_ERR_NOMEM", "SC_ERR_STATE",
                  "SC_ERR_NONFINITE", "SC_ERR_CAPACITY"]
 

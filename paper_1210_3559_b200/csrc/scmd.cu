@@ -177,7 +177,9 @@ int cutoff_max_dim(int64_t N) {
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
 constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
 constexpr int64_t kN3DefaultMinAtoms = 2305, kN3DefaultMinAtomsMixed = 2305;   // measured crossovers
-constexpr int kN3RowsPerThread = 4;
+constexpr int kN3RowsPerThread = 4;     // 2 rows per lane (twice the chunks, half as long) measured in the step loop for small
+                                        // clusters, where the triangle has fewer chunks than the chip has warps: N = 2057 23.4
+                                        // against 24.8, N = 2304 23.3 / 24.3, N = 3072 33.2 / 30.3, N = 4096 48.9 / 38.9 us per step
 constexpr int kN3MaxSegments = 25;                             // j segments (tiles) of the longest row block
 constexpr int kN3MaxPieces = 4096;                             // CTAs of a balanced plan (16 per SM on 256 SMs)
 inline size_t n3_tile_capacity(int64_t N) {                    // the round-1 grid has up to 25 tiles per row block
@@ -1164,6 +1166,7 @@ sc_status sc_get_option(sc_ctx *c, int32_t option, int64_t *value) {
             break;
         case SC_INFO_NEIGHBOUR_CAPACITY: *value = c->cutoff ? c->kmax : 0; break;
         case SC_INFO_NEIGHBOUR_CAPACITY_MAX: *value = c->cutoff ? c->kmax_cap : 0; break;
+        case SC_INFO_ONE_LAUNCH: *value = (small_path_wanted(c) || n3_loop_wanted(c, SC_THERMO_NONE)) ? 1 : 0; break;
         default:
             return fail(c, SC_ERR_INVALID, "sc_get_option: unknown option%s");
     }
