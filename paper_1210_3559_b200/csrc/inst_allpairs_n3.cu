@@ -27,7 +27,6 @@ const void *allpairs_n3p_fn(int it, bool fast, bool force, bool energy) {
 
 const void *allpairs_n3_fn(int it, bool fast, bool force, bool energy) {
     if (it == 4) return fast ? pick<4, 9, 6>(force, energy) : pick<4, 0, 0>(force, energy);
-    if (it == 2) return fast ? pick<2, 9, 6>(force, energy) : pick<2, 0, 0>(force, energy);
     return nullptr;
 }
 }  // namespace scmd

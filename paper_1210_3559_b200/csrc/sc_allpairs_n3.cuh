@@ -101,7 +101,10 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
     // space the epilogue's reduction uses afterwards; (x, y) and (z, s') as two 16-byte arrays: conflict-free), and at
     // step s a lane READS the record of lane + s -- two LDS.128 instead of eight shuffles and the moves that go with
     // them.  Only the reaction sums travel from lane to lane.
-    double2 *jxy = reinterpret_cast<double2 *>(&red[0][0][0][0]) + warp * 64, *jzs = jxy + 32;
+    // Each record is stored twice, at lane and at lane + 32, so that the index lane + s + 1 never wraps: with the steps
+    // unrolled the address is one register plus an immediate (3 integer instructions per step less).
+    static_assert(IT >= 3, "2 KB of chunk records per warp must fit into the warp's part of red");
+    double2 *jxy = reinterpret_cast<double2 *>(&red[0][0][0][0]) + warp * 128, *jzs = jxy + 64;
     for (int c = c_begin + warp; c < c_end; c += NW) {
         const int jidx = (c << 5) + lane;
         double xj, yj, zj, sj;
@@ -119,6 +122,7 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
         struct JRec { double x, y, z, s, g0, g1, g2; };
         __syncwarp();                                      // the previous chunk's readers are done
         jxy[lane] = make_double2(xj, yj); jzs[lane] = make_double2(zj, sj);
+        jxy[lane + 32] = make_double2(xj, yj); jzs[lane + 32] = make_double2(zj, sj);
         __syncwarp();
         const int jbase = c << 5;
         auto step = [&](auto masked, int s, const JRec &in, JRec &out) {
@@ -126,7 +130,7 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
             const int jidx = jbase + ((lane + s) & 31);
             double g0 = in.g0, g1 = in.g1, g2 = in.g2;     // reaction sums travelling with the record
             {   // the record of the NEXT step is fetched first: its latency hides behind this step's arithmetic
-                const int nx = (lane + s + 1) & 31;
+                const int nx = lane + s + 1;               // <= 63: the second copy
                 const double2 pxy = jxy[nx], pzs = jzs[nx];
                 out.x = pxy.x; out.y = pxy.y; out.z = pzs.x; out.s = pzs.y;
             }
@@ -180,7 +184,7 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
                 step(std::integral_constant<bool, true>{}, s + 1, B, A);
             }
         } else {
-#pragma unroll 2
+#pragma unroll 4
             for (int s = 0; s < 32; s += 2) {
                 step(std::integral_constant<bool, false>{}, s, A, B);
                 step(std::integral_constant<bool, false>{}, s + 1, B, A);
