@@ -617,6 +617,8 @@ struct N3LoopArgs {
     unsigned long long barrier_base;
     long long nsteps;
     int energy_every;                   // 1: the pair energy on every step (SC_OPT_ENERGY_EVERY_STEP), else on the last only
+    int thermo;                         // 0: NVE; 1: velocity rescaling to the ramp T_start -> T_end
+    double T_start, T_end, mass, ndof;
 };
 const void *n3_loop_fn(bool fast, bool mixed);
 

@@ -834,12 +834,12 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
 constexpr int64_t kN3LoopMaxAtoms = 12288;
 
 bool n3_loop_wanted(const sc_ctx *c, int thermo) {
-    return thermo == SC_THERMO_NONE && n3_wanted(c) && !c->profile && c->opt_persistent != 2 && c->n3_barrier &&
+    return (thermo == SC_THERMO_NONE || thermo == SC_THERMO_RESCALE) && n3_wanted(c) && !c->profile && c->opt_persistent != 2 && c->n3_barrier &&
            c->N <= kN3LoopMaxAtoms && !(c->opt_warps && c->opt_warps <= 6) && c->opt_n3_pieces >= 0 && c->opt_n3_pieces <= 1;
 }
 
 // positions already carry the first half kick + drift of the call's first step (kick_drift_kernel)
-sc_status run_n3_loop(sc_ctx *c, double dt, int64_t nsteps) {
+sc_status run_n3_loop(sc_ctx *c, double dt, const sc_thermostat *th, int thermo, int64_t nsteps) {
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
     const int N = int(c->N), rb = 32 * kN3RowsPerThread;
     if (!c->n3_seg) {
@@ -861,15 +861,21 @@ sc_status run_n3_loop(sc_ctx *c, double dt, int64_t nsteps) {
     f.hk = 0.5 * dt * kAcc / c->p.mass; f.dt = dt;
     a.barrier = c->n3_barrier; a.barrier_base = c->n3_barrier_count;
     a.nsteps = nsteps; a.energy_every = c->opt_energy_every;
+    a.thermo = thermo == SC_THERMO_RESCALE ? 1 : 0;
+    a.mass = c->p.mass; a.ndof = double(3 * c->N - 3);
+    if (th) { a.T_start = th->T_start; a.T_end = th->T_end; }
     void *params[] = {&a};
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(pieces), dim3(kN3Warps * 32), params, 0, c->stream);
     if (e != cudaSuccess) return fail(c, SC_ERR_CUDA, "Newton's-third-law step loop: %s", cudaGetErrorString(e));
     c->launches += 1;
-    c->n3_barrier_count += (4 * uint64_t(nsteps) - 1) * uint64_t(pieces);
+    c->n3_barrier_count += (4 * uint64_t(nsteps) - 1 + (a.thermo ? uint64_t(nsteps) - 1 : 0)) * uint64_t(pieces);
     const int nfin = ceil_div(N, kN3FinAtoms);
     reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_b, pieces, c->scal, kSlotEPair, c->consts.En);
     reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->part_a, nfin, c->scal, kSlotEEmb, -c->consts.eps_c);
-    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->stage_a, nfin, c->scal, c->p.mass, double(3 * c->N - 3), SC_THERMO_NONE, 0.0);
+    // KE and T of the last step; rescaling: its lambda is left pending as on the other paths (flush_lambda)
+    reduce_ke_kernel<<<1, 1024, 0, c->stream>>>(c->stage_a, nfin, c->scal, c->p.mass, a.ndof, thermo,
+                                             a.thermo ? a.T_start + (a.T_end - a.T_start) * double(nsteps) / double(nsteps) : 0.0);
+    if (a.thermo) c->lambda_pending = true;
     SC_CUDA_CHECK(c, cudaGetLastError());
     c->launches += 3;
     c->emb_pending = 0;
@@ -908,7 +914,9 @@ sc_status do_step(sc_ctx *c, double dt, const sc_thermostat *th, int64_t nsteps)
         SC_CUDA_CHECK(c, cudaGetLastError());
         c->launches += 1;
         c->density_valid = c->forces_valid = c->energy_valid = false;
-        return run_n3_loop(c, dt, nsteps);
+        st = run_n3_loop(c, dt, th, thermo, nsteps);
+        if (st != SC_OK) return st;
+        return flush_lambda(c);
     }
     for (int64_t k = 1; k <= nsteps; ++k) {
         const bool last = (k == nsteps);

@@ -184,6 +184,43 @@ def test_newton3_step_loop(scmd, oracle_ld, n_atoms, precision):
     assert rel(out[0][4], ref["ekin"][-1]) < (1e-10 if precision == 0 else 1e-6)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_newton3_step_loop_rescale(scmd, oracle_ld, precision):
+    """Velocity rescaling inside n3_loop_kernel (BASELINE.json config 3's cooling ramp runs through it): two ramps and
+    an NVE leg in separate calls against the oracle's runs, the temperature on target after every call, and the
+    separate-launch path (SC_OPT_PERSISTENT = 2) to rounding."""
+    import torch
+    from paper_1210_3559_b200.binding import rescale_thermostat
+    n_atoms = 2500
+    w = W.fcc_cluster(n_atoms, 2000.0, seed=87)
+    P = oracle_ld.params()
+    legs = [(25, 1, 2000.0, 1800.0), (10, 1, 1800.0, 1850.0), (5, 0, 0.0, 0.0)]
+    pos, vel = w.pos, w.vel
+    for n, kind, a, b in legs:
+        ref = oracle_ld.run(pos, vel, P, dt=1.0, nsteps=n, thermo_kind=kind, T_start=a, T_end=b)
+        pos, vel = ref["pos"], ref["vel"]
+    out = {}
+    for mode in (0, 2):
+        sc = scmd.SuttonChen(n_atoms, precision=precision)
+        sc.sc_set_option(scmd.SC_OPT_PERSISTENT, mode)
+        sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"), torch.as_tensor(w.vel, device="cuda"))
+        sc.sc_forces()
+        for n, kind, a, b in legs:
+            before = sc.sc_launch_count()
+            sc.sc_step(1.0, n, rescale_thermostat(a, b) if kind else None)
+            if mode == 0:
+                assert sc.sc_launch_count() - before <= 7      # kick + drift, the loop, 3 reductions, the pending scale
+            if kind:
+                assert abs(sc.sc_kinetic()[1] - b) < 1e-9
+        gpos, gvel = sc.sc_get_state()
+        out[mode] = (gpos.cpu().numpy(), gvel.cpu().numpy(), sc.sc_energy())
+        sc.close()
+    assert np.abs(out[0][0] - pos).max() < (TRAJ_TOL if precision == 0 else 1e-5)
+    assert np.abs(out[0][1] - vel).max() < (1e-10 if precision == 0 else 1e-6)
+    assert rel(out[0][2], ref["epot"][-1]) < (1e-10 if precision == 0 else 1e-7)
+    assert np.abs(out[0][0] - out[2][0]).max() < (1e-12 if precision == 0 else 1e-7)
+
+
 @pytest.mark.parametrize("n_atoms", [1, 2, 3, 31, 33, 511, 512, 513, 1025])
 def test_small_and_boundary_sizes(scmd, oracle_ld, n_atoms):
     """Degenerate and tile-boundary sizes.  N = 1: rho = 0, F = 0, U = 0 (reading Q9)."""
