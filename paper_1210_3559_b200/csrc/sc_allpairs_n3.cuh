@@ -520,7 +520,7 @@ __device__ __forceinline__ void n3_finalize_groups(const N3FinalArgs &a, const i
     for (int sg = w; sg < smax; sg += kN3FinWarps) {        // row sums of the tiles of i's own block
 #pragma unroll
         for (int u = 0; u < GB; ++u)
-            if (sg < nseg[u]) {
+            if (GB == 1 || sg < nseg[u]) {          // one group: the loop bound is its own
                 const double4 s = a.self[size_t(sg) * a.n_pad + ii[u]];
                 v[u][0] += s.x; v[u][1] += s.y; v[u][2] += s.z;
             }
@@ -529,7 +529,7 @@ __device__ __forceinline__ void n3_finalize_groups(const N3FinalArgs &a, const i
     for (int b = w; b <= bmax; b += kN3FinWarps) {
 #pragma unroll
         for (int u = 0; u < GB; ++u)
-            if (b <= bi[u]) {
+            if (GB == 1 || b <= bi[u]) {
                 const size_t at = n3_part_offset(b, a.n_pad, a.rb) + size_t(ii[u] - b * a.rb);
                 if constexpr (FORCE) {
                     const double4 p = a.part[at];
