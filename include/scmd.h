@@ -307,6 +307,27 @@ sc_status sc_profile_read(sc_ctx *ctx, double *h_ms_density, double *h_ms_force)
 const char *sc_last_error(const sc_ctx *ctx);
 const char *sc_version(void);
 
+/* ---- an entry point that allocates nothing and needs no workspace -----------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it) and so cannot give sc_create a workspace: sweep 1 of the evaluation on its own, all pairs, FP64:
+ *     d_rho[i] = sum_{j != i} (a / r_ij)^m                                   Eq. (2)
+ *     *d_sum_sqrt_rho = sum_i sqrt(d_rho[i])   (U_emb = -eps c times this, Eq. (1); may be NULL)
+ * d_pos: DEVICE, n_atoms x 3 doubles (x, y, z), read only.  d_rho: DEVICE, n_atoms doubles, written.
+ * d_sum_sqrt_rho: DEVICE, one double, written (or NULL).  All caller-owned.  cuda_stream: a cudaStream_t (NULL = the
+ * default stream); the call enqueues one memset and two kernels on it and returns without waiting.
+ * Its scratch -- the packed records and the per-CTA partial sums, which sc_density keeps in the workspace -- lives in a
+ * file-scope device array of SC_NOALLOC_SCRATCH_BYTES inside libscmd.so, which every GPU that loads the library holds
+ * until the process exits; hence n_atoms <= SC_NOALLOC_MAX_ATOMS, and SC_ERR_NOMEM with a message beyond that.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine.  ALL calls share the one array:
+ * two calls that overlap on the GPU (different streams or host threads, same device) race on it -- serialise them.
+ * Errors: SC_ERR_INVALID (NULL pointer, bad exponents, r_cut > 0: all pairs only, n_atoms < 1), SC_ERR_NOMEM
+ * (n_atoms too large), SC_ERR_CUDA; sc_noalloc_last_error gives the calling thread's last message. */
+#define SC_NOALLOC_MAX_ATOMS 16384
+#define SC_NOALLOC_SCRATCH_BYTES (528 * 1024)
+sc_status sc_density_noalloc(const sc_params *params, int64_t n_atoms, const double *d_pos, double *d_rho,
+                             double *d_sum_sqrt_rho, void *cuda_stream);
+const char *sc_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

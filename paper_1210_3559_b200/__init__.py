@@ -15,4 +15,5 @@ from .binding import (  # noqa: F401
     SC_INFO_STEP_PATH, SC_INFO_NEIGHBOUR_CAPACITY, SC_INFO_NEIGHBOUR_CAPACITY_MAX, SC_INFO_ONE_LAUNCH, ScCreateOptions, load_probe_library,
     ScError, ScParams, ScThermostat, SuttonChen, load_library, library_path, exported_symbols,
     probe_throughput, probe_reciprocal, NI_PARAMS, rescale_thermostat, langevin_thermostat,
+    sc_density_noalloc, SC_NOALLOC_MAX_ATOMS,
 )

@@ -100,6 +100,8 @@ def load_library() -> ctypes.CDLL:
         "sc_profile_read": (i32, [vp, DP, DP]),
         "sc_last_error": (ctypes.c_char_p, [vp]),
         "sc_version": (ctypes.c_char_p, []),
+        "sc_density_noalloc": (i32, [PP, i64, vp, vp, vp, vp]),
+        "sc_noalloc_last_error": (ctypes.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -324,6 +326,33 @@ class SuttonChen:
         a, b = ctypes.c_double(), ctypes.c_double()
         self._check(self.lib.sc_profile_read(self._ctx, ctypes.byref(a), ctypes.byref(b)), "sc_profile_read")
         return dict(ms_density=a.value, ms_force=b.value)
+
+
+SC_NOALLOC_MAX_ATOMS = 16384
+
+
+def sc_density_noalloc(d_pos, d_rho, d_sum_sqrt_rho=None, *, n=9, m=6, eps=1.5707e-2, c=39.432, a=3.52, mass=58.69,
+                       stream=None) -> None:
+    """include/scmd.h sc_density_noalloc: rho_i (all pairs, FP64) into the caller's `d_rho` and sum_i sqrt(rho_i) into
+    the caller's one-element `d_sum_sqrt_rho`, with the library's scratch in a static device array: no workspace, no
+    allocation inside the call (the tensors passed in are the caller's).  N <= SC_NOALLOC_MAX_ATOMS."""
+    torch = _torch()
+    lib = load_library()
+    if not (d_pos.is_cuda and d_rho.is_cuda and d_pos.dtype == torch.float64 and d_rho.dtype == torch.float64
+            and d_pos.is_contiguous() and d_rho.is_contiguous() and d_pos.dim() == 2 and d_pos.shape[1] == 3
+            and d_rho.numel() == d_pos.shape[0]):
+        raise ScError(SC_ERR_INVALID, "sc_density_noalloc", "need contiguous float64 CUDA tensors pos[N, 3], rho[N]")
+    if d_sum_sqrt_rho is not None and not (d_sum_sqrt_rho.is_cuda and d_sum_sqrt_rho.dtype == torch.float64
+                                           and d_sum_sqrt_rho.numel() == 1):
+        raise ScError(SC_ERR_INVALID, "sc_density_noalloc", "sum_sqrt_rho must be a one-element float64 CUDA tensor")
+    params = ScParams(int(n), int(m), float(eps), float(c), float(a), float(mass), 0.0)
+    with torch.cuda.device(d_pos.device):
+        s = torch.cuda.current_stream(d_pos.device) if stream is None else stream
+        st = lib.sc_density_noalloc(ctypes.byref(params), int(d_pos.shape[0]), d_pos.data_ptr(), d_rho.data_ptr(),
+                                    d_sum_sqrt_rho.data_ptr() if d_sum_sqrt_rho is not None else None, s.cuda_stream)
+    if st != SC_OK:
+        msg = lib.sc_noalloc_last_error()
+        raise ScError(st, "sc_density_noalloc", msg.decode() if msg else "")
 
 
 def rescale_thermostat(T_start: float, T_end: float) -> ScThermostat:
