@@ -19,6 +19,9 @@
 // result is bit-reproducible.  Storage: ~N^2 / (2 RB) records of 32 bytes (0.54 GB at N = 65536), which is what
 // limits the variant to N <= 262144 (8.6 GB there; kN3MaxAtoms in scmd.cu).
 #pragma once
+#ifndef SCMD_N3P_UNROLL
+#define SCMD_N3P_UNROLL 4      // rotation steps unrolled in the mixed sweeps: 2 x this
+#endif
 #include "sc_allpairs.cuh"
 #include "sc_device.cuh"
 
@@ -267,10 +270,19 @@ __device__ __forceinline__ f2 rot1_f2(f2 v) {      // the 64-bit shuffle: two SH
     return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31);
 }
 
+// Shared memory of the mixed sweeps: per warp 3584 B of chunk records (below), in the same buffer the epilogue's row sums
+// (kN3Warps x IT x 3 x 32 doubles) use afterwards
+constexpr int kN3pWarpBytes = 3 * 64 * 16 + 64 * 8;
+template <int IT>
+constexpr int kN3pSmemDoubles =
+    (kN3Warps * kN3pWarpBytes > kN3Warps * IT * 3 * 32 * 8 ? kN3Warps * kN3pWarpBytes : kN3Warps * IT * 3 * 32 * 8) / 8;
+constexpr int kN3pUnroll = SCMD_N3P_UNROLL;
+
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
-__device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piece, double (&red)[kN3Warps][IT][3][32],
+__device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piece, double *buf /* kN3pSmemDoubles<IT> */,
                                                 double (&red_e)[kN3Warps]) {
     constexpr int RB = 32 * IT;
+    double (&red)[kN3Warps][IT][3][32] = *reinterpret_cast<double (*)[kN3Warps][IT][3][32]>(buf);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
     const int N = a.n_atoms;
@@ -301,7 +313,10 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
     }
     double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
     double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, RB);
-    ulonglong2 *jq = reinterpret_cast<ulonglong2 *>(&red[0][0][0][0]) + warp * 128;   // 4 x 32 x 16 B per warp, aliasing `red`
+    // chunk records of this warp, every record at lane AND lane + 32 so that the index lane + s + 1 never wraps (as in the
+    // FP64 kernel): three arrays of 64 x 16 B -- (xh, yh), (zh, s'), (xl, yl) -- and one of 64 x 8 B (zl)
+    ulonglong2 *jq = reinterpret_cast<ulonglong2 *>(reinterpret_cast<unsigned char *>(buf) + warp * kN3pWarpBytes);
+    unsigned long long *jq3 = reinterpret_cast<unsigned long long *>(jq + 192);
     auto fetch = [&](int j) -> RecF {
         if (j < N) return a.xfr[j];
         return RecF{-kFarF * float((j & 63) + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -324,17 +339,19 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         // the 2 x 32 records of the chunk sit in shared memory (see the FP64 kernel): at step s a lane reads the pair of
         // records of lane + s with four LDS.128 instead of fourteen shuffles; only the sums travel
         __syncwarp();
-        jq[lane] = make_ulonglong2(nxh, nyh); jq[32 + lane] = make_ulonglong2(nzh, sj);
-        jq[64 + lane] = make_ulonglong2(nxl, nyl); jq[96 + lane] = make_ulonglong2(nzl, 0ull);
+        jq[lane] = make_ulonglong2(nxh, nyh); jq[64 + lane] = make_ulonglong2(nzh, sj);
+        jq[128 + lane] = make_ulonglong2(nxl, nyl); jq3[lane] = nzl;
+        jq[32 + lane] = make_ulonglong2(nxh, nyh); jq[96 + lane] = make_ulonglong2(nzh, sj);
+        jq[160 + lane] = make_ulonglong2(nxl, nyl); jq3[32 + lane] = nzl;
         __syncwarp();
         auto step = [&](auto masked, int s, const JRec &in, JRec &out) {
             const f2 nxh = in.xh, nyh = in.yh, nzh = in.zh, nxl = in.xl, nyl = in.yl, nzl = in.zl, sj = in.s;
             const int jidx_a = ja - lane + ((lane + s) & 31), jidx_b = jidx_a + 32;
             f2 g0 = in.g0, g1 = in.g1, g2 = in.g2, gfar = in.gf;
             {   // the records of the NEXT step first: their latency hides behind this step's arithmetic
-                const int nx = (lane + s + 1) & 31;
-                const ulonglong2 q0 = jq[nx], q1 = jq[32 + nx], q2 = jq[64 + nx], q3 = jq[96 + nx];
-                out.xh = q0.x; out.yh = q0.y; out.zh = q1.x; out.s = q1.y; out.xl = q2.x; out.yl = q2.y; out.zl = q3.x;
+                const int nx = lane + s + 1;               // <= 63: the second copy
+                const ulonglong2 q0 = jq[nx], q1 = jq[64 + nx], q2 = jq[128 + nx];
+                out.xh = q0.x; out.yh = q0.y; out.zh = q1.x; out.s = q1.y; out.xl = q2.x; out.yl = q2.y; out.zl = jq3[nx];
             }
             f2 estep = zero2;                              // sum r^-n over the 2 IT pairs of this step
 #pragma unroll
@@ -409,6 +426,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                 step(std::integral_constant<bool, true>{}, s + 1, B, A);
             }
         } else {
+#pragma unroll kN3pUnroll
             for (int s = 0; s < 32; s += 2) {
                 step(std::integral_constant<bool, false>{}, s, A, B);
                 step(std::integral_constant<bool, false>{}, s + 1, B, A);
@@ -466,9 +484,9 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3FArgs a) {
-    __shared__ double red[kN3Warps][IT][3][32];
+    __shared__ __align__(16) double buf[kN3pSmemDoubles<IT>];
     __shared__ double red_e[kN3Warps];
-    n3p_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, red, red_e);
+    n3p_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, buf, red_e);
 }
 
 // ---- finalize: self[i] + part[0 .. block(i)][i] in that order ----

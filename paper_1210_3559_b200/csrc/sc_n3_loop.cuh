@@ -23,7 +23,8 @@ namespace scmd {
 
 template <int IT, int NE, int ME, bool MIXED>
 __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopArgs a) {
-    __shared__ double red[kN3Warps][IT][3][32];
+    __shared__ __align__(16) double buf[MIXED ? kN3pSmemDoubles<IT> : kN3Warps * IT * 3 * 32];
+    double (&red)[kN3Warps][IT][3][32] = *reinterpret_cast<double (*)[kN3Warps][IT][3][32]>(buf);
     __shared__ double red_e[kN3Warps];
     unsigned long long bar_target = a.barrier_base;
     auto grid_sync = [&]() { bar_target += gridDim.x; grid_barrier(a.barrier, bar_target); };
@@ -64,7 +65,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopA
             grid_sync();
         }
         // sweep 1: density partials
-        if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, false, false>(a.sf, piece, red, red_e);
+        if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, false, false>(a.sf, piece, buf, red_e);
         else n3_sweep_piece<IT, NE, ME, false, false>(a.s, piece, red, red_e);
         grid_sync();
         f.fuse = 0;
@@ -73,10 +74,10 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopA
         grid_sync();
         // sweep 2: force partials (+ pair energy)
         if (last || a.energy_every) {
-            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, true>(a.sf, piece, red, red_e);
+            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, true>(a.sf, piece, buf, red_e);
             else n3_sweep_piece<IT, NE, ME, true, true>(a.s, piece, red, red_e);
         } else {
-            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, false>(a.sf, piece, red, red_e);
+            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, false>(a.sf, piece, buf, red_e);
             else n3_sweep_piece<IT, NE, ME, true, false>(a.s, piece, red, red_e);
         }
         grid_sync();
