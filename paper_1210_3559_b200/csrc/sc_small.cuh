@@ -158,6 +158,77 @@ __device__ __forceinline__ void small_force_term(const double4 &pi, const double
     acc[3] += pn;
 }
 
+// Lean FP64 terms (round 2; the list sweeps' form, sc_cutoff.cuh): the self term is excluded by ONE select -- the high
+// word of the MUFU seed, whose low word is 0 anyway, is replaced by 0, so that every later product is an exact 0 (r^2 = 0
+// of the self pair gives seed = inf, which the select discards before any arithmetic; 0 x 0 on the way, never 0 x inf) --
+// instead of selects on r^2 and on the result around a branch, and the terms go into their sums by fused multiply-adds.
+__device__ __forceinline__ double small_seed_or_zero(double seed, bool keep) {
+    return __hiloint2double(keep ? __double2hiint(seed) : 0, 0);
+}
+template <int ME>
+__device__ __forceinline__ void small_density_acc(const double4 &pi, const double4 &p, bool self, int m_exp, double &acc) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    if constexpr (ME > 0 && ME % 2 == 0) {
+        const double y0 = small_seed_or_zero(rcp_seed(r2), !self);
+        const double e = fma(-r2, y0, 1.0);
+        const double w = fma(y0, fma(e, e, e), y0);
+        if constexpr (ME == 6) acc = fma(w * w, w, acc);
+        else acc += ipow_c<ME / 2>(w);
+    } else {
+        const double y0 = small_seed_or_zero(rsqrt_seed(r2), !self);
+        const double tt = r2 * y0, e = fma(-tt, y0, 1.0);
+        const double y = fma(y0, e * fma(0.375, e, 0.5), y0);
+        acc += (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+    }
+}
+template <int NE, int ME, bool ENERGY>
+__device__ __forceinline__ void small_force_acc(const double4 &pi, const double4 &p, bool self, double An, int n_exp,
+                                                int m_exp, double (&acc)[4]) {
+    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double y0 = small_seed_or_zero(rsqrt_seed(r2), !self);
+    const double tt = r2 * y0, e = fma(-tt, y0, 1.0);
+    const double y = fma(y0, e * fma(0.375, e, 0.5), y0);
+    const double w = y * y;
+    const double ss = pi.w + p.w;
+    double coef;
+    if constexpr (NE == 9 && ME == 6) {
+        const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
+        coef = w4 * fma(An, y3, -ss);
+        if constexpr (ENERGY) acc[3] = fma(w4, y, acc[3]);
+    } else {
+        const double pm = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
+        const double pn = (NE > 0) ? ipow_c<(NE > 0 ? NE : 1)>(y) : ipow_rt(y, n_exp);
+        coef = w * fma(An, pn, -ss * pm);
+        if constexpr (ENERGY) acc[3] += pn;
+    }
+    acc[0] = fma(coef, dx, acc[0]);
+    acc[1] = fma(coef, dy, acc[1]);
+    acc[2] = fma(coef, dz, acc[2]);
+}
+// Sweep 2 of one thread: records q, q + JL, ... of the staged array against row i, two chains of sums (a, b).  The four
+// records of an iteration sit at pj, pj + JL, pj + 2 JL, pj + 3 JL: one pointer and three offsets kept in registers,
+// the self test compares the distance i - j with the same offsets.
+template <int NE, int ME, bool ENERGY>
+__device__ __forceinline__ void small_sweep2(const double4 *sm, int N, int i, int q, int JL, double An, int n_exp, int m_exp,
+                                             double (&acc)[4]) {
+    const double4 pi = sm[i];
+    double b[4] = {0.0, 0.0, 0.0, 0.0};                            // second chain
+    const int JL2 = 2 * JL, JL3 = 3 * JL;
+    const double4 *pj = sm + q;
+    int d = i - q, left = N - q;                                    // self iff d == offset; records left from pj on
+    for (; left > JL3; left -= 4 * JL, d -= 4 * JL, pj += 4 * JL) { // 4 independent pair terms in flight
+        small_force_acc<NE, ME, ENERGY>(pi, pj[0], d == 0, An, n_exp, m_exp, acc);
+        small_force_acc<NE, ME, ENERGY>(pi, pj[JL], d == JL, An, n_exp, m_exp, b);
+        small_force_acc<NE, ME, ENERGY>(pi, pj[JL2], d == JL2, An, n_exp, m_exp, acc);
+        small_force_acc<NE, ME, ENERGY>(pi, pj[JL3], d == JL3, An, n_exp, m_exp, b);
+    }
+    for (; left > 0; left -= JL, d -= JL, pj += JL) small_force_acc<NE, ME, ENERGY>(pi, pj[0], d == 0, An, n_exp, m_exp, acc);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc[c] += b[c];
+}
+
 // ---- mixed precision (binary32 pair arithmetic on split coordinates, binary64 accumulation) ----
 // staged record: x = xh + xl with xh = fl32(x), xl = fl32(x - xh), so that (xh_i - xh_j) + (xl_i - xl_j) keeps the
 // accuracy of a binary64 subtraction to within binary32 rounding of the DIFFERENCE (as in allpairs32_kernel)
@@ -283,14 +354,16 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
             } else if (rowlive) {
                 const double4 pi = sm[i];
                 double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;   // 4 independent chains; summed in a fixed order
-                int j = q;
-                for (; j + 3 * JL < N; j += 4 * JL) {
-                    t0 += small_density_term<ME>(pi, sm[j], j == i, m_exp);              // self term excluded by index
-                    t1 += small_density_term<ME>(pi, sm[j + JL], j + JL == i, m_exp);
-                    t2 += small_density_term<ME>(pi, sm[j + 2 * JL], j + 2 * JL == i, m_exp);
-                    t3 += small_density_term<ME>(pi, sm[j + 3 * JL], j + 3 * JL == i, m_exp);
+                const int JL2 = 2 * JL, JL3 = 3 * JL;
+                const double4 *pj = sm + q;
+                int d = i - q, left = N - q;                      // self term excluded by index: iff d == offset
+                for (; left > JL3; left -= 4 * JL, d -= 4 * JL, pj += 4 * JL) {
+                    small_density_acc<ME>(pi, pj[0], d == 0, m_exp, t0);
+                    small_density_acc<ME>(pi, pj[JL], d == JL, m_exp, t1);
+                    small_density_acc<ME>(pi, pj[JL2], d == JL2, m_exp, t2);
+                    small_density_acc<ME>(pi, pj[JL3], d == JL3, m_exp, t3);
                 }
-                for (; j < N; j += JL) t0 += small_density_term<ME>(pi, sm[j], j == i, m_exp);
+                for (; left > 0; left -= JL, d -= JL, pj += JL) small_density_acc<ME>(pi, pj[0], d == 0, m_exp, t0);
                 acc[0] = (t0 + t1) + (t2 + t3);
             }
             row_reduce<1>(acc, JL, LQ, q, warp_red);
@@ -328,22 +401,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
                     for (int c = 0; c < 4; ++c) acc[c] += double(fa[c] + fb[c]);
                 }
             } else if (rowlive) {
-                const double4 pi = sm[i];
-                double b[4] = {0.0, 0.0, 0.0, 0.0};               // second chain
-                int j = q;
-                for (; j + 3 * JL < N; j += 4 * JL) {              // 4 independent pair terms in flight
-                    small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
-                    small_force_term<NE, ME>(pi, sm[j + JL], j + JL == i, An, n_exp, m_exp, b);
-                    small_force_term<NE, ME>(pi, sm[j + 2 * JL], j + 2 * JL == i, An, n_exp, m_exp, acc);
-                    small_force_term<NE, ME>(pi, sm[j + 3 * JL], j + 3 * JL == i, An, n_exp, m_exp, b);
-                }
-                for (; j + JL < N; j += 2 * JL) {
-                    small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
-                    small_force_term<NE, ME>(pi, sm[j + JL], j + JL == i, An, n_exp, m_exp, b);
-                }
-                if (j < N) small_force_term<NE, ME>(pi, sm[j], j == i, An, n_exp, m_exp, acc);
-#pragma unroll
-                for (int c = 0; c < 4; ++c) acc[c] += b[c];
+                // the pair energy is formed on the call's last step only (block-uniform choice of the instantiation)
+                if (k == a.nsteps) small_sweep2<NE, ME, true>(sm, N, i, q, JL, An, n_exp, m_exp, acc);
+                else small_sweep2<NE, ME, false>(sm, N, i, q, JL, An, n_exp, m_exp, acc);
             }
             row_reduce<4>(acc, JL, LQ, q, warp_red);
             // ---- D: second half kick (+ Langevin), |v|^2 ----
