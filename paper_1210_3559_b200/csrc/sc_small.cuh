@@ -271,6 +271,81 @@ __device__ __forceinline__ void small_force_term_f(const SmallRecF &pi, const Sm
     acc[3] += pn;
 }
 
+// Lean binary32 terms: the self term by one select on the MUFU seed (a zero seed makes every later product an exact 0:
+// the Newton step forms 0 x 0, never 0 x inf), sums by fused multiply-adds; ENERGY as in the FP64 form
+template <int ME>
+__device__ __forceinline__ void small_density_acc_f(const SmallRecF &pi, const SmallRecF &p, bool self, int m_exp, float &acc) {
+    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if constexpr (ME > 0 && ME % 2 == 0) {
+        float y0;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(r2));
+        y0 = self ? 0.f : y0;
+        const float w = fmaf(y0, fmaf(-r2, y0, 1.0f), y0);
+        if constexpr (ME == 6) acc = fmaf(w * w, w, acc);
+        else acc += ipow_cf<ME / 2>(w);
+    } else {
+        float y0;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(r2));
+        y0 = self ? 0.f : y0;
+        const float e = fmaf(-(r2 * y0), y0, 1.0f);
+        const float y = fmaf(y0 * e, 0.5f, y0);
+        acc += (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+    }
+}
+template <int NE, int ME, bool ENERGY>
+__device__ __forceinline__ void small_force_acc_f(const SmallRecF &pi, const SmallRecF &p, bool self, float Anf, int n_exp,
+                                                  int m_exp, float (&acc)[4]) {
+    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    float y0;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y0) : "f"(r2));
+    y0 = self ? 0.f : y0;
+    const float e = fmaf(-(r2 * y0), y0, 1.0f);
+    const float y = fmaf(y0 * e, 0.5f, y0);
+    const float w = y * y;
+    const float ss = pi.s + p.s;
+    float coef;
+    if constexpr (NE == 9 && ME == 6) {
+        const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
+        coef = w4 * fmaf(Anf, y3, -ss);
+        if constexpr (ENERGY) acc[3] = fmaf(w4, y, acc[3]);
+    } else {
+        const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
+        const float pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
+        coef = w * fmaf(Anf, pn, -ss * pm);
+        if constexpr (ENERGY) acc[3] += pn;
+    }
+    acc[0] = fmaf(coef, dx, acc[0]);
+    acc[1] = fmaf(coef, dy, acc[1]);
+    acc[2] = fmaf(coef, dz, acc[2]);
+}
+// mixed sweep 2 of one thread: binary32 partial sums over <= 8 terms (two chains of four), then binary64
+template <int NE, int ME, bool ENERGY>
+__device__ __forceinline__ void small_sweep2_f(const SmallRecF *smf, int N, int i, int q, int JL, float Anf, int n_exp,
+                                               int m_exp, double (&acc)[4]) {
+    const SmallRecF pi = smf[i];
+    const SmallRecF *pj = smf + q;
+    int d = i - q, left = N - q;
+    const int JL7 = 7 * JL;
+    for (; left > JL7; left -= 8 * JL, d -= 8 * JL, pj += 8 * JL) {
+        float fa[4] = {0.f, 0.f, 0.f, 0.f}, fb[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            small_force_acc_f<NE, ME, ENERGY>(pi, pj[(2 * u) * JL], d == (2 * u) * JL, Anf, n_exp, m_exp, fa);
+            small_force_acc_f<NE, ME, ENERGY>(pi, pj[(2 * u + 1) * JL], d == (2 * u + 1) * JL, Anf, n_exp, m_exp, fb);
+        }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[c] += double(fa[c] + fb[c]);
+    }
+    if (left > 0) {                                                 // <= 7 records left
+        float fa[4] = {0.f, 0.f, 0.f, 0.f};
+        for (; left > 0; left -= JL, d -= JL, pj += JL) small_force_acc_f<NE, ME, ENERGY>(pi, pj[0], d == 0, Anf, n_exp, m_exp, fa);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[c] += double(fa[c]);
+    }
+}
+
 template <int NE, int ME, bool MIXED>
 __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const SmallStepArgs a) {
     unsigned long long bar_target = a.barrier_base;
@@ -340,16 +415,22 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
             double acc[1] = {0.0};
             if (rowlive && MIXED) {
                 const SmallRecF pi = smf[i];
-                int j = q;
-                while (j < N) {                                   // binary32 partial sums over <= 8 terms, then binary64
+                const SmallRecF *pj = smf + q;
+                int d = i - q, left = N - q;
+                const int JL7 = 7 * JL;
+                for (; left > JL7; left -= 8 * JL, d -= 8 * JL, pj += 8 * JL) {   // binary32 partial sums over 8 terms, then binary64
                     float t0 = 0.f, t1 = 0.f;
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        if (j < N) t0 += small_density_term_f<ME>(pi, smf[j], j == i, m_exp);
-                        if (j + JL < N) t1 += small_density_term_f<ME>(pi, smf[j + JL], j + JL == i, m_exp);
-                        j += 2 * JL;
+                        small_density_acc_f<ME>(pi, pj[(2 * u) * JL], d == (2 * u) * JL, m_exp, t0);
+                        small_density_acc_f<ME>(pi, pj[(2 * u + 1) * JL], d == (2 * u + 1) * JL, m_exp, t1);
                     }
                     acc[0] += double(t0 + t1);
+                }
+                if (left > 0) {
+                    float t0 = 0.f;
+                    for (; left > 0; left -= JL, d -= JL, pj += JL) small_density_acc_f<ME>(pi, pj[0], d == 0, m_exp, t0);
+                    acc[0] += double(t0);
                 }
             } else if (rowlive) {
                 const double4 pi = sm[i];
@@ -387,19 +468,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         {
             double acc[4] = {0.0, 0.0, 0.0, 0.0};
             if (rowlive && MIXED) {
-                const SmallRecF pi = smf[i];
-                int j = q;
-                while (j < N) {
-                    float fa[4] = {0.f, 0.f, 0.f, 0.f}, fb[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        if (j < N) small_force_term_f<NE, ME>(pi, smf[j], j == i, Anf, n_exp, m_exp, fa);
-                        if (j + JL < N) small_force_term_f<NE, ME>(pi, smf[j + JL], j + JL == i, Anf, n_exp, m_exp, fb);
-                        j += 2 * JL;
-                    }
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) acc[c] += double(fa[c] + fb[c]);
-                }
+                if (k == a.nsteps) small_sweep2_f<NE, ME, true>(smf, N, i, q, JL, Anf, n_exp, m_exp, acc);
+                else small_sweep2_f<NE, ME, false>(smf, N, i, q, JL, Anf, n_exp, m_exp, acc);
             } else if (rowlive) {
                 // the pair energy is formed on the call's last step only (block-uniform choice of the instantiation)
                 if (k == a.nsteps) small_sweep2<NE, ME, true>(sm, N, i, q, JL, An, n_exp, m_exp, acc);
