@@ -785,21 +785,28 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
     a.n_atoms = N;
     a.rows = ceil_div(N, c->small_ctas);
     const int grid = ceil_div(N, a.rows);
-    // rows per warp (1, 2 or 4): more rows per warp = fewer shared-memory wavefronts per pair (the 32 lanes of a
-    // load touch 32 / rpw records), at the price of padding the row count to a multiple of rpw
-    int rpw = c->opt_tpr ? 32 / c->opt_tpr : (a.rows >= 12 ? 8 : (a.rows >= 2 ? 2 : 1));   // measured: 8 rows per warp +4 % at N >= 2057
-    if (rpw > kSmallMaxRowsPerWarp) rpw = kSmallMaxRowsPerWarp;
-    if (rpw < 1) rpw = 1;
-    int jl = 1, rows_p = 0;
-    for (;; rpw /= 2) {
-        rows_p = (a.rows + rpw - 1) / rpw * rpw;
-        jl = 1;
-        while (jl * 2 * rows_p <= kSmallThreads && jl < 512) jl *= 2;
-        if (rows_p * jl <= kSmallThreads && jl * rpw >= 32) break;   // a warp must be filled by rpw rows x (32 / rpw) lanes
-        if (rpw == 1) break;
-    }
-    a.jl = jl;
-    a.lq = jl < 32 / rpw ? jl : 32 / rpw;
+    // Thread layout: a warp holds rpw = 1, 2, 4 or 8 rows (lq = 32 / rpw lanes each; more rows per warp = fewer
+    // shared-memory wavefronts per pair), a row group of rpw rows is spread over wpg warps (ANY count, not a power of two:
+    // jl = lq x wpg threads stride the j range of a row), and the groups x wpg warps share the SM's four sub-partitions.
+    // The sweeps last (warps of the busiest sub-partition) x (pairs per thread); the host takes the layout that makes
+    // that product smallest, the larger rpw on a tie.  (Round 1 took jl as a power of two: N = 1415 -- 10 rows per CTA --
+    // ran 10 warps of 44 pairs per thread, 2 - 3 per sub-partition, too few to hide the FP64 latency: sweeps of 4.0 + 4.7 us
+    // where 15 warps of 30 pairs take 2.9 + 3.6.)
+    int best_rpw = 1, best_wpg = 1;
+    double best_cost = 0.0;
+    const int forced = c->opt_tpr ? std::min(32 / c->opt_tpr, kSmallMaxRowsPerWarp) : 0;   // SC_OPT_LANES_PER_ROW
+    for (int pass = 0; pass < 2 && best_cost == 0.0; ++pass)       // second pass: the forced layout does not fit
+        for (int rpw : {8, 4, 2, 1}) {
+            if (pass == 0 && forced && rpw != forced) continue;
+            const int groups = ceil_div(a.rows, rpw), wpg = (kSmallThreads / 32) / groups;
+            if (wpg < 1) continue;
+            const int jl_c = (32 / rpw) * wpg, warps = groups * wpg;
+            const double cost = double(ceil_div(warps, 4)) * double(ceil_div(N, jl_c));
+            if (best_cost == 0.0 || cost < best_cost) { best_cost = cost; best_rpw = rpw; best_wpg = wpg; }
+        }
+    if (best_cost == 0.0) return fail(c, SC_ERR_INVALID, "one-launch step loop: no thread layout for this size%s");
+    a.lq = 32 / best_rpw;
+    a.jl = a.lq * best_wpg;
     if (32 / a.lq > kSmallMaxRowsPerWarp) return fail(c, SC_ERR_INVALID, "one-launch step loop: more than 8 rows per warp%s");
     a.nsteps = nsteps; a.hk = 0.5 * dt * kAcc / c->p.mass; a.dt = dt; a.mass = c->p.mass; a.ndof = double(3 * c->N - 3);
     a.thermo = thermo;
