@@ -57,8 +57,15 @@ struct SmallStepArgs {
     PairConsts c;
 };
 
+// Staged records in shared memory: blocks of 8 records, the 8 first halves (16 B: x, y / xh, yh, zh, s') followed by the
+// 8 second halves (z, s' / xl, yl, zl).  The lq lanes of a row read lq CONSECUTIVE records: as whole 32-byte records
+// that is a 16-byte access at a 32-byte stride -- 2 x the wavefronts, and at N = 1415 (16 lanes per row) ncu showed the
+// shared-memory pipe saturated by 1.2 M bank conflicts per step; in this layout the same access is contiguous.
+// A thread steps through records jl apart; jl is a multiple of 8, so its address advances by jl x 32 bytes.
+__host__ __device__ inline int small_rec_off(int j) { return ((j >> 3) << 8) + ((j & 7) << 4); }
+__host__ __device__ inline int small_rec_bytes(int n_atoms) { return ((n_atoms + 7) >> 3) << 8; }
 inline size_t small_step_smem_bytes(int n_atoms) {
-    return size_t(n_atoms) * sizeof(double4) + (kSmallThreads / 32) * 8 * 4 * sizeof(double) + kSmallThreads * sizeof(double);
+    return size_t(small_rec_bytes(n_atoms)) + (kSmallThreads / 32) * 8 * 4 * sizeof(double) + kSmallThreads * sizeof(double);
 }
 
 #ifdef SCMD_MAIN_TU
@@ -158,6 +165,31 @@ __device__ __forceinline__ void small_force_term(const double4 &pi, const double
     acc[3] += pn;
 }
 
+template <class Rec> __device__ __forceinline__ Rec small_load(const unsigned char *p);
+template <> __device__ __forceinline__ double4 small_load<double4>(const unsigned char *p) {
+    const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 128);
+    return make_double4(a.x, a.y, b.x, b.y);
+}
+template <> __device__ __forceinline__ RecF small_load<RecF>(const unsigned char *p) {
+    const float4 a = *reinterpret_cast<const float4 *>(p), b = *reinterpret_cast<const float4 *>(p + 128);
+    return RecF{a.x, a.y, a.z, a.w, b.x, b.y, b.z, 0.f};
+}
+__device__ __forceinline__ void small_store(unsigned char *p, const double4 &r) {
+    *reinterpret_cast<double2 *>(p) = make_double2(r.x, r.y);
+    *reinterpret_cast<double2 *>(p + 128) = make_double2(r.z, r.w);
+}
+__device__ __forceinline__ void small_store(unsigned char *p, const RecF &r) {
+    *reinterpret_cast<float4 *>(p) = make_float4(r.xh, r.yh, r.zh, r.s);
+    *reinterpret_cast<float4 *>(p + 128) = make_float4(r.xl, r.yl, r.zl, 0.f);
+}
+// a thread's cursor in the staged records: [k] is the record k places further on (k a multiple of 8)
+template <class Rec>
+struct SmallCursor {
+    const unsigned char *p;
+    __device__ __forceinline__ Rec operator[](int k) const { return small_load<Rec>(p + k * 32); }
+    __device__ __forceinline__ SmallCursor &operator+=(int k) { p += k * 32; return *this; }
+};
+
 // Lean FP64 terms (round 2; the list sweeps' form, sc_cutoff.cuh): the self term is excluded by ONE select -- the high
 // word of the MUFU seed, whose low word is 0 anyway, is replaced by 0, so that every later product is an exact 0 (r^2 = 0
 // of the self pair gives seed = inf, which the select discards before any arithmetic; 0 x 0 on the way, never 0 x inf) --
@@ -211,12 +243,12 @@ __device__ __forceinline__ void small_force_acc(const double4 &pi, const double4
 // records of an iteration sit at pj, pj + JL, pj + 2 JL, pj + 3 JL: one pointer and three offsets kept in registers,
 // the self test compares the distance i - j with the same offsets.
 template <int NE, int ME, bool ENERGY>
-__device__ __forceinline__ void small_sweep2(const double4 *sm, int N, int i, int q, int JL, double An, int n_exp, int m_exp,
+__device__ __forceinline__ void small_sweep2(const unsigned char *sm, int N, int i, int q, int JL, double An, int n_exp, int m_exp,
                                              double (&acc)[4]) {
-    const double4 pi = sm[i];
+    const double4 pi = small_load<double4>(sm + small_rec_off(i));
     double b[4] = {0.0, 0.0, 0.0, 0.0};                            // second chain
     const int JL2 = 2 * JL, JL3 = 3 * JL;
-    const double4 *pj = sm + q;
+    SmallCursor<double4> pj{sm + small_rec_off(q)};
     int d = i - q, left = N - q;                                    // self iff d == offset; records left from pj on
     for (; left > JL3; left -= 4 * JL, d -= 4 * JL, pj += 4 * JL) { // 4 independent pair terms in flight
         small_force_acc<NE, ME, ENERGY>(pi, pj[0], d == 0, An, n_exp, m_exp, acc);
@@ -322,10 +354,10 @@ __device__ __forceinline__ void small_force_acc_f(const SmallRecF &pi, const Sma
 }
 // mixed sweep 2 of one thread: binary32 partial sums over <= 8 terms (two chains of four), then binary64
 template <int NE, int ME, bool ENERGY>
-__device__ __forceinline__ void small_sweep2_f(const SmallRecF *smf, int N, int i, int q, int JL, float Anf, int n_exp,
+__device__ __forceinline__ void small_sweep2_f(const unsigned char *sm, int N, int i, int q, int JL, float Anf, int n_exp,
                                                int m_exp, double (&acc)[4]) {
-    const SmallRecF pi = smf[i];
-    const SmallRecF *pj = smf + q;
+    const SmallRecF pi = small_load<SmallRecF>(sm + small_rec_off(i));
+    SmallCursor<SmallRecF> pj{sm + small_rec_off(q)};
     int d = i - q, left = N - q;
     const int JL7 = 7 * JL;
     for (; left > JL7; left -= 8 * JL, d -= 8 * JL, pj += 8 * JL) {
@@ -352,9 +384,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
     auto grid_sync = [&]() { bar_target += gridDim.x; grid_barrier(a.barrier, bar_target); };
     extern __shared__ __align__(32) unsigned char smem_raw[];
     const int N = a.n_atoms;
-    double4 *sm = reinterpret_cast<double4 *>(smem_raw);
-    SmallRecF *smf = reinterpret_cast<SmallRecF *>(smem_raw);          // MIXED: the same bytes hold split binary32 records
-    double *warp_red = reinterpret_cast<double *>(sm + N);
+    unsigned char *sm = smem_raw;                                       // staged records (small_rec_off); MIXED: split binary32
+    double *warp_red = reinterpret_cast<double *>(smem_raw + small_rec_bytes(N));
     double *rowval = warp_red + (kSmallThreads / 32) * kSmallMaxRowsPerWarp * 4;
     __shared__ double s_lambda;
 
@@ -391,8 +422,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         __syncthreads();                                    // everyone is done with the previous contents
         for (int j = t; j < N; j += kSmallThreads) {
             const double4 p = load_record_cg(cur + j);
-            if constexpr (MIXED) smf[j] = split_record(p);
-            else sm[j] = p;
+            if constexpr (MIXED) small_store(sm + small_rec_off(j), split_record(p));
+            else small_store(sm + small_rec_off(j), p);
         }
         __syncthreads();
     };
@@ -414,8 +445,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         {
             double acc[1] = {0.0};
             if (rowlive && MIXED) {
-                const SmallRecF pi = smf[i];
-                const SmallRecF *pj = smf + q;
+                const SmallRecF pi = small_load<SmallRecF>(sm + small_rec_off(i));
+                SmallCursor<SmallRecF> pj{sm + small_rec_off(q)};
                 int d = i - q, left = N - q;
                 const int JL7 = 7 * JL;
                 for (; left > JL7; left -= 8 * JL, d -= 8 * JL, pj += 8 * JL) {   // binary32 partial sums over 8 terms, then binary64
@@ -433,10 +464,10 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
                     acc[0] += double(t0);
                 }
             } else if (rowlive) {
-                const double4 pi = sm[i];
+                const double4 pi = small_load<double4>(sm + small_rec_off(i));
                 double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;   // 4 independent chains; summed in a fixed order
                 const int JL2 = 2 * JL, JL3 = 3 * JL;
-                const double4 *pj = sm + q;
+                SmallCursor<double4> pj{sm + small_rec_off(q)};
                 int d = i - q, left = N - q;                      // self term excluded by index: iff d == offset
                 for (; left > JL3; left -= 4 * JL, d -= 4 * JL, pj += 4 * JL) {
                     small_density_acc<ME>(pi, pj[0], d == 0, m_exp, t0);
@@ -461,15 +492,15 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
 
         // ---- C: sweep 2 (positions are still staged; fetch the s' of this step) ----
         for (int j = t; j < N; j += kSmallThreads) {
-            if constexpr (MIXED) smf[j].s = float(__ldcg(a.sprime + j));
-            else sm[j].w = __ldcg(a.sprime + j);
+            if constexpr (MIXED) *reinterpret_cast<float *>(sm + small_rec_off(j) + 12) = float(__ldcg(a.sprime + j));
+            else *reinterpret_cast<double *>(sm + small_rec_off(j) + 128 + 8) = __ldcg(a.sprime + j);
         }
         __syncthreads();
         {
             double acc[4] = {0.0, 0.0, 0.0, 0.0};
             if (rowlive && MIXED) {
-                if (k == a.nsteps) small_sweep2_f<NE, ME, true>(smf, N, i, q, JL, Anf, n_exp, m_exp, acc);
-                else small_sweep2_f<NE, ME, false>(smf, N, i, q, JL, Anf, n_exp, m_exp, acc);
+                if (k == a.nsteps) small_sweep2_f<NE, ME, true>(sm, N, i, q, JL, Anf, n_exp, m_exp, acc);
+                else small_sweep2_f<NE, ME, false>(sm, N, i, q, JL, Anf, n_exp, m_exp, acc);
             } else if (rowlive) {
                 // the pair energy is formed on the call's last step only (block-uniform choice of the instantiation)
                 if (k == a.nsteps) small_sweep2<NE, ME, true>(sm, N, i, q, JL, An, n_exp, m_exp, acc);

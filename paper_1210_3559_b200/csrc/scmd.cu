@@ -798,7 +798,9 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
     for (int pass = 0; pass < 2 && best_cost == 0.0; ++pass)       // second pass: the forced layout does not fit
         for (int rpw : {8, 4, 2, 1}) {
             if (pass == 0 && forced && rpw != forced) continue;
-            const int groups = ceil_div(a.rows, rpw), wpg = (kSmallThreads / 32) / groups;
+            const int groups = ceil_div(a.rows, rpw);
+            int wpg = (kSmallThreads / 32) / groups;
+            if (rpw == 8) wpg &= ~1;                                // jl = lq x wpg must be a multiple of 8 (small_rec_off)
             if (wpg < 1) continue;
             const int jl_c = (32 / rpw) * wpg, warps = groups * wpg;
             const double cost = double(ceil_div(warps, 4)) * double(ceil_div(N, jl_c));
