@@ -42,7 +42,7 @@ UNIT = "ordered pairs/s (both sweeps)"
 # thread-level FP64-pipe instructions (FP64 path) / FMA-pipe lane operations (mixed path)
 I_DENSITY = {"fp64": 11, "mixed": 16}
 I_FORCE_ENERGY = {"fp64": 22, "mixed": 27}
-# Newton's-third-law sweeps (all pairs, default from N = 2305 up to 262144: csrc/sc_allpairs_n3.cuh): 13 / 25 FP64 instructions
+# Newton's-third-law sweeps (all pairs, default from N = 2961 up to 262144: csrc/sc_allpairs_n3.cuh): 13 / 25 FP64 instructions
 # per UNORDERED pair = 6.5 / 12.5 per ordered pair
 I_DENSITY_N3 = {"fp64": 6.5, "mixed": 10.0}      # mixed: 20 / 30 FMA-pipe lane operations per unordered pair
 I_FORCE_ENERGY_N3 = {"fp64": 12.5, "mixed": 15.0}

@@ -108,7 +108,7 @@ typedef enum {
                                      such loops exist: the one-sided one with the records staged in
                                      shared memory (N <= 6144, any thermostat), and the one through
                                      the Newton's-third-law sweeps (NVE and rescale steps, 2048 <= N <= 12288).
-                                     0: library default (the first for N <= 2304, the second for NVE and
+                                     0: library default (the first for N <= 2960, the second for NVE and
                                      rescale steps where SC_OPT_NEWTON3 applies and N <= 12288: the measured
                                      crossovers), 1: the first, 2: neither (one launch per sweep
                                      and per integrator stage), 3: never the first.  Off while
@@ -124,7 +124,7 @@ typedef enum {
     SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 2048 <= N <= 262144 (the range in which
                                      sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
-                                     both atoms.  0: library default (on from N = 2305), 1: on,
+                                     both atoms.  0: library default (on from N = 2961), 1: on,
                                      2: off = the one-sided sweeps                               */
     SC_OPT_CUTOFF_SHIFT = 11,     /* cutoff path: 0 (default) plain truncation, as BASELINE.json's
                                      configs; 1 energy-shifted terms: inside r_cut every pair term

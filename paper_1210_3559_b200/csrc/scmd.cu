@@ -176,7 +176,7 @@ int cutoff_max_dim(int64_t N) {
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
 constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
-constexpr int64_t kN3DefaultMinAtoms = 2305, kN3DefaultMinAtomsMixed = 2305;   // measured crossovers
+constexpr int64_t kN3DefaultMinAtoms = 2961, kN3DefaultMinAtomsMixed = 2961;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;     // 2 rows per lane (twice the chunks, half as long) measured in the step loop for small
                                         // clusters, where the triangle has fewer chunks than the chip has warps: N = 2057 23.4
                                         // against 24.8, N = 2304 23.3 / 24.3, N = 3072 33.2 / 30.3, N = 4096 48.9 / 38.9 us per step
@@ -753,8 +753,10 @@ sc_status copy_out(sc_ctx *c, const double *src, double *d_dst, int width) {
 // mixed: N = 2057 23 (loop) against 28 us, N = 2500 44 against 37 us
 // round 2, after the balanced plan and n3_loop_kernel (500-step NVE calls, us per step, one-launch loop of sc_small.cuh
 // against the Newton's-third-law loop): FP64 N = 2057 20.5 / 24.3, 2304 22.0 / 24.7, 2560 37.5 / 24.5, 3072 43.9 / 30.5,
-// 4096 62.2 / 39.0; mixed 2304 21.7 / 23.4, 2560 38.0 / 23.6, 3072 44.7 / 30.9
-constexpr int64_t kSmallDefaultMaxAtoms = 2304, kSmallDefaultMaxAtomsMixed = 2304;
+// 4096 62.2 / 39.0; mixed 2304 21.7 / 23.4, 2560 38.0 / 23.6, 3072 44.7 / 30.9.  After the lean terms, the conflict-free staged
+// records and the free thread layout of the one-sided loop (1000-step calls): FP64 N = 2368 18.9 / 24.6, 2560 24.7 / 25.4,
+// 2960 27.5 / 30.6, 3072 32.3 / 30.6; mixed 2368 17.8 / 23.4, 2960 25.7 / 30.4, 3552 33.5 / 31.4: up to 20 rows per CTA on 148 SMs
+constexpr int64_t kSmallDefaultMaxAtoms = 2960, kSmallDefaultMaxAtomsMixed = 2960;
 
 bool small_path_wanted(const sc_ctx *c) {
     if (c->cutoff || !c->xs_b || c->opt_persistent >= 2 || c->profile || c->split) return false;

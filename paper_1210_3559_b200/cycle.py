@@ -6,7 +6,7 @@ An n-shell Mackay icosahedron (8 shells = Ni2057) under the Langevin thermostat 
 dt = 1 fs) is heated from t_low to t_high and cooled back at `rate` K/ps; every `block` steps one line
 "T_bath  T_kin  E_pot/atom" is printed (the caloric curve; the paper reads the melting and the
 solidification temperature off its jump, ~400 K apart).  Everything runs in the CUDA kernels: one
-cooperative launch per block of steps for N <= 2304 (the library's default; possible up to 6144).  The paper's cycle is 2 x 10^6 steps.
+cooperative launch per block of steps for N <= 2960 (the library's default; possible up to 6144).  The paper's cycle is 2 x 10^6 steps.
 """
 from __future__ import annotations
 

@@ -119,7 +119,7 @@ def test_newton3_plans(scmd, oracle_ld, n_atoms, pieces, precision):
     sc.sc_set_option(scmd.SC_OPT_NEWTON3, 1)
     sc.sc_set_option(scmd.SC_OPT_NEWTON3_PIECES, pieces)
     assert sc.sc_get_option(scmd.SC_OPT_NEWTON3_PIECES) == pieces
-    assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == (2 if n_atoms <= 2304 else 1)  # sc_step at the two small sizes: one-launch loop
+    assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == (2 if n_atoms <= 2960 else 1)  # sc_step at the two small sizes: one-launch loop
     sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"))
     rho, f, e = sc.sc_density().cpu().numpy(), sc.sc_forces().cpu().numpy(), sc.sc_energy()
     tol = (RHO_TOL, FORCE_TOL, ENERGY_TOL) if precision == 0 else (2e-6, 1e-5, 1e-7)
@@ -152,7 +152,7 @@ def test_newton3_trajectory(scmd, oracle_ld):
 
 
 @pytest.mark.parametrize("precision", [0, 1])
-@pytest.mark.parametrize("n_atoms", [2305, 5003, 12288])
+@pytest.mark.parametrize("n_atoms", [2961, 5003, 12288])
 def test_newton3_step_loop(scmd, oracle_ld, n_atoms, precision):
     """n3_loop_kernel (csrc/sc_n3_loop.cuh): NVE sc_step calls through the Newton's-third-law sweeps in one cooperative
     launch.  Same device functions, same sums in the same order as the four launches per step (SC_OPT_PERSISTENT = 2),

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
     (7003, {}, {}), (7003, {}, {"SC_OPT_NEWTON3": 2}),                     # Newton's third law / one-sided, FP64
     (16391, dict(precision=1), {}), (7003, dict(precision=1), {"SC_OPT_NEWTON3": 2}),   # mixed: Newton's third law / one-sided
     (4101, {}, {}), (2051, {}, {"SC_OPT_NEWTON3": 1, "SC_OPT_PERSISTENT": 2}),   # Newton's third law: the step loop in one launch / smallest carved size, separate launches
-    (2311, {}, {}), (2311, dict(precision=1), {}),                         # ... at its default's lower end (2305), both precisions
+    (2967, {}, {}), (2967, dict(precision=1), {}),                         # ... at its default's lower end (2961), both precisions
     (4611, dict(precision=1), {}), (3001, dict(precision=1), {"SC_OPT_NEWTON3": 2}),   # mixed: Newton's third law; one-sided packed sweeps
     (12301, {}, {}),                                                       # just above the one-launch range: four launches per step
     (3001, dict(r_cut=8.0, skin=1.0), {}), (3001, dict(r_cut=8.0, skin=1.0, precision=1), {}),
