@@ -63,6 +63,24 @@ __device__ __forceinline__ double rot1(double v) {   // as a 64-bit integer: two
     return __longlong_as_double(__shfl_sync(0xffffffffu, __double_as_longlong(v), (threadIdx.x + 1) & 31));
 }
 __device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
+// The MUFU seeds of 1 / x and x^-1/2 come as a high word; the library form (sc_device.cuh) completes them with a ZERO low
+// word, one move per seed (4 of the 116 instructions of a rotation step).  Any low word will do: it perturbs the seed by
+// < 2^-20 relative, about the seed's own error, and the cubic refinement leaves (2 e0)^3 ~ 2^-57 of it.  Here the low
+// word is that of `dead`, a value the caller no longer needs (the partial sum dx^2 + dy^2), so that the seed can take
+// over its register pair and no move is issued.  Deterministic: the bits are a function of the inputs alone.
+__device__ __forceinline__ double seed_with_low_of(double seed, double dead) {
+    return __hiloint2double(__double2hiint(seed), __double2loint(dead));
+}
+__device__ __forceinline__ double rcp_fast_lo(double x, double dead) {
+    const double y0 = seed_with_low_of(rcp_seed(x), dead);
+    const double e = fma(-x, y0, 1.0);
+    return fma(y0, fma(e, e, e), y0);
+}
+__device__ __forceinline__ double rsqrt_fast_lo(double x, double dead) {
+    const double y0 = seed_with_low_of(rsqrt_seed(x), dead);
+    const double tt = x * y0, e = fma(-tt, y0, 1.0);
+    return fma(y0, e * fma(0.375, e, 0.5), y0);
+}
 
 // One CTA's piece of a sweep (the whole of allpairs_n3_kernel; a phase of n3_loop_kernel, sc_n3_loop.cuh).
 // red: per-warp row sums of the epilogue, also the chunk records during the rotation; red_e: per-warp energy sums.
@@ -140,22 +158,23 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
 #pragma unroll
             for (int k = 0; k < IT; ++k) {
                 const double dx = xi[k] - xj, dy = yi[k] - yj, dz = zi[k] - zj;
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                const double r2xy = fma(dy, dy, dx * dx);
+                const double r2 = fma(dz, dz, r2xy);
                 if constexpr (!FORCE) {
                     double term;
                     if constexpr (ME > 0 && ME % 2 == 0) {
-                        double w = rcp_fast(r2);
+                        double w = rcp_fast_lo(r2, r2xy);
                         if constexpr (decltype(masked)::value) w = jidx > irow[k] ? w : 0.0;
                         term = ipow_c<ME / 2>(w);
                     } else {
-                        double y = rsqrt_fast(r2);
+                        double y = rsqrt_fast_lo(r2, r2xy);
                         if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.0;
                         term = (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
                     }
                     f0[k] += term;
                     g0 += term;
                 } else {
-                    double y = rsqrt_fast(r2);
+                    double y = rsqrt_fast_lo(r2, r2xy);
                     if constexpr (decltype(masked)::value) y = jidx > irow[k] ? y : 0.0;
                     const double w = y * y;
                     const double ss = si[k] + sj;
