@@ -327,7 +327,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         if (irow[k] < N) p = a.xfr[irow[k]];
         else p = RecF{kFarF * float(k + 2), -kFarF * float(lane + 1), 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         xh[k] = f2_dup(p.xh); yh[k] = f2_dup(p.yh); zh[k] = f2_dup(p.zh);
-        xl[k] = f2_dup(p.xl); yl[k] = f2_dup(p.yl); zl[k] = f2_dup(p.zl); si[k] = f2_dup(p.s);
+        xl[k] = f2_dup(p.xl); yl[k] = f2_dup(p.yl); zl[k] = f2_dup(p.zl); si[k] = f2_dup(-p.s);    // s' NEGATED on both sides: -(s'_i + s'_j) is one addition
         F0[k] = F1[k] = F2[k] = 0.0;
     }
     double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
@@ -346,7 +346,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         // negated j records, (a, b) in the (low, high) halves
         f2 nxh = f2_make(-pa.xh, -pb.xh), nyh = f2_make(-pa.yh, -pb.yh), nzh = f2_make(-pa.zh, -pb.zh);
         f2 nxl = f2_make(-pa.xl, -pb.xl), nyl = f2_make(-pa.yl, -pb.yl), nzl = f2_make(-pa.zl, -pb.zl);
-        const f2 sj = f2_make(pa.s, pb.s);
+        const f2 sj = f2_make(-pa.s, -pb.s);
         f2 f0[IT], f1[IT], f2v[IT], ffar[IT];
 #pragma unroll
         for (int k = 0; k < IT; ++k) f0[k] = f1[k] = f2v[k] = ffar[k] = zero2;
@@ -409,7 +409,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                     f2 y = f2_fma(f2_mul(y0, ep), mhalf2, y0);                           // y0 - y0 e' / 2
                     if constexpr (decltype(masked)::value) y = f2_make(ka ? f2_lo(y) : 0.f, kb ? f2_hi(y) : 0.f);
                     const f2 w = f2_mul(y, y);
-                    const f2 nss = f2_fma(f2_add(si[k], sj), mone2, zero2);              // -(s'_i + s'_j)
+                    const f2 nss = f2_add(si[k], sj);                                    // -(s'_i + s'_j): both come negated
                     f2 coef, pnw;
                     if constexpr (NE == 9 && ME == 6) {
                         const f2 w2 = f2_mul(w, w), w4 = f2_mul(w2, w2), y3 = f2_mul(w, y);
@@ -422,8 +422,9 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                     }
                     if constexpr (ENERGY) estep = f2_add(estep, pnw);
                     f0[k] = f2_fma(coef, dx, f0[k]); f1[k] = f2_fma(coef, dy, f1[k]); f2v[k] = f2_fma(coef, dz, f2v[k]);
-                    const f2 ncoef = f2_mul(coef, mone2);
-                    g0 = f2_fma(ncoef, dx, g0); g1 = f2_fma(ncoef, dy, g1); g2 = f2_fma(ncoef, dz, g2);
+                    // the reaction sums collect +coef d; their sign is turned when they are stored (one packed multiply per row
+                    // and step less: binary32 pair instructions have no negated operands)
+                    g0 = f2_fma(coef, dx, g0); g1 = f2_fma(coef, dy, g1); g2 = f2_fma(coef, dz, g2);
                 }
             }
             // The pair energy leaves binary32 after EVERY step (2 IT terms): a sum that lived for a whole chunk lost
@@ -454,8 +455,8 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         const f2 g0 = A.g0, g1 = A.g1, g2 = A.g2, gfar = A.gf;             // both records are home again
         // both records are home again
         if constexpr (FORCE) {
-            if (ja < N) part[ja - row0] = make_double4(double(f2_lo(g0)), double(f2_lo(g1)), double(f2_lo(g2)), 0.0);
-            if (jb < N) part[jb - row0] = make_double4(double(f2_hi(g0)), double(f2_hi(g1)), double(f2_hi(g2)), 0.0);
+            if (ja < N) part[ja - row0] = make_double4(-double(f2_lo(g0)), -double(f2_lo(g1)), -double(f2_lo(g2)), 0.0);
+            if (jb < N) part[jb - row0] = make_double4(-double(f2_hi(g0)), -double(f2_hi(g1)), -double(f2_hi(g2)), 0.0);
         } else {
             if (ja < N) part_rho[ja - row0] = double(f2_lo(g0)) + double(f2_lo(gfar));
             if (jb < N) part_rho[jb - row0] = double(f2_hi(g0)) + double(f2_hi(gfar));
