@@ -301,6 +301,7 @@ template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piece, double *buf /* kN3pSmemDoubles<IT> */,
                                                 double (&red_e)[kN3Warps]) {
     constexpr int RB = 32 * IT;
+    constexpr bool kNeg = !FORCE && ME > 0 && ME % 2 == 0 && (ME / 2) % 2 == 1;   // sweep 1 sums -r^-m (see the term)
     double (&red)[kN3Warps][IT][3][32] = *reinterpret_cast<double (*)[kN3Warps][IT][3][32]>(buf);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
@@ -384,8 +385,11 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                 if constexpr (!FORCE) {
                     f2 term;
                     if constexpr (ME > 0 && ME % 2 == 0) {
-                        const f2 y0 = f2_make(mufu_rcp(f2_lo(r2)), mufu_rcp(f2_hi(r2)));
-                        const f2 e = f2_fma(r2, f2_mul(y0, mone2), one2);              // 1 - x y0, one rounding
+                        // seed of -x (the negation rides on the MUFU operand): e = 1 + x (-y0) in one rounding, w = -(1 / r^2),
+                        // so no packed multiply by -1 is needed; for an odd ME / 2 the term and all sums of this sweep
+                        // are then NEGATIVE (kNeg) and their sign is turned when they leave binary32
+                        const f2 y0 = f2_make(mufu_rcp(-f2_lo(r2)), mufu_rcp(-f2_hi(r2)));
+                        const f2 e = f2_fma(r2, y0, one2);
                         f2 w = f2_fma(y0, e, y0);
                         if constexpr (decltype(masked)::value) w = f2_make(ka ? f2_lo(w) : 0.f, kb ? f2_hi(w) : 0.f);
                         term = f2_ipow_c<ME / 2>(w);
@@ -399,7 +403,8 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                     // two sums per accumulator (see the header of this section), split WITHOUT selects: the part of a
                     // term below 2^-26 A^-m (r^-6 at 20 A) goes to the far sum, what exceeds it to the near sum:
                     // tf = min(term, T) is exact, tn = term - tf is 0 for a far term and one rounding for a near one
-                    const f2 tf = f2_make(fminf(f2_lo(term), kN3FarTerm), fminf(f2_hi(term), kN3FarTerm));
+                    const f2 tf = kNeg ? f2_make(fmaxf(f2_lo(term), -kN3FarTerm), fmaxf(f2_hi(term), -kN3FarTerm))
+                                       : f2_make(fminf(f2_lo(term), kN3FarTerm), fminf(f2_hi(term), kN3FarTerm));
                     const f2 tn = f2_fma(tf, mone2, term);
                     f0[k] = f2_add(f0[k], tn); ffar[k] = f2_add(ffar[k], tf);
                     g0 = f2_add(g0, tn); gfar = f2_add(gfar, tf);
@@ -458,17 +463,20 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
             if (ja < N) part[ja - row0] = make_double4(-double(f2_lo(g0)), -double(f2_lo(g1)), -double(f2_lo(g2)), 0.0);
             if (jb < N) part[jb - row0] = make_double4(-double(f2_hi(g0)), -double(f2_hi(g1)), -double(f2_hi(g2)), 0.0);
         } else {
-            if (ja < N) part_rho[ja - row0] = double(f2_lo(g0)) + double(f2_lo(gfar));
-            if (jb < N) part_rho[jb - row0] = double(f2_hi(g0)) + double(f2_hi(gfar));
+            const double sgn = kNeg ? -1.0 : 1.0;
+            if (ja < N) part_rho[ja - row0] = sgn * (double(f2_lo(g0)) + double(f2_lo(gfar)));
+            if (jb < N) part_rho[jb - row0] = sgn * (double(f2_hi(g0)) + double(f2_hi(gfar)));
         }
 #pragma unroll
         for (int k = 0; k < IT; ++k) {                     // one chunk of binary32 row sums into binary64
-            F0[k] += double(f2_lo(f0[k]) + f2_hi(f0[k]));
+            if constexpr (!FORCE && kNeg) F0[k] -= double(f2_lo(f0[k]) + f2_hi(f0[k]));
+            else F0[k] += double(f2_lo(f0[k]) + f2_hi(f0[k]));
             if constexpr (FORCE) {
                 F1[k] += double(f2_lo(f1[k]) + f2_hi(f1[k]));
                 F2[k] += double(f2_lo(f2v[k]) + f2_hi(f2v[k]));
             } else {
-                F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
+                if constexpr (kNeg) F0[k] -= double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
+                else F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
             }
         }
     }
