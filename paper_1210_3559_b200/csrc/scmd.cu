@@ -761,6 +761,7 @@ constexpr int64_t kSmallDefaultMaxAtoms = 2960, kSmallDefaultMaxAtomsMixed = 296
 bool small_path_wanted(const sc_ctx *c) {
     if (c->cutoff || !c->xs_b || c->opt_persistent >= 2 || c->profile || c->split) return false;
     if (c->N > kSmallMaxAtoms) return false;
+    if (ceil_div(c->N, c->sm_count) > (kSmallThreads / 32) * kSmallMaxRowsPerWarp) return false;   // no thread layout (a device with few SMs)
     return c->opt_persistent == 1 || c->N <= (c->precision == SC_PREC_MIXED ? kSmallDefaultMaxAtomsMixed : kSmallDefaultMaxAtoms);
 }
 
