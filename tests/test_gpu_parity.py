@@ -221,6 +221,24 @@ def test_newton3_step_loop_rescale(scmd, oracle_ld, precision):
     assert np.abs(out[0][0] - out[2][0]).max() < (1e-12 if precision == 0 else 1e-7)
 
 
+def test_step_path_queries(scmd):
+    """SC_INFO_STEP_PATH / SC_INFO_ONE_LAUNCH tell which kernels a context runs as configured (bench.py asks them
+    instead of repeating the library's thresholds)."""
+    cases = [  # (N, kwargs, options, path, one_launch)
+        (147, {}, {}, 2, 1), (2960, {}, {}, 2, 1), (2961, {}, {}, 1, 1), (12288, dict(precision=1), {}, 1, 1),
+        (12289, {}, {}, 1, 0), (5003, {}, {scmd.SC_OPT_PERSISTENT: 2}, 1, 0), (5003, {}, {scmd.SC_OPT_NEWTON3: 2}, 0, 0),
+        (5003, {}, {scmd.SC_OPT_NEWTON3_PIECES: -1}, 1, 0), (1415, {}, {scmd.SC_OPT_PERSISTENT: 2}, 0, 0),
+        (3001, dict(r_cut=8.0, skin=1.0), {}, 3, 0),
+    ]
+    for n, kw, opts, path, one in cases:
+        sc = scmd.SuttonChen(n, **kw)
+        for k, v in opts.items():
+            sc.sc_set_option(k, v)
+        assert sc.sc_get_option(scmd.SC_INFO_STEP_PATH) == path, (n, kw, opts)
+        assert sc.sc_get_option(scmd.SC_INFO_ONE_LAUNCH) == one, (n, kw, opts)
+        sc.close()
+
+
 @pytest.mark.parametrize("n_atoms", [1, 2, 3, 31, 33, 511, 512, 513, 1025])
 def test_small_and_boundary_sizes(scmd, oracle_ld, n_atoms):
     """Degenerate and tile-boundary sizes.  N = 1: rho = 0, F = 0, U = 0 (reading Q9)."""
