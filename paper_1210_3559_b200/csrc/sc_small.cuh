@@ -418,14 +418,25 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         const double4 p = load_record_cg(a.xs + i);
         px = p.x; py = p.y; pz = p.z; sp = p.w;
     }
+    // The two position buffers the steps alternate between hold the records ALREADY in the staged layout (and, MIXED,
+    // already split): staging is one bulk async copy (TMA) per CTA instead of N / 512 load-convert-store rounds per
+    // thread.  The copy runs in the async proxy and reads what other CTAs wrote through the generic proxy before the
+    // grid barrier, hence the proxy fence.
+    __shared__ uint64_t stage_bar;
+    uint32_t stage_uses = 0;
+    if (t == 0) { mbar_init(&stage_bar, 1); mbar_fence_init(); }
+    __syncthreads();
     auto stage = [&](const double4 *cur) {
         __syncthreads();                                    // everyone is done with the previous contents
-        for (int j = t; j < N; j += kSmallThreads) {
-            const double4 p = load_record_cg(cur + j);
-            if constexpr (MIXED) small_store(sm + small_rec_off(j), split_record(p));
-            else small_store(sm + small_rec_off(j), p);
+        if (t == 0) {
+            asm volatile("fence.proxy.async.global;" ::: "memory");
+            const uint32_t bytes = uint32_t(small_rec_bytes(N));
+            mbar_arrive_expect_tx(&stage_bar, bytes);
+            for (uint32_t off = 0; off < bytes; off += 32768u)
+                bulk_copy_g2s(sm + off, reinterpret_cast<const unsigned char *>(cur) + off, min(32768u, bytes - off), &stage_bar);
         }
-        __syncthreads();
+        mbar_wait(&stage_bar, stage_uses & 1u);
+        ++stage_uses;
     };
 
     for (long long k = 1; k <= a.nsteps; ++k) {
@@ -435,7 +446,9 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
             vx *= lambda; vy *= lambda; vz *= lambda;
             vx = fma(a.hk, fx, vx); vy = fma(a.hk, fy, vy); vz = fma(a.hk, fz, vz);
             px = fma(a.dt, vx, px); py = fma(a.dt, vy, py); pz = fma(a.dt, vz, pz);
-            cur[i] = make_double4(px, py, pz, sp);
+            unsigned char *dst = reinterpret_cast<unsigned char *>(cur) + small_rec_off(i);
+            if constexpr (MIXED) small_store(dst, split_record(make_double4(px, py, pz, sp)));
+            else small_store(dst, make_double4(px, py, pz, sp));
         }
         lambda = 1.0;
         grid_sync();
@@ -560,10 +573,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_step_kernel(const Smal
         a.vel[3 * size_t(i)] = vx * lambda; a.vel[3 * size_t(i) + 1] = vy * lambda; a.vel[3 * size_t(i) + 2] = vz * lambda;
         a.force[3 * size_t(i)] = fx; a.force[3 * size_t(i) + 1] = fy; a.force[3 * size_t(i) + 2] = fz;
         a.rho[i] = my_rho;
-        a.xs[i] = make_double4(px, py, pz, sp);             // after the last barrier: nobody stages any more
+        a.xs[i] = make_double4(px, py, pz, sp);             // after the last barrier: nobody stages any more (back to the plain layout)
         if (a.xf) store_split_record(a.xf, i, px, py, pz, float(sp));
         if (a.xfr) a.xfr[i] = split_record(make_double4(px, py, pz, sp));
     }
+    // the staged layout spilled into the up to 7 padding records behind record N - 1 of xs: zero again, as sc_create left them
+    if (blockIdx.x == 0 && t < 8 && N + t < ((N + 7) & ~7)) a.xs[N + t] = make_double4(0.0, 0.0, 0.0, 0.0);
     if (t == 0) { a.part_emb[blockIdx.x] = e_emb; a.part_pair[blockIdx.x] = e_pair; }
     grid_sync();
     if (blockIdx.x == 0 && t < 32) {

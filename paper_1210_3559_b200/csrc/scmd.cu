@@ -212,7 +212,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         c->rdf_counts = rc; c->rdf_refs = rr; c->rdf_meta = rm; c->msd_part = mp; c->msd_meta = mm;
     }
     if (!(prm->r_cut > 0.0) && N <= kSmallMaxAtoms && !row_split(opt)) {
-        double4 *xb = w.take<double4>(n);
+        double4 *xb = w.take<double4>(n + 8);                  // staged layout: whole blocks of 8 records (sc_small.cuh)
         double *spr = w.take<double>(n);
         unsigned long long *bar = w.take<unsigned long long>(2);
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
