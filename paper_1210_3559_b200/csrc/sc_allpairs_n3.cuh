@@ -82,14 +82,27 @@ __device__ __forceinline__ double rsqrt_fast_lo(double x, double dead) {
     return fma(y0, e * fma(0.375, e, 0.5), y0);
 }
 
+// Row blocks come in PAIRS (late round 2): a tile is a run of chunks of a pair block of 2 RB rows.  Warps 0 .. NW/2 - 1 hold
+// the first RB rows in registers (set A), warps NW/2 .. NW - 1 the second RB rows (set B); warp p of A and warp p of B
+// rotate the SAME chunk, each against its own rows, B hands its reaction sums to A through shared memory (two named
+// barriers of 64 threads per chunk) and A stores ONE partial record per (pair block, j): N^2 / 512 records instead of
+// N^2 / 256 -- half the workspace (4.3 GB at N = 262144), half the DRAM writes of sweep 2 (241 MB at N = 65536) and half
+// the reads of the finalize.  Set B has no pairs in the first IT chunks of the pair block (they are below its diagonal).
+__device__ __forceinline__ void n3_pair_barrier(int pair) {
+    asm volatile("bar.sync %0, 64;" ::"r"(pair + 1) : "memory");
+}
+constexpr int kN3SlotBytes = 3 * 32 * 8;              // reaction sums of one warp's chunk on their way from set B to set A
+
 // One CTA's piece of a sweep (the whole of allpairs_n3_kernel; a phase of n3_loop_kernel, sc_n3_loop.cuh).
 // red: per-warp row sums of the epilogue, also the chunk records during the rotation; red_e: per-warp energy sums.
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece, double (&red)[kN3Warps][IT][3][32],
-                                               double (&red_e)[kN3Warps]) {
+                                               double (&red_e)[kN3Warps], unsigned char *slots /* kN3Warps / 2 x kN3SlotBytes */) {
     constexpr int RB = 32 * IT;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;                          // 12, or 6 (two CTAs per SM: finer tiles for mid-size clusters)
+    const int H = NW >> 1, set = warp >= H ? 1 : 0, wp = warp - set * H;   // row set (A: 0, B: 1), index of the warp pair
+    double *slot = reinterpret_cast<double *>(slots + wp * kN3SlotBytes);
     const int N = a.n_atoms;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
@@ -97,7 +110,8 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
     const int t_end = a.piece_start[piece + 1];
     for (int t = a.piece_start[piece]; t < t_end; ++t) {
     const N3Tile tile = a.tiles[t];
-    const int row0 = tile.b * RB;
+    const int row0p = tile.b * 2 * RB;                       // first row of the pair block
+    const int row0 = row0p + set * RB;                       // ... and of this warp's row set
 
     int irow[IT];
     double xi[IT], yi[IT], zi[IT], si[IT];
@@ -114,10 +128,10 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
         f0[k] = f1[k] = f2[k] = 0.0;
     }
 
-    const int cb = row0 >> 5;
+    const int cb = row0 >> 5, cbB = (row0p >> 5) + IT;        // first chunk of this set's rows; of set B's rows
     const int c_begin = tile.c_begin, c_end = tile.c_end;
-    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
-    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, RB);
+    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, 2 * RB);
+    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, 2 * RB);
     // The 32 records of a chunk do not change while the warp rotates it: they sit in shared memory (1 KB per warp, in the
     // space the epilogue's reduction uses afterwards; (x, y) and (z, s') as two 16-byte arrays: conflict-free), and at
     // step s a lane READS the record of lane + s -- two LDS.128 instead of eight shuffles and the moves that go with
@@ -126,8 +140,11 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
     // unrolled the address is one register plus an immediate (3 integer instructions per step less).
     static_assert(IT >= 3, "2 KB of chunk records per warp must fit into the warp's part of red");
     double2 *jxy = reinterpret_cast<double2 *>(&red[0][0][0][0]) + warp * 128, *jzs = jxy + 64;
-    for (int c = c_begin + warp; c < c_end; c += NW) {
+    for (int c = c_begin + wp; c < c_end; c += H) {
         const int jidx = (c << 5) + lane;
+        const bool both = c >= cbB;                        // set B has pairs in this chunk (the same for the two warps)
+        double g0 = 0.0, g1 = 0.0, g2 = 0.0;
+        if (set == 0 || both) {
         double xj, yj, zj, sj;
         if (jidx < N) {
             const double4 p = a.xs[jidx];
@@ -135,7 +152,6 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
         } else {
             xj = -kN3Far * double(lane + 1); yj = kN3Far; zj = kN3Far; sj = 0.0;
         }
-        const int jhome = jidx;
         const bool diag = c < cb + IT;                     // warp-uniform
         // One rotation step: evaluate the IT rows against the record held (`in`), hand it on with the reaction sums
         // accumulated on it so far (`out`).  Two register sets alternate (A -> B, B -> A): no value is ever moved back
@@ -212,11 +228,23 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
                 step(std::integral_constant<bool, false>{}, s + 1, B, A);
             }
         }
-        const double g0 = A.g0, g1 = A.g1, g2 = A.g2;
-        // the record is home again (32 rotations by one lane)
-        if (jhome < N) {
-            if constexpr (FORCE) part[jhome - row0] = make_double4(g0, g1, g2, 0.0);
-            else part_rho[jhome - row0] = g0;
+        g0 = A.g0; g1 = A.g1; g2 = A.g2;                   // the record is home again (32 rotations by one lane)
+        }
+        if (both) {                                        // set B -> set A: reaction sums of the second RB rows
+            n3_pair_barrier(wp);                           // A has read the slot of the previous chunk
+            if (set) {
+                slot[lane] = g0;
+                if constexpr (FORCE) { slot[32 + lane] = g1; slot[64 + lane] = g2; }
+            }
+            n3_pair_barrier(wp);
+            if (!set) {
+                g0 += slot[lane];
+                if constexpr (FORCE) { g1 += slot[32 + lane]; g2 += slot[64 + lane]; }
+            }
+        }
+        if (!set && jidx < N) {
+            if constexpr (FORCE) part[jidx - row0p] = make_double4(g0, g1, g2, 0.0);
+            else part_rho[jidx - row0p] = g0;
         }
     }
 
@@ -228,10 +256,10 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
         if constexpr (FORCE) { red[warp][k][1][lane] = f1[k]; red[warp][k][2][lane] = f2[k]; }
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < RB; r += NW * 32) {
-        const int k = r >> 5, l = r & 31, i = row0 + r;
+    for (int r = threadIdx.x; r < 2 * RB; r += NW * 32) {
+        const int rs = r >= RB ? 1 : 0, k = (r - rs * RB) >> 5, l = r & 31, i = row0p + r;
         double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        for (int w = 0; w < NW; ++w) {
+        for (int w = rs * H; w < rs * H + H; ++w) {       // the warps that hold this row's set
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
@@ -255,7 +283,8 @@ template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3Args a) {
     __shared__ double red[kN3Warps][IT][3][32];
     __shared__ double red_e[kN3Warps];
-    n3_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, red, red_e);
+    __shared__ __align__(16) unsigned char slots[(kN3Warps / 2) * kN3SlotBytes];
+    n3_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, red, red_e, slots);
 }
 
 // ---- mixed precision: the same rotation in binary32 on split records (x = xh + xl, RecF), binary64 accumulation ----
@@ -299,12 +328,14 @@ constexpr int kN3pUnroll = SCMD_N3P_UNROLL;
 
 template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piece, double *buf /* kN3pSmemDoubles<IT> */,
-                                                double (&red_e)[kN3Warps]) {
+                                                double (&red_e)[kN3Warps], unsigned char *slots) {
     constexpr int RB = 32 * IT;
     constexpr bool kNeg = !FORCE && ME > 0 && ME % 2 == 0 && (ME / 2) % 2 == 1;   // sweep 1 sums -r^-m (see the term)
     double (&red)[kN3Warps][IT][3][32] = *reinterpret_cast<double (*)[kN3Warps][IT][3][32]>(buf);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
+    const int H = NW >> 1, set = warp >= H ? 1 : 0, wp = warp - set * H;   // as in n3_sweep_piece
+    f2 *slot = reinterpret_cast<f2 *>(slots + wp * kN3SlotBytes);
     const int N = a.n_atoms;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const f2 An2 = f2_dup(float(a.c.An));
@@ -314,8 +345,8 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
     const int t_end = a.piece_start[piece + 1];
     for (int t = a.piece_start[piece]; t < t_end; ++t) {
     const N3Tile tile = a.tiles[t];
-    const int row0 = tile.b * RB;
-    const int cb = row0 >> 6;
+    const int row0p = tile.b * 2 * RB, row0 = row0p + set * RB;
+    const int cb = row0 >> 6, cbB = (row0p >> 6) + IT / 2;
     const int c_begin = tile.c_begin, c_end = tile.c_end;   // chunks of 64 atoms
 
     int irow[IT];
@@ -331,8 +362,8 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         xl[k] = f2_dup(p.xl); yl[k] = f2_dup(p.yl); zl[k] = f2_dup(p.zl); si[k] = f2_dup(-p.s);    // s' NEGATED on both sides: -(s'_i + s'_j) is one addition
         F0[k] = F1[k] = F2[k] = 0.0;
     }
-    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, RB);
-    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, RB);
+    double4 *part = a.part + n3_part_offset(tile.b, a.n_pad, 2 * RB);
+    double *part_rho = a.part_rho + n3_part_offset(tile.b, a.n_pad, 2 * RB);
     // chunk records of this warp, every record at lane AND lane + 32 so that the index lane + s + 1 never wraps (as in the
     // FP64 kernel): three arrays of 64 x 16 B -- (xh, yh), (zh, s'), (xl, yl) -- and one of 64 x 8 B (zl)
     ulonglong2 *jq = reinterpret_cast<ulonglong2 *>(reinterpret_cast<unsigned char *>(buf) + warp * kN3pWarpBytes);
@@ -341,8 +372,11 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         if (j < N) return a.xfr[j];
         return RecF{-kFarF * float((j & 63) + 1), kFarF, kFarF, 0.f, 0.f, 0.f, 0.f, 0.f};
     };
-    for (int c = c_begin + warp; c < c_end; c += NW) {
+    for (int c = c_begin + wp; c < c_end; c += H) {
         const int ja = (c << 6) + lane, jb = ja + 32;
+        const bool both = c >= cbB;
+        f2 g0 = zero2, g1 = zero2, g2 = zero2, gfar = zero2;
+        if (set == 0 || both) {
         const RecF pa = fetch(ja), pb = fetch(jb);
         // negated j records, (a, b) in the (low, high) halves
         f2 nxh = f2_make(-pa.xh, -pb.xh), nyh = f2_make(-pa.yh, -pb.yh), nzh = f2_make(-pa.zh, -pb.zh);
@@ -457,16 +491,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                 step(std::integral_constant<bool, false>{}, s + 1, B, A);
             }
         }
-        const f2 g0 = A.g0, g1 = A.g1, g2 = A.g2, gfar = A.gf;             // both records are home again
-        // both records are home again
-        if constexpr (FORCE) {
-            if (ja < N) part[ja - row0] = make_double4(-double(f2_lo(g0)), -double(f2_lo(g1)), -double(f2_lo(g2)), 0.0);
-            if (jb < N) part[jb - row0] = make_double4(-double(f2_hi(g0)), -double(f2_hi(g1)), -double(f2_hi(g2)), 0.0);
-        } else {
-            const double sgn = kNeg ? -1.0 : 1.0;
-            if (ja < N) part_rho[ja - row0] = sgn * (double(f2_lo(g0)) + double(f2_lo(gfar)));
-            if (jb < N) part_rho[jb - row0] = sgn * (double(f2_hi(g0)) + double(f2_hi(gfar)));
-        }
+        g0 = A.g0; g1 = A.g1; g2 = A.g2; gfar = A.gf;      // both records are home again
 #pragma unroll
         for (int k = 0; k < IT; ++k) {                     // one chunk of binary32 row sums into binary64
             if constexpr (!FORCE && kNeg) F0[k] -= double(f2_lo(f0[k]) + f2_hi(f0[k]));
@@ -479,6 +504,26 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
                 else F0[k] += double(f2_lo(ffar[k]) + f2_hi(ffar[k]));
             }
         }
+        }   // this set has pairs in the chunk
+        f2 b0 = zero2, b1 = zero2, b2 = zero2;             // set B's sums (binary32, as they travelled)
+        if (both) {
+            n3_pair_barrier(wp);
+            if (set) { slot[lane] = g0; slot[32 + lane] = FORCE ? g1 : gfar; if constexpr (FORCE) slot[64 + lane] = g2; }
+            n3_pair_barrier(wp);
+            if (!set) { b0 = slot[lane]; b1 = slot[32 + lane]; if constexpr (FORCE) b2 = slot[64 + lane]; }
+        }
+        if (!set) {
+            if constexpr (FORCE) {
+                if (ja < N) part[ja - row0p] = make_double4(-(double(f2_lo(g0)) + double(f2_lo(b0))), -(double(f2_lo(g1)) + double(f2_lo(b1))),
+                                                            -(double(f2_lo(g2)) + double(f2_lo(b2))), 0.0);
+                if (jb < N) part[jb - row0p] = make_double4(-(double(f2_hi(g0)) + double(f2_hi(b0))), -(double(f2_hi(g1)) + double(f2_hi(b1))),
+                                                            -(double(f2_hi(g2)) + double(f2_hi(b2))), 0.0);
+            } else {
+                const double sgn = kNeg ? -1.0 : 1.0;
+                if (ja < N) part_rho[ja - row0p] = sgn * ((double(f2_lo(g0)) + double(f2_lo(gfar))) + (double(f2_lo(b0)) + double(f2_lo(b1))));
+                if (jb < N) part_rho[jb - row0p] = sgn * ((double(f2_hi(g0)) + double(f2_hi(gfar))) + (double(f2_hi(b0)) + double(f2_hi(b1))));
+            }
+        }
     }
     __syncthreads();                                       // every warp is done with its chunk records (same memory)
 #pragma unroll
@@ -487,10 +532,10 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         if constexpr (FORCE) { red[warp][k][1][lane] = F1[k]; red[warp][k][2][lane] = F2[k]; }
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < RB; r += NW * 32) {
-        const int k = r >> 5, l = r & 31, i = row0 + r;
+    for (int r = threadIdx.x; r < 2 * RB; r += NW * 32) {
+        const int rs = r >= RB ? 1 : 0, k = (r - rs * RB) >> 5, l = r & 31, i = row0p + r;
         double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        for (int w = 0; w < NW; ++w) {
+        for (int w = rs * H; w < rs * H + H; ++w) {       // the warps that hold this row's set
             v0 += red[w][k][0][l];
             if constexpr (FORCE) { v1 += red[w][k][1][l]; v2 += red[w][k][2][l]; }
         }
@@ -514,7 +559,8 @@ template <int IT, int NE, int ME, bool FORCE, bool ENERGY>
 __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3p_kernel(const N3FArgs a) {
     __shared__ __align__(16) double buf[kN3pSmemDoubles<IT>];
     __shared__ double red_e[kN3Warps];
-    n3p_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, buf, red_e);
+    __shared__ __align__(16) unsigned char slots[(kN3Warps / 2) * kN3SlotBytes];
+    n3p_sweep_piece<IT, NE, ME, FORCE, ENERGY>(a, blockIdx.x, buf, red_e, slots);
 }
 
 // ---- finalize: self[i] + part[0 .. block(i)][i] in that order ----

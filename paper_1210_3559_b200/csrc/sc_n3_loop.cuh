@@ -26,6 +26,7 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopA
     __shared__ __align__(16) double buf[MIXED ? kN3pSmemDoubles<IT> : kN3Warps * IT * 3 * 32];
     double (&red)[kN3Warps][IT][3][32] = *reinterpret_cast<double (*)[kN3Warps][IT][3][32]>(buf);
     __shared__ double red_e[kN3Warps];
+    __shared__ __align__(16) unsigned char slots[(kN3Warps / 2) * kN3SlotBytes];
     unsigned long long bar_target = a.barrier_base;
     auto grid_sync = [&]() { bar_target += gridDim.x; grid_barrier(a.barrier, bar_target); };
     constexpr int GB = 4;                                   // groups of 32 atoms a finalize phase handles at once
@@ -65,8 +66,8 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopA
             grid_sync();
         }
         // sweep 1: density partials
-        if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, false, false>(a.sf, piece, buf, red_e);
-        else n3_sweep_piece<IT, NE, ME, false, false>(a.s, piece, red, red_e);
+        if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, false, false>(a.sf, piece, buf, red_e, slots);
+        else n3_sweep_piece<IT, NE, ME, false, false>(a.s, piece, red, red_e, slots);
         grid_sync();
         f.fuse = 0;
         for (int g = piece; g < ngroups; g += GB * gridDim.x)
@@ -74,11 +75,11 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) n3_loop_kernel(const N3LoopA
         grid_sync();
         // sweep 2: force partials (+ pair energy)
         if (last || a.energy_every) {
-            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, true>(a.sf, piece, buf, red_e);
-            else n3_sweep_piece<IT, NE, ME, true, true>(a.s, piece, red, red_e);
+            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, true>(a.sf, piece, buf, red_e, slots);
+            else n3_sweep_piece<IT, NE, ME, true, true>(a.s, piece, red, red_e, slots);
         } else {
-            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, false>(a.sf, piece, buf, red_e);
-            else n3_sweep_piece<IT, NE, ME, true, false>(a.s, piece, red, red_e);
+            if constexpr (MIXED) n3p_sweep_piece<IT, NE, ME, true, false>(a.sf, piece, buf, red_e, slots);
+            else n3_sweep_piece<IT, NE, ME, true, false>(a.s, piece, red, red_e, slots);
         }
         grid_sync();
         f.fuse = (last || a.thermo == 1) ? 1 : 2;

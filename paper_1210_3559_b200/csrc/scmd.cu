@@ -180,6 +180,7 @@ constexpr int64_t kN3DefaultMinAtoms = 2961, kN3DefaultMinAtomsMixed = 2961;   /
 constexpr int kN3RowsPerThread = 4;     // 2 rows per lane (twice the chunks, half as long) measured in the step loop for small
                                         // clusters, where the triangle has fewer chunks than the chip has warps: N = 2057 23.4
                                         // against 24.8, N = 2304 23.3 / 24.3, N = 3072 33.2 / 30.3, N = 4096 48.9 / 38.9 us per step
+constexpr int kN3PairRows = 64 * kN3RowsPerThread;             // rows of a pair block (two row sets per CTA: sc_allpairs_n3.cuh)
 constexpr int kN3MaxSegments = 25;                             // j segments (tiles) of the longest row block
 constexpr int kN3MaxPieces = 4096;                             // CTAs of a balanced plan (16 per SM on 256 SMs)
 inline size_t n3_tile_capacity(int64_t N) {                    // the round-1 grid has up to 25 tiles per row block
@@ -218,7 +219,7 @@ size_t carve(sc_ctx *c, void *base, int64_t N, const sc_params *prm, int32_t pre
         if (c && base) { c->xs_b = xb; c->sprime = spr; c->small_barrier = bar; }
     }
     if (!(prm->r_cut > 0.0) && N >= kN3MinAtoms && N <= kN3MaxAtoms && !(opt && opt->newton3_storage == 2) && !row_split(opt)) {
-        double4 *np = w.take<double4>(n3_part_records(int(N), 32 * kN3RowsPerThread));
+        double4 *np = w.take<double4>(n3_part_records(int(N), kN3PairRows));
         double4 *ns = w.take<double4>((n + 32) * kN3MaxSegments);
         RecF *xr = precision == SC_PREC_MIXED ? w.take<RecF>(n + 1) : nullptr;    // split records of the mixed variant
         N3Tile *tl = w.take<N3Tile>(n3_tile_capacity(N));
@@ -504,10 +505,10 @@ int choose_n3_segment(const sc_ctx *c, int *warps_out) {
 // Balanced plan (the default).  The triangle, row block after row block, is cut into P = SMs x k pieces of equal COST,
 // one CTA each; k = 1 (one wave of resident CTAs: nothing is left to the order in which SMs fall free; measured against
 // k = 2 / 4 / 8 per SM, SC_OPT_NEWTON3_PIECES: N = 8000 103.7 / 110.1 us per step, N = 65536 5158 / 5157 / 5161 / 5180).
-// Cost of a tile of L chunks: ceil(L / 4) -- the CTA's 12 warps take the
-// chunks round-robin, warps w, w + 4, w + 8 share one SM sub-partition and its issue slot, so the tile lasts as long as
-// the ceil(L / 4) chunks of its busiest sub-partition -- plus a fixed 0.15 for the tile's row loads and its reduction
-// (two CTA barriers).  The smallest cost bound T for which the greedy cut (fill a piece up to T, never with a sliver
+// Cost of a tile of L chunks of a PAIR block (2 x 128 rows, sc_allpairs_n3.cuh): ceil(L / 2) -- a chunk occupies two warps,
+// one per row set; the six warp pairs take the chunks round-robin and land three to an SM sub-partition, so the tile lasts
+// as long as the ceil(L / 2) chunk rotations of its busiest sub-partition (before the pair blocks: ceil(L / 4) for
+// 12 warps on 128 rows) -- plus a fixed 0.15 for the tile's row loads and its reduction (two CTA barriers).  The smallest cost bound T for which the greedy cut (fill a piece up to T, never with a sliver
 // shorter than 4 chunks unless it ends the row block) needs <= P pieces is found by bisection.  N = 8000: 7938 chunks
 // on 148 SMs = 13.4 per sub-partition, the plan gives every CTA <= 14; the round-1 grid gave the longest 18 (6 rounds x
 // 3 warps) and the sweep lasted 78 us where 14 / 18 of that is 61 -- measured 61.2 (300-step calls, us per step, grid
@@ -534,7 +535,7 @@ bool n3_cut(int nb, int nch, int cpb, double T, double fixed, int max_pieces, N3
         while (cpos < nch) {
             const int rest = nch - cpos;
             const double room = T - cur - fixed;
-            int fit = room >= 1.0 ? 4 * int(room + 1e-9) : 0;
+            int fit = room >= 1.0 ? 2 * int(room + 1e-9) : 0;
             if (fit < rest && fit < 4) fit = 0;
             if (fit <= 0) {
                 if (cur == 0.0) return false;                  // T below one tile's cost
@@ -544,7 +545,7 @@ bool n3_cut(int nb, int nch, int cpb, double T, double fixed, int max_pieces, N3
             const int len = std::min(fit, rest);
             if (slot >= kN3MaxSegments) return false;
             out->tiles.push_back(N3Tile{b, cpos, cpos + len, slot++});
-            cur += fixed + double(ceil_div(len, 4));
+            cur += fixed + double(ceil_div(len, 2));
             cpos += len;
         }
         out->blk_slots[size_t(b)] = slot;
@@ -556,7 +557,7 @@ bool n3_cut(int nb, int nch, int cpb, double T, double fixed, int max_pieces, N3
 int choose_n3_segment(const sc_ctx *c, int *warps_out);
 
 sc_status plan_n3(sc_ctx *c) {
-    const int N = int(c->N), rb = 32 * kN3RowsPerThread, nb = ceil_div(N, rb);
+    const int N = int(c->N), rb = kN3PairRows, nb = ceil_div(N, rb);   // pair blocks
     const bool mixed = c->precision == SC_PREC_MIXED;
     const int chunk = mixed ? 64 : 32, nch = ceil_div(N, chunk), cpb = rb / chunk;
     N3Plan plan;
@@ -579,7 +580,7 @@ sc_status plan_n3(sc_ctx *c) {
         const int P = std::min(std::min(kN3MaxPieces, N / 2), c->sm_count * (kN3Warps / c->n3_warps) * per_sm);   // part_b holds N + 1
         const double fixed = 0.15;
         double total = 0.0;
-        for (int b = 0; b < nb; ++b) total += fixed + double(ceil_div(nch - b * cpb, 4));
+        for (int b = 0; b < nb; ++b) total += fixed + double(ceil_div(nch - b * cpb, 2));
         double lo = 1.0, hi = total + 2.0;                          // hi: everything in one piece, always feasible
         N3Plan trial;
         for (int it = 0; it < 48; ++it) {
@@ -603,7 +604,7 @@ sc_status plan_n3(sc_ctx *c) {
 // all pairs, every unordered pair once (sc_allpairs_n3.cuh): sweep + finalize + scalar reduction
 sc_status run_sweep_n3(sc_ctx *c, bool force, bool energy) {
     const bool fast = (c->p.n == 9 && c->p.m == 6);
-    const int it = kN3RowsPerThread, rb = 32 * it, N = int(c->N);   // measured: 2 rows per thread lose 10 % at N = 65536
+    const int it = kN3RowsPerThread, rb = kN3PairRows, N = int(c->N);   // measured: 2 rows per thread lose 10 % at N = 65536
     const void *fn = allpairs_n3_fn(it, fast, force, energy);
     const int nb = ceil_div(N, rb);
     const bool mixed = c->precision == SC_PREC_MIXED;
@@ -853,7 +854,7 @@ bool n3_loop_wanted(const sc_ctx *c, int thermo) {
 // positions already carry the first half kick + drift of the call's first step (kick_drift_kernel)
 sc_status run_n3_loop(sc_ctx *c, double dt, const sc_thermostat *th, int thermo, int64_t nsteps) {
     const bool fast = (c->p.n == 9 && c->p.m == 6), mixed = c->precision == SC_PREC_MIXED;
-    const int N = int(c->N), rb = 32 * kN3RowsPerThread;
+    const int N = int(c->N), rb = kN3PairRows;
     if (!c->n3_seg) {
         sc_status st = plan_n3(c);
         if (st != SC_OK) return st;
