@@ -88,9 +88,18 @@ __device__ __forceinline__ double rsqrt_fast_lo(double x, double dead) {
 // barriers of 64 threads per chunk) and A stores ONE partial record per (pair block, j): N^2 / 512 records instead of
 // N^2 / 256 -- half the workspace (4.3 GB at N = 262144), half the DRAM writes of sweep 2 (241 MB at N = 65536) and half
 // the reads of the finalize.  Set B has no pairs in the first IT chunks of the pair block (they are below its diagonal).
-__device__ __forceinline__ void n3_pair_barrier(int pair) {
-    asm volatile("bar.sync %0, 64;" ::"r"(pair + 1) : "memory");
+// The hand-over is a producer / consumer pair of named barriers per warp pair (PTX bar.arrive / bar.sync, 64 threads):
+// FULL -- B arrives after writing a slot, A waits before reading it; EMPTY -- A arrives after reading, B waits before it
+// writes the slot again.  Neither warp waits for the other in step: B may finish the next chunk's rotation before A has
+// read this one, A waits only when B is behind.  ONE slot per pair: a barrier counts threads, not roles, so with two slots
+// A could arrive twice at EMPTY before B waits once and complete it alone (tried: deadlock).  (One symmetric bar.sync per chunk cost the density sweep 1.5 %: the two warps stalled together.)
+__device__ __forceinline__ void n3_full_arrive(int pair) {
+    __threadfence_block();
+    asm volatile("bar.arrive %0, 64;" ::"r"(2 * pair + 1) : "memory");
 }
+__device__ __forceinline__ void n3_full_wait(int pair) { asm volatile("bar.sync %0, 64;" ::"r"(2 * pair + 1) : "memory"); }
+__device__ __forceinline__ void n3_empty_arrive(int pair) { asm volatile("bar.arrive %0, 64;" ::"r"(2 * pair + 2) : "memory"); }
+__device__ __forceinline__ void n3_empty_wait(int pair) { asm volatile("bar.sync %0, 64;" ::"r"(2 * pair + 2) : "memory"); }
 constexpr int kN3SlotBytes = 3 * 32 * 8;              // reaction sums of one warp's chunk on their way from set B to set A
 
 // One CTA's piece of a sweep (the whole of allpairs_n3_kernel; a phase of n3_loop_kernel, sc_n3_loop.cuh).
@@ -103,6 +112,7 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
     const int NW = blockDim.x >> 5;                          // 12, or 6 (two CTAs per SM: finer tiles for mid-size clusters)
     const int H = NW >> 1, set = warp >= H ? 1 : 0, wp = warp - set * H;   // row set (A: 0, B: 1), index of the warp pair
     double *slot = reinterpret_cast<double *>(slots + wp * kN3SlotBytes);
+    int nx = 0;                                              // exchanges so far (the same count in both warps of the pair)
     const int N = a.n_atoms;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const double An = a.c.An;
@@ -231,16 +241,18 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
         g0 = A.g0; g1 = A.g1; g2 = A.g2;                   // the record is home again (32 rotations by one lane)
         }
         if (both) {                                        // set B -> set A: reaction sums of the second RB rows
-            n3_pair_barrier(wp);                           // A has read the slot of the previous chunk
             if (set) {
+                if (nx >= 1) n3_empty_wait(wp);            // A has read the slot's previous contents
                 slot[lane] = g0;
                 if constexpr (FORCE) { slot[32 + lane] = g1; slot[64 + lane] = g2; }
-            }
-            n3_pair_barrier(wp);
-            if (!set) {
+                n3_full_arrive(wp);
+            } else {
+                n3_full_wait(wp);
                 g0 += slot[lane];
                 if constexpr (FORCE) { g1 += slot[32 + lane]; g2 += slot[64 + lane]; }
+                n3_empty_arrive(wp);
             }
+            ++nx;
         }
         if (!set && jidx < N) {
             if constexpr (FORCE) part[jidx - row0p] = make_double4(g0, g1, g2, 0.0);
@@ -267,6 +279,7 @@ __device__ __forceinline__ void n3_sweep_piece(const N3Args &a, const int piece,
     }
     __syncthreads();                                       // the next tile's chunk records go into the same memory
     }   // tiles of this CTA's piece
+    if (set && nx >= 1) n3_empty_wait(wp);                 // absorb A's last arrival: the barriers are clean for the next sweep
     if constexpr (FORCE && ENERGY) {
         esum = warp_sum(esum);                             // over all tiles of the piece
         if (lane == 0) red_e[warp] = esum;
@@ -335,7 +348,8 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int NW = blockDim.x >> 5;
     const int H = NW >> 1, set = warp >= H ? 1 : 0, wp = warp - set * H;   // as in n3_sweep_piece
-    f2 *slot = reinterpret_cast<f2 *>(slots + wp * kN3SlotBytes);
+    f2 *slot = reinterpret_cast<f2 *>(slots + wp * kN3SlotBytes);   // one slot per warp pair here (shared memory is full)
+    int nx = 0;
     const int N = a.n_atoms;
     const int n_exp = (NE > 0) ? NE : a.c.n, m_exp = (ME > 0) ? ME : a.c.m;
     const f2 An2 = f2_dup(float(a.c.An));
@@ -507,10 +521,16 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
         }   // this set has pairs in the chunk
         f2 b0 = zero2, b1 = zero2, b2 = zero2;             // set B's sums (binary32, as they travelled)
         if (both) {
-            n3_pair_barrier(wp);
-            if (set) { slot[lane] = g0; slot[32 + lane] = FORCE ? g1 : gfar; if constexpr (FORCE) slot[64 + lane] = g2; }
-            n3_pair_barrier(wp);
-            if (!set) { b0 = slot[lane]; b1 = slot[32 + lane]; if constexpr (FORCE) b2 = slot[64 + lane]; }
+            if (set) {
+                if (nx >= 1) n3_empty_wait(wp);
+                slot[lane] = g0; slot[32 + lane] = FORCE ? g1 : gfar; if constexpr (FORCE) slot[64 + lane] = g2;
+                n3_full_arrive(wp);
+            } else {
+                n3_full_wait(wp);
+                b0 = slot[lane]; b1 = slot[32 + lane]; if constexpr (FORCE) b2 = slot[64 + lane];
+                n3_empty_arrive(wp);
+            }
+            ++nx;
         }
         if (!set) {
             if constexpr (FORCE) {
@@ -543,6 +563,7 @@ __device__ __forceinline__ void n3p_sweep_piece(const N3FArgs &a, const int piec
     }
     __syncthreads();                                       // the next tile's chunk records go into the same memory
     }   // tiles of this CTA's piece
+    if (set && nx >= 1) n3_empty_wait(wp);                 // absorb A's last arrival
     if constexpr (FORCE && ENERGY) {
         esum = warp_sum(esum);                             // over all tiles of the piece
         if (lane == 0) red_e[warp] = esum;
