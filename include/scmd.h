@@ -122,7 +122,7 @@ typedef enum {
     SC_OPT_ATOMS_PER_CTA = 9,     /* cutoff path: consecutive atoms one CTA of the list sweeps
                                      works through (rounded to the warp layout)                  */
     SC_OPT_NEWTON3 = 10,          /* all pairs, either precision, 2048 <= N <= 262144 (the range in which
-                                     sc_workspace_bytes includes the ~N^2 / 8 bytes of partial
+                                     sc_workspace_bytes includes the ~N^2 / 16 bytes of partial
                                      sums): evaluate every unordered pair once and add its term to
                                      both atoms.  0: library default (on from N = 2961), 1: on,
                                      2: off = the one-sided sweeps                               */
@@ -159,7 +159,7 @@ typedef struct {
                                      1.3 x the fcc number density 4 / a^3 inside the list sphere, which a system denser
                                      than that overflows (SC_ERR_CAPACITY) -- then create the context again with the
                                      max_neighbours sc_stats reported, plus headroom                                    */
-    int32_t newton3_storage;      /* all pairs: 0 = carve the ~N^2 / 8 bytes of partial sums of the Newton's-third-law
+    int32_t newton3_storage;      /* all pairs: 0 = carve the ~N^2 / 16 bytes of partial sums of the Newton's-third-law
                                      sweeps where they apply (2048 <= N <= 262144), 2 = never (SC_OPT_NEWTON3 is then
                                      fixed at 2: one-sided sweeps, O(N) workspace)                                      */
     int32_t row_begin, row_end;   /* all pairs over several GPUs: this context is ONE RANK of a row split

@@ -2,22 +2,24 @@
 // evaluated once and its term is added to both atoms, 13 / 25 FP64 instructions per unordered pair instead of
 // 2 x 11 / 2 x 22 for the two ordered pairs (PAPER.md:127 has one particle per thread and full N^2).
 //
-// Decomposition.  A CTA (12 warps) owns a block of RB = 32 * IT rows i; lane t of EVERY warp holds rows
-// row0 + k * 32 + t (k < IT) in registers.  The j range is cut into chunks of 32 atoms; the block takes the chunks
-// from its own first chunk to the end (the upper triangle), warp w every 12th of them.  For a chunk, lane t loads
+// Decomposition.  A row block is RB = 32 * IT rows i; lane t of every warp that works on it holds rows
+// row0 + k * 32 + t (k < IT) in registers.  (A CTA of 12 warps holds a PAIR of row blocks, six warps each: see
+// n3_sweep_piece.)  The j range is cut into chunks of 32 atoms; a block takes the chunks from its own first chunk to the
+// end (the upper triangle), its warps in turn.  For a chunk, lane t loads
 // atom j = 32 c + t and the warp ROTATES the chunk through its lanes: 32 steps, in each of which a lane evaluates
 // its IT rows against the j record it currently holds and then passes the record -- together with the reaction
 // sums accumulated on it so far -- to the next lane by warp shuffles.  After 32 steps every record is back in its
-// home lane carrying the sum over the warp's 32 * IT rows, and is stored as this block's partial for j.  No atomics,
-// no shared memory in the loop; rows i accumulate in registers as in the one-sided sweeps.
+// home lane carrying the sum over the warp's 32 * IT rows, and is stored as the block's partial for j (after the sums
+// of the pair's second row block have been added).  No atomics; rows i accumulate in registers as in the one-sided
+// sweeps.  (Since round 2 the records of the chunk sit in shared memory and only the sums travel: see the kernel.)
 //
 // Diagonal: in the chunks that overlap the block's own rows a pair counts iff j > i (by index); pairs with i or j
 // beyond N are evaluated on dummy records 1e100 away, whose terms underflow to exact zeros.
 //
-// Sums.  part[b][j] (j >= first row of block b: triangular storage) holds block b's reaction sums, self[i] the
-// row sums of i's own block, one per j segment; a finalize kernel adds self[0..][i] + part[0..block(i)][i] in that fixed order, so the
-// result is bit-reproducible.  Storage: ~N^2 / (2 RB) records of 32 bytes (0.54 GB at N = 65536), which is what
-// limits the variant to N <= 262144 (8.6 GB there; kN3MaxAtoms in scmd.cu).
+// Sums.  part[b][j] (j >= first row of PAIR block b: triangular storage) holds the pair block's reaction sums, self[i]
+// the row sums of i's own block, one per tile; a finalize kernel adds self[0..][i] + part[0..block(i)][i] in that fixed
+// order, so the result is bit-reproducible.  Storage: ~N^2 / (4 RB) records of 32 bytes (0.27 GB at N = 65536, 4.3 GB at
+// 262144, the top of the range: kN3MaxAtoms in scmd.cu).
 #pragma once
 #ifndef SCMD_N3P_UNROLL
 #define SCMD_N3P_UNROLL 4      // rotation steps unrolled in the mixed sweeps: 2 x this
@@ -86,7 +88,7 @@ __device__ __forceinline__ double rsqrt_fast_lo(double x, double dead) {
 // the first RB rows in registers (set A), warps NW/2 .. NW - 1 the second RB rows (set B); warp p of A and warp p of B
 // rotate the SAME chunk, each against its own rows, B hands its reaction sums to A through shared memory (two named
 // barriers of 64 threads per chunk) and A stores ONE partial record per (pair block, j): N^2 / 512 records instead of
-// N^2 / 256 -- half the workspace (4.3 GB at N = 262144), half the DRAM writes of sweep 2 (241 MB at N = 65536) and half
+// N^2 / 256 -- half the workspace (4.3 GB at N = 262144), half the DRAM writes of sweep 2 (215 MB at N = 65536) and half
 // the reads of the finalize.  Set B has no pairs in the first IT chunks of the pair block (they are below its diagonal).
 // The hand-over is a producer / consumer pair of named barriers per warp pair (PTX bar.arrive / bar.sync, 64 threads):
 // FULL -- B arrives after writing a slot, A waits before reading it; EMPTY -- A arrives after reading, B waits before it

@@ -175,7 +175,7 @@ int cutoff_max_dim(int64_t N) {
 }
 
 // Newton's-third-law all-pairs sweeps (sc_allpairs_n3.cuh): sizes for which their partial sums are carved
-constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (8.6 GB at the top)
+constexpr int64_t kN3MinAtoms = 2048, kN3MaxAtoms = 262144;   // workspace carved in this range (4.3 GB at the top)
 constexpr int64_t kN3DefaultMinAtoms = 2961, kN3DefaultMinAtomsMixed = 2961;   // measured crossovers
 constexpr int kN3RowsPerThread = 4;     // 2 rows per lane (twice the chunks, half as long) measured in the step loop for small
                                         // clusters, where the triangle has fewer chunks than the chip has warps: N = 2057 23.4
@@ -843,7 +843,7 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
 // ---------------------------------------------------------------------------------------------
 // Measured against the four launches per step (300-step calls, us per step): N = 4096 39.0 / 45.1, N = 8000 100.2 / 103.1,
 // mixed 82.6 / 87.9, N = 16384 353.7 / 352.6, N = 32768 1373 / 1328: beyond ~12000 atoms the finalize phases, which read
-// N^2 / 256 partial records with 8 warps per SM, cost more than the stand-alone finalize kernels (64 warps per SM) save.
+// N^2 / 512 partial records with 8 warps per SM, cost more than the stand-alone finalize kernels (64 warps per SM) save.
 constexpr int64_t kN3LoopMaxAtoms = 12288;
 
 bool n3_loop_wanted(const sc_ctx *c, int thermo) {
