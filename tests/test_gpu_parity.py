@@ -136,6 +136,25 @@ def test_newton3_plans(scmd, oracle_ld, n_atoms, pieces, precision):
     sc.close()
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_newton3_six_warp_ctas(scmd, oracle_ld, precision):
+    """SC_OPT_WARPS_PER_CTA <= 6 with the Newton's-third-law sweeps: CTAs of six warps (two row sets of three warps, the
+    pair hand-over on three pairs of named barriers), two CTAs per SM."""
+    import torch
+    w = W.fcc_cluster(7003, 1500.0, seed=88)
+    rho_o, f_o, (e_o, _, _) = oracle_ld.energy_forces(w.pos, oracle_ld.params())
+    sc = scmd.SuttonChen(w.n_atoms, precision=precision)
+    sc.sc_set_option(scmd.SC_OPT_NEWTON3, 1)
+    sc.sc_set_option(scmd.SC_OPT_WARPS_PER_CTA, 6)
+    sc.sc_set_state(torch.as_tensor(w.pos, device="cuda"))
+    rho, f, e = sc.sc_density().cpu().numpy(), sc.sc_forces().cpu().numpy(), sc.sc_energy()
+    sc.close()
+    tol = (RHO_TOL, FORCE_TOL, ENERGY_TOL) if precision == 0 else (2e-6, 1e-5, 1e-7)
+    assert np.max(np.abs(rho - rho_o) / rho_o) < tol[0]
+    assert rel_l2(f, f_o) < tol[1]
+    assert rel(e, e_o) < tol[2]
+
+
 def test_newton3_trajectory(scmd, oracle_ld):
     """100 velocity-Verlet steps at N = 8192 through the Newton's-third-law sweeps: positions within 1e-8 A."""
     import torch
