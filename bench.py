@@ -307,7 +307,7 @@ def measure(scmd, spec: Spec, steps: int, warmup: int, rank: int, world: int, de
     # In the one-launch loop (small all-pairs clusters, csrc/sc_small.cuh) a bench step is one sc_step call of
     # MD_PER_CALL MD steps and the roofline kernel is the loop itself.
     # Where the library runs all steps of a call in one launch (SC_INFO_ONE_LAUNCH: the one-sided loop for small
-    # clusters, the Newton's-third-law loop up to 12288 atoms) a bench step is one sc_step call of 100 MD steps and the
+    # clusters, the Newton's-third-law loop up to 16384 atoms) a bench step is one sc_step call of 100 MD steps and the
     # roofline kernel is the loop itself: the WHOLE step (both sweeps, finalize phases, integrator, grid barriers) is
     # set against the sweeps' instruction counts.
     step_path = sc.sc_get_option(scmd.SC_INFO_STEP_PATH)

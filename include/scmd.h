@@ -107,9 +107,9 @@ typedef enum {
                                      launch with grid barriers between the phases of a step.  Two
                                      such loops exist: the one-sided one with the records staged in
                                      shared memory (N <= 6144, any thermostat), and the one through
-                                     the Newton's-third-law sweeps (NVE and rescale steps, 2048 <= N <= 12288).
+                                     the Newton's-third-law sweeps (NVE and rescale steps, 2048 <= N <= 16384).
                                      0: library default (the first for N <= 2960, the second for NVE and
-                                     rescale steps where SC_OPT_NEWTON3 applies and N <= 12288: the measured
+                                     rescale steps where SC_OPT_NEWTON3 applies and N <= 16384: the measured
                                      crossovers), 1: the first, 2: neither (one launch per sweep
                                      and per integrator stage), 3: never the first.  Off while
                                      sc_profile is on.                                          */

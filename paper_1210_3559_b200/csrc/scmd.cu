@@ -844,7 +844,9 @@ sc_status run_small_steps(sc_ctx *c, double dt, const sc_thermostat *th, int the
 // Measured against the four launches per step (300-step calls, us per step): N = 4096 39.0 / 45.1, N = 8000 100.2 / 103.1,
 // mixed 82.6 / 87.9, N = 16384 353.7 / 352.6, N = 32768 1373 / 1328: beyond ~12000 atoms the finalize phases, which read
 // N^2 / 512 partial records with 8 warps per SM, cost more than the stand-alone finalize kernels (64 warps per SM) save.
-constexpr int64_t kN3LoopMaxAtoms = 12288;
+// After the pair blocks (finalize phases read half as much): N = 12288 196.8 / 200.4, 14336 262.0 / 264.7, 16384 337.5 / 337.9,
+// 20480 520.7 / 510.4; mixed 16384 248.3 / 250.0, 20480 381.4 / 373.0.
+constexpr int64_t kN3LoopMaxAtoms = 16384;
 
 bool n3_loop_wanted(const sc_ctx *c, int thermo) {
     return (thermo == SC_THERMO_NONE || thermo == SC_THERMO_RESCALE) && n3_wanted(c) && !c->profile && c->opt_persistent != 2 && c->n3_barrier &&

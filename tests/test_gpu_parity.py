@@ -244,8 +244,8 @@ def test_step_path_queries(scmd):
     """SC_INFO_STEP_PATH / SC_INFO_ONE_LAUNCH tell which kernels a context runs as configured (bench.py asks them
     instead of repeating the library's thresholds)."""
     cases = [  # (N, kwargs, options, path, one_launch)
-        (147, {}, {}, 2, 1), (2960, {}, {}, 2, 1), (2961, {}, {}, 1, 1), (12288, dict(precision=1), {}, 1, 1),
-        (12289, {}, {}, 1, 0), (5003, {}, {scmd.SC_OPT_PERSISTENT: 2}, 1, 0), (5003, {}, {scmd.SC_OPT_NEWTON3: 2}, 0, 0),
+        (147, {}, {}, 2, 1), (2960, {}, {}, 2, 1), (2961, {}, {}, 1, 1), (16384, dict(precision=1), {}, 1, 1),
+        (16385, {}, {}, 1, 0), (5003, {}, {scmd.SC_OPT_PERSISTENT: 2}, 1, 0), (5003, {}, {scmd.SC_OPT_NEWTON3: 2}, 0, 0),
         (5003, {}, {scmd.SC_OPT_NEWTON3_PIECES: -1}, 1, 0), (1415, {}, {scmd.SC_OPT_PERSISTENT: 2}, 0, 0),
         (3001, dict(r_cut=8.0, skin=1.0), {}, 3, 0),
     ]

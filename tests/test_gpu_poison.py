@@ -17,7 +17,7 @@ pytestmark = pytest.mark.gpu
     (4101, {}, {}), (2051, {}, {"SC_OPT_NEWTON3": 1, "SC_OPT_PERSISTENT": 2}),   # Newton's third law: the step loop in one launch / smallest carved size, separate launches
     (2967, {}, {}), (2967, dict(precision=1), {}),                         # ... at its default's lower end (2961), both precisions
     (4611, dict(precision=1), {}), (3001, dict(precision=1), {"SC_OPT_NEWTON3": 2}),   # mixed: Newton's third law; one-sided packed sweeps
-    (12301, {}, {}),                                                       # just above the one-launch range: four launches per step
+    (16391, {}, {}),                                                       # just above the one-launch range: four launches per step
     (3001, dict(r_cut=8.0, skin=1.0), {}), (3001, dict(r_cut=8.0, skin=1.0, precision=1), {}),
 ])
 def test_poisoned_workspace(scmd, oracle_ld, n_atoms, kw, opts):
