@@ -124,47 +124,6 @@ __device__ __forceinline__ double warp0_sum_partials(const double *part, int n) 
     return s;
 }
 
-// one term of sweep 1: r^-m (self == true: the reciprocal is replaced by 0, so the term is exactly 0)
-template <int ME>
-__device__ __forceinline__ double small_density_term(const double4 &pi, const double4 &p, bool self, int m_exp) {
-    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
-    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-    r2 = self ? 1.0 : r2;
-    if constexpr (ME > 0 && ME % 2 == 0) {
-        const double w = self ? 0.0 : rcp_fast(r2);
-        return ipow_c<ME / 2>(w);
-    } else {
-        const double y = self ? 0.0 : rsqrt_fast(r2);
-        return (ME > 0) ? ipow_c<(ME > 0 ? ME : 1)>(y) : ipow_rt(y, m_exp);
-    }
-}
-
-// one term of sweep 2 added into (fx, fy, fz, sum r^-n)
-template <int NE, int ME>
-__device__ __forceinline__ void small_force_term(const double4 &pi, const double4 &p, bool self, double An, int n_exp,
-                                                 int m_exp, double (&acc)[4]) {
-    const double dx = pi.x - p.x, dy = pi.y - p.y, dz = pi.z - p.z;
-    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-    r2 = self ? 1.0 : r2;
-    const double y = self ? 0.0 : rsqrt_fast(r2);          // self: every power below is exactly 0
-    const double w = y * y;
-    const double ss = pi.w + p.w;
-    double coef, pn;
-    if constexpr (NE == 9 && ME == 6) {
-        const double w2 = w * w, w4 = w2 * w2, y3 = w * y;
-        coef = w4 * fma(An, y3, -ss);
-        pn = w4 * y;
-    } else {
-        const double pm = (ME > 0) ? ipow_c<ME>(y) : ipow_rt(y, m_exp);
-        pn = (NE > 0) ? ipow_c<NE>(y) : ipow_rt(y, n_exp);
-        coef = w * fma(An, pn, -ss * pm);
-    }
-    acc[0] = fma(coef, dx, acc[0]);
-    acc[1] = fma(coef, dy, acc[1]);
-    acc[2] = fma(coef, dz, acc[2]);
-    acc[3] += pn;
-}
-
 template <class Rec> __device__ __forceinline__ Rec small_load(const unsigned char *p);
 template <> __device__ __forceinline__ double4 small_load<double4>(const unsigned char *p) {
     const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 128);
@@ -265,44 +224,6 @@ __device__ __forceinline__ void small_sweep2(const unsigned char *sm, int N, int
 // staged record: x = xh + xl with xh = fl32(x), xl = fl32(x - xh), so that (xh_i - xh_j) + (xl_i - xl_j) keeps the
 // accuracy of a binary64 subtraction to within binary32 rounding of the DIFFERENCE (as in allpairs32_kernel)
 using SmallRecF = RecF;
-template <int ME>
-__device__ __forceinline__ float small_density_term_f(const SmallRecF &pi, const SmallRecF &p, bool self, int m_exp) {
-    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
-    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    r2 = self ? 1.0f : r2;
-    if constexpr (ME > 0 && ME % 2 == 0) {
-        const float w = self ? 0.f : rcp_fast_f(r2);
-        return ipow_cf<ME / 2>(w);
-    } else {
-        const float y = self ? 0.f : rsqrt_fast_f(r2);
-        return (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
-    }
-}
-template <int NE, int ME>
-__device__ __forceinline__ void small_force_term_f(const SmallRecF &pi, const SmallRecF &p, bool self, float Anf, int n_exp,
-                                                   int m_exp, float (&acc)[4]) {
-    const float dx = (pi.xh - p.xh) + (pi.xl - p.xl), dy = (pi.yh - p.yh) + (pi.yl - p.yl), dz = (pi.zh - p.zh) + (pi.zl - p.zl);
-    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    r2 = self ? 1.0f : r2;
-    const float y = self ? 0.f : rsqrt_fast_f(r2);
-    const float w = y * y;
-    const float ss = pi.s + p.s;
-    float coef, pn;
-    if constexpr (NE == 9 && ME == 6) {
-        const float w2 = w * w, w4 = w2 * w2, y3 = w * y;
-        coef = w4 * fmaf(Anf, y3, -ss);
-        pn = w4 * y;
-    } else {
-        const float pm = (ME > 0) ? ipow_cf<(ME > 0 ? ME : 1)>(y) : ipow_rtf(y, m_exp);
-        pn = (NE > 0) ? ipow_cf<(NE > 0 ? NE : 1)>(y) : ipow_rtf(y, n_exp);
-        coef = w * fmaf(Anf, pn, -ss * pm);
-    }
-    acc[0] = fmaf(coef, dx, acc[0]);
-    acc[1] = fmaf(coef, dy, acc[1]);
-    acc[2] = fmaf(coef, dz, acc[2]);
-    acc[3] += pn;
-}
-
 // Lean binary32 terms: the self term by one select on the MUFU seed (a zero seed makes every later product an exact 0:
 // the Newton step forms 0 x 0, never 0 x inf), sums by fused multiply-adds; ENERGY as in the FP64 form
 template <int ME>
