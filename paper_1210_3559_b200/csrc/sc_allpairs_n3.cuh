@@ -64,7 +64,6 @@ inline size_t n3_part_records(int n_atoms, int rb) {
 __device__ __forceinline__ double rot1(double v) {   // as a 64-bit integer: two SHFL on the register pair, no repacking
     return __longlong_as_double(__shfl_sync(0xffffffffu, __double_as_longlong(v), (threadIdx.x + 1) & 31));
 }
-__device__ __forceinline__ int rot1(int v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
 // The MUFU seeds of 1 / x and x^-1/2 come as a high word; the library form (sc_device.cuh) completes them with a ZERO low
 // word, one move per seed (4 of the 116 instructions of a rotation step).  Any low word will do: it perturbs the seed by
 // < 2^-20 relative, about the seed's own error, and the cubic refinement leaves (2 e0)^3 ~ 2^-57 of it.  Here the low
@@ -311,7 +310,6 @@ __global__ void __launch_bounds__(kN3Warps * 32, 1) allpairs_n3_kernel(const N3A
 // split).  The pair-energy sum of sweep 2 (r^-9) needs the same split, at 10 A: unsplit it lost 1e-7 of the energy of
 // the N = 8000 liquid droplet (a lane's sum holds a nearest-neighbour term with probability ~1500 / N); the force
 // terms have the same loss, far inside their 1e-5 tolerance.
-__device__ __forceinline__ float rot1(float v) { return __shfl_sync(0xffffffffu, v, (threadIdx.x + 1) & 31); }
 
 struct N3FArgs {
     const RecF *xfr;        // [N] split binary32 records
